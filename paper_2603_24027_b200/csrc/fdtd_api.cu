@@ -1,0 +1,751 @@
+// fdtd_api.cu — host side of libfdtd_b200: the C ABI declared in include/fdtd.h.
+// Argument validation, workspace carving, CPML tables, launch sequencing (R2 forward order, R9 reverse
+// order).  Every step of the path runs in the kernels of fdtd_stencil.cuh / fdtd_store.cuh; there is no CPU path.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/fdtd.h"
+#include "fdtd_stencil.cuh"
+#include "fdtd_store.cuh"
+
+using namespace fdtd;
+
+namespace {
+
+constexpr int kMaxSources = 128;
+constexpr size_t kAmpStageFloats = 1u << 20;
+constexpr double kC0 = 299792458.0;
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Layout {
+  size_t ce, E[3], H[3], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
+  size_t lE[3], lH[3], lpsiE[2][3][2], lpsiH[2][3][2], acc;
+  size_t eps_own, mon_stage, grad_stage, amp_stage;
+  size_t store_cap;
+  int slots_cap;
+  size_t total;
+};
+
+}  // namespace
+
+struct fdtd_sim {
+  int n[3] = {0, 0, 0};
+  int P = 0;
+  double dx = 0, dt = 0, Sd = 0;
+  cudaStream_t stream = nullptr;
+  mutable std::string err;
+  const float* eps_dev = nullptr;
+  double cpml[4] = {0.8, 1.0, 0.01, 3.0};
+  bool has_design = false;
+  int dlo[3] = {0, 0, 0}, dhi[3] = {0, 0, 0};
+  bool has_mon = false;
+  BoxDev mon{};
+  float* mon_rec = nullptr;
+  // workspace
+  char* ws = nullptr;
+  size_t ws_bytes = 0;
+  int max_nsteps = 0, max_k = 1, max_dtype = 0;
+  unsigned flags = 0;
+  Layout L{};
+  Dev d{};
+  StoreDev st{};
+  std::vector<float> tables_host;
+  std::vector<SrcDev> src_host;
+  std::vector<float> waves_host;
+  int nsrc = 0;
+  int V = 1;
+  int xch = 8;
+  // run state
+  int nsteps = 0, k = 1, dtype = 0;
+  bool forward_done = false, state_final = false;
+  bool use_graphs = true;
+  unsigned long long launches = 0;
+};
+
+namespace {
+
+fdtd_status fail(const fdtd_sim* s, fdtd_status code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (s) s->err = buf;
+  return code;
+}
+#define CUDA_TRY(s, call)                                                                          \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+long long face_size(const fdtd_sim* s, int f) {
+  const int a = f / 2;
+  return (long long)(s->n[(a + 1) % 3] - 2 * s->P) * (s->n[(a + 2) % 3] - 2 * s->P);
+}
+long long slot_values(const fdtd_sim* s) {
+  long long v = 0;
+  for (int f = 0; f < 6; ++f) v += 6 * face_size(s, f);
+  return v;
+}
+int elem_bytes_host(int dt) { return dt == DT_F32 ? 4 : (dt == DT_E4M3S ? 1 : 2); }
+int num_slots(int nsteps, int k) { return nsteps / k + 1 + (nsteps % k ? 1 : 0); }
+long long psi_elems(const fdtd_sim* s, int a) { return 2LL * s->P * s->n[(a + 1) % 3] * s->n[(a + 2) % 3]; }
+long long design_cells(const fdtd_sim* s) {
+  return s->has_design ? (long long)(s->dhi[0] - s->dlo[0]) * (s->dhi[1] - s->dlo[1]) * (s->dhi[2] - s->dlo[2]) : 0;
+}
+long long mon_floats_per_step(const fdtd_sim* s) {
+  return s->has_mon ? (long long)s->mon.ncomp * (s->mon.hi[0] - s->mon.lo[0]) * (s->mon.hi[1] - s->mon.lo[1]) *
+                          (s->mon.hi[2] - s->mon.lo[2])
+                    : 0;
+}
+
+Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned flags) {
+  Layout L{};
+  size_t o = 0;
+  const size_t N = (size_t)s->n[0] * s->n[1] * s->n[2];
+  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + std::max<size_t>(bytes, 4)); return r; };
+  L.ce = take(N * 4);
+  for (int c = 0; c < 3; ++c) L.E[c] = take(N * 4);
+  for (int c = 0; c < 3; ++c) L.H[c] = take(N * 4);
+  for (int c = 0; c < 3; ++c)
+    for (int t = 0; t < 2; ++t) L.psiE[c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
+  for (int c = 0; c < 3; ++c)
+    for (int t = 0; t < 2; ++t) L.psiH[c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
+  L.tab = take((size_t)6 * (s->n[0] + s->n[1] + s->n[2]) * 4);
+  L.step = take(16);
+  L.scratch = take(16);
+  L.srcdesc = take(sizeof(SrcDev) * kMaxSources);
+  L.waves = take((size_t)kMaxSources * nsteps * 4);
+  const int slots = num_slots(nsteps, k);
+  L.slots_cap = slots;
+  L.store_cap = (size_t)slots * slot_values(s) * elem_bytes_host(dtype);
+  L.store = take(L.store_cap);
+  L.scales = take((size_t)slots * 36 * 4);
+  L.amax = take((size_t)slots * 36 * 4);
+  if (flags & FDTD_WS_REVERSE) {
+    for (int c = 0; c < 3; ++c) L.lE[c] = take(N * 4);
+    for (int c = 0; c < 3; ++c) L.lH[c] = take(N * 4);
+    for (int b = 0; b < 2; ++b)
+      for (int c = 0; c < 3; ++c)
+        for (int t = 0; t < 2; ++t) {
+          L.lpsiE[b][c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
+          L.lpsiH[b][c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
+        }
+    L.acc = take((size_t)design_cells(s) * 8);
+  }
+  if (flags & FDTD_WS_HOST_IO) {
+    L.eps_own = take(N * 4);
+    L.mon_stage = take((size_t)mon_floats_per_step(s) * nsteps * 4);
+    L.grad_stage = take((size_t)design_cells(s) * 4);
+    L.amp_stage = take(kAmpStageFloats * 4);
+  }
+  L.total = o;
+  return L;
+}
+
+// CPML coefficient tables (ref. 17; constants = DESIGN.md R5): per axis bE cE kE bH cH kH.
+// E-type terms sit at integer depth, H-type terms at half-integer depth.  b = exp(-(sigma/kappa + alpha)),
+// c = sigma/(sigma*kappa + kappa^2*alpha)*(b - 1), k = 1/kappa - 1; sigma, alpha per time step (dimensionless).
+void build_tables(fdtd_sim* s) {
+  const int tot = s->n[0] + s->n[1] + s->n[2];
+  s->tables_host.assign((size_t)6 * tot, 0.0f);
+  const int P = s->P;
+  if (P == 0) return;
+  const double sf = s->cpml[0], kmax = s->cpml[1], amax = s->cpml[2], gm = s->cpml[3];
+  const double S = (double)(float)s->Sd;
+  const double sigma_max = sf * (gm + 1.0) * S;
+  size_t base = 0;
+  for (int a = 0; a < 3; ++a) {
+    const int Na = s->n[a];
+    for (int i = 0; i < Na; ++i) {
+      const double rhoE = std::max(std::max((double)(P - i) / P, (double)(i - (Na - P)) / P), 0.0);
+      const double rhoH = std::max(std::max((P - i - 0.5) / P, (i + 0.5 - (Na - P)) / P), 0.0);
+      for (int h = 0; h < 2; ++h) {
+        const double rho = h ? rhoH : rhoE;
+        double b = 0, c = 0, kk = 0;
+        if (rho > 0) {
+          const double g = std::pow(rho, gm);
+          const double sig = sigma_max * g;
+          const double kap = 1.0 + (kmax - 1.0) * g;
+          const double alp = amax * (1.0 - rho);
+          b = std::exp(-(sig / kap + alp));
+          const double den = sig * kap + kap * kap * alp;
+          c = den > 0 ? sig / den * (b - 1.0) : 0.0;
+          kk = 1.0 / kap - 1.0;
+        }
+        s->tables_host[base + (size_t)(3 * h + 0) * Na + i] = (float)b;
+        s->tables_host[base + (size_t)(3 * h + 1) * Na + i] = (float)c;
+        s->tables_host[base + (size_t)(3 * h + 2) * Na + i] = (float)kk;
+      }
+    }
+    base += (size_t)6 * Na;
+  }
+}
+
+bool box_ok(const int lo[3], const int hi[3], const int inner_lo[3], const int inner_hi[3]) {
+  for (int a = 0; a < 3; ++a)
+    if (lo[a] < inner_lo[a] || hi[a] > inner_hi[a] || hi[a] <= lo[a]) return false;
+  return true;
+}
+bool in_interior(const fdtd_sim* s, const int lo[3], const int hi[3]) {
+  int ilo[3], ihi[3];
+  for (int a = 0; a < 3; ++a) { ilo[a] = s->P; ihi[a] = s->n[a] - s->P; }
+  return box_ok(lo, hi, ilo, ihi);
+}
+bool in_grid(const fdtd_sim* s, const int lo[3], const int hi[3]) {
+  int ilo[3] = {0, 0, 0};
+  return box_ok(lo, hi, ilo, s->n);
+}
+
+dim3 grid_all(const fdtd_sim* s, int zdim) {
+  return dim3((unsigned)((s->n[2] + 32 * s->V - 1) / (32 * s->V)), (unsigned)((s->n[1] + TY - 1) / TY), (unsigned)zdim);
+}
+bool grid_inner(const fdtd_sim* s, dim3* g) {
+  const int P = s->P, V = s->V;
+  const int klo = P + 1, khi = s->n[2] - P - 1, rows = s->n[1] - 2 * P - 2, planes = s->n[0] - 2 * P - 2;
+  if (khi <= klo || rows <= 0 || planes <= 0) return false;
+  const int kg0 = (klo / V) * V;
+  const int groups = (khi - kg0 + V - 1) / V;
+  *g = dim3((unsigned)((groups + 31) / 32), (unsigned)((rows + TY - 1) / TY), (unsigned)planes);
+  return true;
+}
+
+#define LAUNCH(s, kern, grid, block, ...)            \
+  do {                                               \
+    kern<<<grid, block, 0, (s)->stream>>>(__VA_ARGS__); \
+    ++(s)->launches;                                 \
+  } while (0)
+
+void launch_fwd_e(fdtd_sim* s) {
+  const dim3 g = grid_all(s, (s->n[0] + s->xch - 1) / s->xch), b(32, TY);
+  if (s->V == 4) LAUNCH(s, k_fwd_e<4>, g, b, s->d, s->xch);
+  else LAUNCH(s, k_fwd_e<1>, g, b, s->d, s->xch);
+}
+void launch_fwd_h(fdtd_sim* s) {
+  const dim3 g = grid_all(s, (s->n[0] + s->xch - 1) / s->xch), b(32, TY);
+  if (s->V == 4) LAUNCH(s, k_fwd_h<4>, g, b, s->d, s->xch);
+  else LAUNCH(s, k_fwd_h<1>, g, b, s->d, s->xch);
+}
+void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
+  if (s->nsrc == 0) return;
+  long long maxc = 1;
+  for (int i = 0; i < s->nsrc; ++i) {
+    const SrcDev& q = s->src_host[i];
+    maxc = std::max(maxc, (long long)(q.hi[0] - q.lo[0]) * (q.hi[1] - q.lo[1]) * (q.hi[2] - q.lo[2]));
+  }
+  const int threads = maxc >= 128 ? 128 : 32;
+  const dim3 g((unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024), (unsigned)s->nsrc);
+  LAUNCH(s, k_sources, g, threads, s->d, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
+         reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign);
+}
+void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode) {
+  const long long tot = (long long)b.ncomp * (b.hi[0] - b.lo[0]) * (b.hi[1] - b.lo[1]) * (b.hi[2] - b.lo[2]);
+  if (tot <= 0) return;
+  LAUNCH(s, k_box, (unsigned)((tot + 255) / 256), 256, s->d, b, rec, m_base, step_dev, mode);
+}
+void launch_record(fdtd_sim* s, int m_base, const int* step_dev) {
+  const unsigned g = (unsigned)((s->st.slot_values + 255) / 256);
+  switch (s->dtype) {
+    case DT_F32: LAUNCH(s, k_record<DT_F32>, g, 256, s->d, s->st, m_base, step_dev); break;
+    case DT_F16: LAUNCH(s, k_record<DT_F16>, g, 256, s->d, s->st, m_base, step_dev); break;
+    case DT_BF16: LAUNCH(s, k_record<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev); break;
+    default:
+      LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev);
+      LAUNCH(s, k_record<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev);
+  }
+}
+void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp) {
+  const unsigned g = (unsigned)((s->st.cell_off[6] + 255) / 256);
+  switch (s->dtype) {
+    case DT_F32: LAUNCH(s, k_inject<DT_F32>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
+    case DT_F16: LAUNCH(s, k_inject<DT_F16>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
+    case DT_BF16: LAUNCH(s, k_inject<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
+    default: LAUNCH(s, k_inject<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp);
+  }
+}
+
+// One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
+void forward_step(fdtd_sim* s, int m_base, const int* step_dev, bool record) {
+  launch_fwd_e(s);
+  launch_sources(s, m_base, step_dev, 1.0f);
+  launch_fwd_h(s);
+  if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0);
+  if (record) launch_record(s, m_base, step_dev);
+}
+
+// One reverse step m -> m-1 (R9).
+void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
+  const dim3 b(32, TY);
+  if (dmon && s->has_mon) launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
+  dim3 gi;
+  const bool inner = grid_inner(s, &gi);
+  if (inner) {
+    if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
+    else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
+  }
+  const dim3 ga = grid_all(s, s->n[0]);
+  if (s->V == 4) LAUNCH(s, k_adj_h<4>, ga, b, s->d, pb);
+  else LAUNCH(s, k_adj_h<1>, ga, b, s->d, pb);
+  launch_inject(s, m_base, step_dev, 1, interp);
+  launch_sources(s, m_base, step_dev, -1.0f);
+  if (inner) {
+    if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d);
+    else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d);
+  }
+  launch_inject(s, m_base, step_dev, 0, interp);
+  if (s->V == 4) LAUNCH(s, k_adj_e<4>, ga, b, s->d, pb);
+  else LAUNCH(s, k_adj_e<1>, ga, b, s->d, pb);
+}
+
+fdtd_status zero_state(fdtd_sim* s) {
+  const size_t N = (size_t)s->d.N;
+  for (int c = 0; c < 3; ++c) {
+    CUDA_TRY(s, cudaMemsetAsync(s->d.E[c], 0, N * 4, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->d.H[c], 0, N * 4, s->stream));
+    for (int t = 0; t < 2; ++t) {
+      const size_t pe = (size_t)psi_elems(s, (c + 1 + t) % 3) * 4;
+      if (pe) {
+        CUDA_TRY(s, cudaMemsetAsync(s->d.psiE[c][t], 0, pe, s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->d.psiH[c][t], 0, pe, s->stream));
+      }
+    }
+  }
+  s->forward_done = s->state_final = false;
+  return FDTD_OK;
+}
+
+fdtd_status make_ce(fdtd_sim* s) {
+  unsigned* scratch = reinterpret_cast<unsigned*>(s->ws + s->L.scratch);
+  const unsigned init = 0x7f7fffffu;
+  CUDA_TRY(s, cudaMemcpyAsync(scratch, &init, 4, cudaMemcpyHostToDevice, s->stream));
+  LAUNCH(s, k_min_eps, 592, 256, s->eps_dev, s->d.N, scratch);
+  LAUNCH(s, k_make_ce, 1184, 256, s->eps_dev, const_cast<float*>(s->d.ce), s->d.N, s->d.S);
+  unsigned bits = 0;
+  CUDA_TRY(s, cudaMemcpyAsync(&bits, scratch, 4, cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  float mn;
+  std::memcpy(&mn, &bits, 4);
+  if (!(mn >= 1.0f)) return fail(s, FDTD_ERR_INVALID_ARG, "eps must be >= 1 everywhere (min %g)", (double)mn);
+  return FDTD_OK;
+}
+
+fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, bool amp_is_host) {
+  if (nsrc < 0 || nsrc > kMaxSources) return fail(s, FDTD_ERR_INVALID_ARG, "nsrc must be in [0, %d]", kMaxSources);
+  if (nsrc > 0 && !src) return fail(s, FDTD_ERR_INVALID_ARG, "src is NULL");
+  s->src_host.assign(std::max(nsrc, 1), SrcDev{});
+  s->waves_host.assign((size_t)std::max(nsrc, 1) * nsteps, 0.0f);
+  size_t amp_used = 0;
+  float* amp_stage = (s->flags & FDTD_WS_HOST_IO) ? reinterpret_cast<float*>(s->ws + s->L.amp_stage) : nullptr;
+  for (int i = 0; i < nsrc; ++i) {
+    const fdtd_source& q = src[i];
+    if (q.comp < 0 || q.comp > 2) return fail(s, FDTD_ERR_INVALID_ARG, "source %d: comp must be 0..2", i);
+    if (!in_interior(s, q.lo, q.hi)) return fail(s, FDTD_ERR_INVALID_ARG, "source %d: box outside the interior", i);
+    if (!q.wave) return fail(s, FDTD_ERR_INVALID_ARG, "source %d: wave is NULL", i);
+    SrcDev& o = s->src_host[i];
+    o.comp = q.comp;
+    for (int a = 0; a < 3; ++a) { o.lo[a] = q.lo[a]; o.hi[a] = q.hi[a]; }
+    o.wave_off = (long long)i * nsteps;
+    std::memcpy(&s->waves_host[(size_t)i * nsteps], q.wave, (size_t)nsteps * 4);
+    o.amp = q.amp;
+    if (q.amp && amp_is_host) {
+      const size_t cells = (size_t)(q.hi[0] - q.lo[0]) * (q.hi[1] - q.lo[1]) * (q.hi[2] - q.lo[2]);
+      if (!amp_stage || amp_used + cells > kAmpStageFloats)
+        return fail(s, FDTD_ERR_OOM, "source amplitudes exceed the host-io staging area");
+      CUDA_TRY(s, cudaMemcpyAsync(amp_stage + amp_used, q.amp, cells * 4, cudaMemcpyHostToDevice, s->stream));
+      o.amp = amp_stage + amp_used;
+      amp_used += cells;
+    }
+  }
+  s->nsrc = nsrc;
+  if (nsrc > 0) {
+    CUDA_TRY(s, cudaMemcpyAsync(s->ws + s->L.srcdesc, s->src_host.data(), sizeof(SrcDev) * nsrc, cudaMemcpyHostToDevice,
+                                s->stream));
+    CUDA_TRY(s, cudaMemcpyAsync(s->ws + s->L.waves, s->waves_host.data(), (size_t)nsrc * nsteps * 4,
+                                cudaMemcpyHostToDevice, s->stream));
+    // the host vectors are pageable: the copies above have been staged when the calls return
+  }
+  return FDTD_OK;
+}
+
+fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k, bool amp_is_host) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace: call fdtd_set_workspace first");
+  if (nsteps < 1) return fail(s, FDTD_ERR_INVALID_ARG, "nsteps must be >= 1");
+  if (k < 1) return fail(s, FDTD_ERR_INVALID_ARG, "k must be >= 1");
+  if ((int)dt < 0 || (int)dt > 3) return fail(s, FDTD_ERR_INVALID_ARG, "unknown store dtype %d", (int)dt);
+  const int slots = num_slots(nsteps, k);
+  const size_t need = (size_t)slots * slot_values(s) * elem_bytes_host(dt);
+  if (nsteps > s->max_nsteps || slots > s->L.slots_cap || need > s->L.store_cap)
+    return fail(s, FDTD_ERR_OOM, "workspace too small: store needs %zu bytes in %d slots, has %zu in %d (nsteps %d, max %d)",
+                need, slots, s->L.store_cap, s->L.slots_cap, nsteps, s->max_nsteps);
+  s->forward_done = s->state_final = false;
+  fdtd_status r = upload_sources(s, nsteps, src, nsrc, amp_is_host);
+  if (r != FDTD_OK) return r;
+  s->nsteps = nsteps; s->k = k; s->dtype = (int)dt;
+  s->st.nslots = slots; s->st.nsteps = nsteps; s->st.k = k; s->st.dtype = (int)dt;
+  s->st.slot_bytes = (size_t)slot_values(s) * elem_bytes_host(dt);
+  if (dt == FDTD_F8E4M3_SCALED) CUDA_TRY(s, cudaMemsetAsync(s->st.amax, 0, (size_t)slots * 36 * 4, s->stream));
+  launch_record(s, 0, nullptr);                       // state 0 (R10)
+  for (int m = 1; m <= nsteps; ++m) forward_step(s, m, nullptr, m % k == 0 || m == nsteps);
+  CUDA_TRY(s, cudaGetLastError());
+  s->forward_done = s->state_final = true;
+  return FDTD_OK;
+}
+
+fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dmon, fdtd_interp interp, float* grad_dev) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!s->forward_done || !s->state_final) return fail(s, FDTD_ERR_STATE, "fdtd_reverse needs a completed fdtd_forward");
+  if (!(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "workspace was sized without FDTD_WS_REVERSE");
+  if ((int)interp < 0 || (int)interp > 1) return fail(s, FDTD_ERR_INVALID_ARG, "unknown interpolation %d", (int)interp);
+  if (dmon && !s->has_mon) return fail(s, FDTD_ERR_INVALID_ARG, "dL_dmon given but no monitor is set");
+  const size_t N = (size_t)s->d.N;
+  for (int c = 0; c < 3; ++c) {
+    CUDA_TRY(s, cudaMemsetAsync(s->d.lE[c], 0, N * 4, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->d.lH[c], 0, N * 4, s->stream));
+    for (int t = 0; t < 2; ++t) {
+      const size_t pe = (size_t)psi_elems(s, (c + 1 + t) % 3) * 4;
+      for (int b = 0; b < 2 && pe; ++b) {
+        CUDA_TRY(s, cudaMemsetAsync(s->d.lpsiE[b][c][t], 0, pe, s->stream));
+        CUDA_TRY(s, cudaMemsetAsync(s->d.lpsiH[b][c][t], 0, pe, s->stream));
+      }
+    }
+  }
+  if (s->has_design) CUDA_TRY(s, cudaMemsetAsync(s->d.acc, 0, (size_t)design_cells(s) * 8, s->stream));
+  if (fin) {
+    if (!in_grid(s, fin->lo, fin->hi) || !(fin->comp_mask & 63u) || !fin->g_dev)
+      return fail(s, FDTD_ERR_INVALID_ARG, "dL_dfinal: bad box, mask or pointer");
+    BoxDev b{};
+    for (int a = 0; a < 3; ++a) { b.lo[a] = fin->lo[a]; b.hi[a] = fin->hi[a]; }
+    b.mask = fin->comp_mask & 63u;
+    b.ncomp = __builtin_popcount(b.mask);
+    launch_box(s, b, const_cast<float*>(fin->g_dev), 0, nullptr, 3);
+  }
+  s->state_final = false;
+  int pb = 0;
+  for (int m = s->nsteps; m >= 1; --m, pb ^= 1) reverse_step(s, m, nullptr, dmon, (int)interp, pb);
+  if (grad_dev && s->has_design)
+    LAUNCH(s, k_grad_finalize, (unsigned)((design_cells(s) + 255) / 256), 256, s->d, s->eps_dev, grad_dev);
+  CUDA_TRY(s, cudaGetLastError());
+  return FDTD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, double dt, int pml_width, const float* eps_dev,
+                        void* cuda_stream) {
+  if (!out) return FDTD_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (nx < 3 || ny < 3 || nz < 3 || pml_width < 0 || !eps_dev || !(dx > 0) || !(dt > 0)) return FDTD_ERR_INVALID_ARG;
+  if (nx - 2 * pml_width < 2 || ny - 2 * pml_width < 2 || nz - 2 * pml_width < 2) return FDTD_ERR_INVALID_ARG;
+  if ((long long)nx * ny * nz > (1LL << 40)) return FDTD_ERR_INVALID_ARG;
+  const double S = kC0 * dt / dx;
+  if (S > (1.0 / std::sqrt(3.0)) * (1.0 + 1e-9)) return FDTD_ERR_INVALID_ARG;   // PAPER.md:37-39 CFL limit
+  fdtd_sim* s = new (std::nothrow) fdtd_sim();
+  if (!s) return FDTD_ERR_OOM;
+  s->n[0] = nx; s->n[1] = ny; s->n[2] = nz; s->P = pml_width; s->dx = dx; s->dt = dt; s->Sd = S;
+  s->eps_dev = eps_dev;
+  s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  *out = s;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_set_cpml(fdtd_sim* s, double sigma_factor, double kappa_max, double alpha_max, double grade_m) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (s->ws) return fail(s, FDTD_ERR_STATE, "fdtd_set_cpml must precede fdtd_set_workspace");
+  if (sigma_factor < 0 || kappa_max < 1 || alpha_max < 0 || grade_m <= 0) return fail(s, FDTD_ERR_INVALID_ARG, "bad CPML constants");
+  s->cpml[0] = sigma_factor; s->cpml[1] = kappa_max; s->cpml[2] = alpha_max; s->cpml[3] = grade_m;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_set_design(fdtd_sim* s, const int lo[3], const int hi[3]) {
+  if (!s || !lo || !hi) return FDTD_ERR_INVALID_ARG;
+  if (s->ws) return fail(s, FDTD_ERR_STATE, "fdtd_set_design must precede fdtd_set_workspace");
+  if (!in_interior(s, lo, hi)) return fail(s, FDTD_ERR_INVALID_ARG, "design box must lie inside the interior");
+  for (int a = 0; a < 3; ++a) { s->dlo[a] = lo[a]; s->dhi[a] = hi[a]; }
+  s->has_design = true;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_set_monitor(fdtd_sim* s, const int lo[3], const int hi[3], unsigned comp_mask, float* record_dev) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!lo || !hi) { s->has_mon = false; s->mon_rec = nullptr; return FDTD_OK; }
+  if (!in_grid(s, lo, hi) || !(comp_mask & 63u)) return fail(s, FDTD_ERR_INVALID_ARG, "monitor: bad box or mask");
+  BoxDev b{};
+  for (int a = 0; a < 3; ++a) { b.lo[a] = lo[a]; b.hi[a] = hi[a]; }
+  b.mask = comp_mask & 63u;
+  b.ncomp = __builtin_popcount(b.mask);
+  if (s->ws && (s->flags & FDTD_WS_HOST_IO) && s->has_mon &&
+      (long long)b.ncomp * (hi[0] - lo[0]) * (hi[1] - lo[1]) * (hi[2] - lo[2]) > mon_floats_per_step(s))
+    return fail(s, FDTD_ERR_STATE, "monitor grew after the host-io workspace was sized");
+  s->mon = b;
+  s->has_mon = true;
+  s->mon_rec = record_dev;
+  return FDTD_OK;
+}
+
+size_t fdtd_workspace_bytes(const fdtd_sim* s, int nsteps, fdtd_dtype dt, int k, unsigned flags) {
+  if (!s || nsteps < 1 || k < 1 || (int)dt < 0 || (int)dt > 3) return 0;
+  return make_layout(s, nsteps, (int)dt, k, flags).total;
+}
+
+fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nsteps, fdtd_dtype dt, int k, unsigned flags) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!ws_dev || nsteps < 1 || k < 1 || (int)dt < 0 || (int)dt > 3) return fail(s, FDTD_ERR_INVALID_ARG, "bad workspace arguments");
+  if (reinterpret_cast<uintptr_t>(ws_dev) % 256) return fail(s, FDTD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+  const Layout L = make_layout(s, nsteps, (int)dt, k, flags);
+  if (bytes < L.total) return fail(s, FDTD_ERR_OOM, "workspace too small: need %zu bytes, got %zu", L.total, bytes);
+  s->ws = static_cast<char*>(ws_dev);
+  s->ws_bytes = bytes; s->L = L; s->flags = flags;
+  s->max_nsteps = nsteps; s->max_k = k; s->max_dtype = (int)dt;
+  Dev& d = s->d;
+  d = Dev{};
+  for (int a = 0; a < 3; ++a) d.n[a] = s->n[a];
+  d.P = s->P;
+  d.sy = s->n[2];
+  d.sx = (long long)s->n[1] * s->n[2];
+  d.N = (long long)s->n[0] * s->n[1] * s->n[2];
+  d.S = (float)s->Sd;
+  char* w = s->ws;
+  d.ce = reinterpret_cast<float*>(w + L.ce);
+  for (int c = 0; c < 3; ++c) {
+    d.E[c] = reinterpret_cast<float*>(w + L.E[c]);
+    d.H[c] = reinterpret_cast<float*>(w + L.H[c]);
+    for (int t = 0; t < 2; ++t) {
+      d.psiE[c][t] = reinterpret_cast<float*>(w + L.psiE[c][t]);
+      d.psiH[c][t] = reinterpret_cast<float*>(w + L.psiH[c][t]);
+    }
+  }
+  size_t base = 0;
+  for (int a = 0; a < 3; ++a) {
+    for (int t = 0; t < 6; ++t) d.tab[a][t] = reinterpret_cast<float*>(w + L.tab) + base + (size_t)t * s->n[a];
+    base += (size_t)6 * s->n[a];
+  }
+  if (flags & FDTD_WS_REVERSE) {
+    for (int c = 0; c < 3; ++c) {
+      d.lE[c] = reinterpret_cast<float*>(w + L.lE[c]);
+      d.lH[c] = reinterpret_cast<float*>(w + L.lH[c]);
+      for (int b = 0; b < 2; ++b)
+        for (int t = 0; t < 2; ++t) {
+          d.lpsiE[b][c][t] = reinterpret_cast<float*>(w + L.lpsiE[b][c][t]);
+          d.lpsiH[b][c][t] = reinterpret_cast<float*>(w + L.lpsiH[b][c][t]);
+        }
+    }
+    d.acc = reinterpret_cast<double*>(w + L.acc);
+  }
+  d.has_design = s->has_design ? 1 : 0;
+  for (int a = 0; a < 3; ++a) { d.dlo[a] = s->dlo[a]; d.dhi[a] = s->dhi[a]; }
+  // store geometry
+  StoreDev& st = s->st;
+  st = StoreDev{};
+  st.base = w + L.store;
+  st.scales = reinterpret_cast<float*>(w + L.scales);
+  st.amax = reinterpret_cast<unsigned*>(w + L.amax);
+  st.slot_values = slot_values(s);
+  st.val_off[0] = st.cell_off[0] = 0;
+  for (int f = 0; f < 6; ++f) {
+    const int a = f / 2;
+    const int b0 = a == 0 ? 1 : 0, b1 = a == 2 ? 1 : 2;
+    st.du[f] = s->n[b0] - 2 * s->P;
+    st.dv[f] = s->n[b1] - 2 * s->P;
+    st.val_off[f + 1] = st.val_off[f] + 6 * face_size(s, f);
+    st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
+  }
+  s->V = (s->n[2] % 4 == 0 && s->P % 4 == 0) ? 4 : 1;
+  {
+    // x chunk per block of the marching forward kernels: enough blocks to fill 148 SMs several times over
+    const long long gxy = (long long)((s->n[2] + 32 * s->V - 1) / (32 * s->V)) * ((s->n[1] + TY - 1) / TY);
+    long long chunks = std::max<long long>(1, (148LL * 8 + gxy - 1) / gxy);
+    int xch = (int)std::max<long long>(4, (s->n[0] + chunks - 1) / chunks);
+    if (const char* e = std::getenv("FDTD_XCH")) xch = std::max(1, atoi(e));
+    s->xch = std::min(xch, s->n[0]);
+  }
+  build_tables(s);
+  CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
+  CUDA_TRY(s, cudaMemsetAsync(w + L.step, 0, 16, s->stream));
+  fdtd_status r = make_ce(s);
+  if (r != FDTD_OK) { s->ws = nullptr; return r; }
+  return zero_state(s);
+}
+
+fdtd_status fdtd_set_eps(fdtd_sim* s, const float* eps_dev) {
+  if (!s || !eps_dev) return FDTD_ERR_INVALID_ARG;
+  s->eps_dev = eps_dev;
+  if (!s->ws) return FDTD_OK;
+  fdtd_status r = make_ce(s);
+  if (r != FDTD_OK) return r;
+  return zero_state(s);
+}
+
+fdtd_status fdtd_reset(fdtd_sim* s) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
+  return zero_state(s);
+}
+
+fdtd_status fdtd_set_graphs(fdtd_sim* s, int enabled) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  s->use_graphs = enabled != 0;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_forward(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k) {
+  return forward_impl(s, nsteps, src, nsrc, dt, k, false);
+}
+
+fdtd_status fdtd_reverse(fdtd_sim* s, const fdtd_cotangent* fin, const float* dmon, fdtd_interp interp, float* grad_dev) {
+  return reverse_impl(s, fin, dmon, interp, grad_dev);
+}
+
+size_t fdtd_store_bytes(const fdtd_sim* s) {
+  if (!s || !s->forward_done) return 0;
+  return (size_t)s->st.nslots * (s->st.slot_bytes + (s->dtype == DT_E4M3S ? 36 * 4 : 0));
+}
+
+fdtd_status fdtd_get_fields(fdtd_sim* s, float* out_dev) {
+  if (!s || !out_dev) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
+  const size_t N = (size_t)s->d.N;
+  for (int c = 0; c < 3; ++c) {
+    CUDA_TRY(s, cudaMemcpyAsync(out_dev + c * N, s->d.E[c], N * 4, cudaMemcpyDeviceToDevice, s->stream));
+    CUDA_TRY(s, cudaMemcpyAsync(out_dev + (3 + c) * N, s->d.H[c], N * 4, cudaMemcpyDeviceToDevice, s->stream));
+  }
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_get_adjoint(fdtd_sim* s, float* out_dev) {
+  if (!s || !out_dev) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws || !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "no reverse workspace");
+  const size_t N = (size_t)s->d.N;
+  for (int c = 0; c < 3; ++c) {
+    CUDA_TRY(s, cudaMemcpyAsync(out_dev + c * N, s->d.lE[c], N * 4, cudaMemcpyDeviceToDevice, s->stream));
+    CUDA_TRY(s, cudaMemcpyAsync(out_dev + (3 + c) * N, s->d.lH[c], N * 4, cudaMemcpyDeviceToDevice, s->stream));
+  }
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_get_box(fdtd_sim* s, const int lo[3], const int hi[3], unsigned comp_mask, float* out_dev) {
+  if (!s || !lo || !hi || !out_dev) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
+  if (!in_grid(s, lo, hi) || !(comp_mask & 63u)) return fail(s, FDTD_ERR_INVALID_ARG, "get_box: bad box or mask");
+  BoxDev b{};
+  for (int a = 0; a < 3; ++a) { b.lo[a] = lo[a]; b.hi[a] = hi[a]; }
+  b.mask = comp_mask & 63u;
+  b.ncomp = __builtin_popcount(b.mask);
+  launch_box(s, b, out_dev, 0, nullptr, 2);
+  CUDA_TRY(s, cudaGetLastError());
+  return FDTD_OK;
+}
+
+int fdtd_num_slots(const fdtd_sim* s) { return (s && s->forward_done) ? s->st.nslots : 0; }
+size_t fdtd_slot_values(const fdtd_sim* s) { return s ? (size_t)slot_values(s) : 0; }
+fdtd_status fdtd_slot_ptr(const fdtd_sim* s, int j, const void** data_dev, const float** scales_dev) {
+  if (!s || !s->forward_done || j < 0 || j >= s->st.nslots) return FDTD_ERR_INVALID_ARG;
+  if (data_dev) *data_dev = s->st.base + (size_t)j * s->st.slot_bytes;
+  if (scales_dev) *scales_dev = s->st.scales + (size_t)j * 36;
+  return FDTD_OK;
+}
+
+// ---- host-buffer variants ----
+fdtd_status fdtd_set_eps_host(fdtd_sim* s, const float* eps_host) {
+  if (!s || !eps_host) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws || !(s->flags & FDTD_WS_HOST_IO)) return fail(s, FDTD_ERR_STATE, "needs a workspace with FDTD_WS_HOST_IO");
+  float* own = reinterpret_cast<float*>(s->ws + s->L.eps_own);
+  CUDA_TRY(s, cudaMemcpyAsync(own, eps_host, (size_t)s->d.N * 4, cudaMemcpyHostToDevice, s->stream));
+  return fdtd_set_eps(s, own);
+}
+
+fdtd_status fdtd_forward_host(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k, float* mon_host) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws || !(s->flags & FDTD_WS_HOST_IO)) return fail(s, FDTD_ERR_STATE, "needs a workspace with FDTD_WS_HOST_IO");
+  float* saved = s->mon_rec;
+  if (s->has_mon) s->mon_rec = reinterpret_cast<float*>(s->ws + s->L.mon_stage);
+  fdtd_status r = forward_impl(s, nsteps, src, nsrc, dt, k, true);
+  if (r == FDTD_OK && s->has_mon && mon_host)
+    r = cudaMemcpyAsync(mon_host, s->mon_rec, (size_t)mon_floats_per_step(s) * nsteps * 4, cudaMemcpyDeviceToHost, s->stream) == cudaSuccess
+            ? FDTD_OK : fail(s, FDTD_ERR_CUDA, "monitor download failed");
+  s->mon_rec = saved;
+  if (r != FDTD_OK) return r;
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_reverse_host(fdtd_sim* s, const float* dmon_host, fdtd_interp interp, float* grad_host) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws || !(s->flags & FDTD_WS_HOST_IO)) return fail(s, FDTD_ERR_STATE, "needs a workspace with FDTD_WS_HOST_IO");
+  float* stage = reinterpret_cast<float*>(s->ws + s->L.mon_stage);
+  if (dmon_host) {
+    if (!s->has_mon) return fail(s, FDTD_ERR_INVALID_ARG, "dmon given but no monitor is set");
+    CUDA_TRY(s, cudaMemcpyAsync(stage, dmon_host, (size_t)mon_floats_per_step(s) * s->nsteps * 4, cudaMemcpyHostToDevice, s->stream));
+  }
+  float* gstage = reinterpret_cast<float*>(s->ws + s->L.grad_stage);
+  fdtd_status r = reverse_impl(s, nullptr, dmon_host ? stage : nullptr, interp, grad_host ? gstage : nullptr);
+  if (r != FDTD_OK) return r;
+  if (grad_host && s->has_design)
+    CUDA_TRY(s, cudaMemcpyAsync(grad_host, gstage, (size_t)design_cells(s) * 4, cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  return FDTD_OK;
+}
+
+// ---- stand-alone codec ----
+fdtd_status fdtd_codec_encode(fdtd_dtype dt, const float* x_dev, size_t n, void* codes_dev, float* scale_dev,
+                              unsigned* scratch_dev, void* cuda_stream) {
+  if (!x_dev || !codes_dev || !scale_dev || (int)dt < 0 || (int)dt > 3) return FDTD_ERR_INVALID_ARG;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
+  switch ((int)dt) {
+    case DT_F32: k_codec_encode<DT_F32><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
+    case DT_F16: k_codec_encode<DT_F16><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
+    case DT_BF16: k_codec_encode<DT_BF16><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
+    default:
+      if (!scratch_dev) return FDTD_ERR_INVALID_ARG;
+      if (cudaMemsetAsync(scratch_dev, 0, 4, st) != cudaSuccess) return FDTD_ERR_CUDA;
+      k_codec_amax<<<g, 256, 0, st>>>(x_dev, n, scratch_dev);
+      k_codec_encode<DT_E4M3S><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, scratch_dev);
+  }
+  return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
+}
+
+fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* const codes_dev[4], const float scales[4],
+                             int num, int den, size_t n, float* out_dev, void* cuda_stream) {
+  if (!codes_dev || !scales || !out_dev || den < 1 || num < 0 || num >= den || (int)dt < 0 || (int)dt > 3) return FDTD_ERR_INVALID_ARG;
+  const int mode = num == 0 ? 0 : ((int)interp == 1 ? 2 : 1);
+  if (!codes_dev[1] || (mode >= 1 && !codes_dev[2]) || (mode == 2 && (!codes_dev[0] || !codes_dev[3]))) return FDTD_ERR_INVALID_ARG;
+  FetchArgs a;
+  for (int j = 0; j < 4; ++j) { a.codes[j] = codes_dev[j]; a.scales[j] = scales[j]; }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
+  switch ((int)dt) {
+    case DT_F32: k_codec_fetch<DT_F32><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
+    case DT_F16: k_codec_fetch<DT_F16><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
+    case DT_BF16: k_codec_fetch<DT_BF16><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
+    default: k_codec_fetch<DT_E4M3S><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev);
+  }
+  return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
+}
+
+fdtd_status fdtd_sync(fdtd_sim* s) {
+  if (!s) return FDTD_ERR_INVALID_ARG;
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  CUDA_TRY(s, cudaGetLastError());
+  return FDTD_OK;
+}
+
+const char* fdtd_last_error(const fdtd_sim* s) { return s ? s->err.c_str() : "null handle"; }
+
+void fdtd_destroy(fdtd_sim* s) { delete s; }
+
+unsigned long long fdtd_launch_count(const fdtd_sim* s) { return s ? s->launches : 0; }
+
+}  // extern "C"

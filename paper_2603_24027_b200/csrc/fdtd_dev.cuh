@@ -1,0 +1,100 @@
+// fdtd_dev.cuh — device-side data layout and small helpers shared by the kernels of libfdtd_b200.
+// Product code (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fdtd {
+
+// Everything a kernel needs to find its data.  Passed by value (__grid_constant__).
+// Layout in HBM: six component-planar f32 arrays [nx][ny][nz], z fastest; ce = S/eps;
+// CPML psi arrays stored compactly (slab cells only): psi?[c][t] belongs to component c and derivative axis
+// a = (c+1+t)%3, its extent along a is 2P (low slab then high slab), the other two extents are the grid's.
+struct Dev {
+  int n[3];
+  int P;
+  long long sx, sy;  // strides of i and j (k stride = 1)
+  long long N;
+  float S;           // Courant number c*dt/dx (eq. 1)
+  float* E[3];
+  float* H[3];
+  const float* ce;   // fl(S * fl(1/eps))
+  float* psiE[3][2];
+  float* psiH[3][2];
+  const float* tab[3][6];  // per axis: bE cE kE bH cH kH (kE = 1/kappa - 1), length n[axis]
+  // adjoint
+  float* lE[3];
+  float* lH[3];
+  float* lpsiE[2][3][2];   // ping-pong buffers [buf][c][t]
+  float* lpsiH[2][3][2];
+  double* acc;             // dL/d(1/eps) / S accumulator over the design box
+  int dlo[3], dhi[3];
+  int has_design;
+};
+
+__device__ __forceinline__ bool in_slab(int i, int n, int P) { return i < P || i >= n - P; }
+__device__ __forceinline__ int slab_s(int i, int n, int P) { return i < P ? i : i - (n - 2 * P); }
+__device__ __forceinline__ long long psi_index(const Dev& d, int a, int i, int j, int k) {
+  const int P2 = 2 * d.P;
+  if (a == 0) return ((long long)slab_s(i, d.n[0], d.P) * d.n[1] + j) * d.n[2] + k;
+  if (a == 1) return ((long long)i * P2 + slab_s(j, d.n[1], d.P)) * d.n[2] + k;
+  return ((long long)i * d.n[1] + j) * P2 + slab_s(k, d.n[2], d.P);
+}
+
+// V consecutive z cells held by one thread (V = 4: one 16-byte access; V = 1: scalar path for odd shapes).
+template <int V> struct VF { float v[V]; };
+template <int V> __device__ __forceinline__ VF<V> ldv(const float* p) {
+  VF<V> r;
+  if constexpr (V == 4) {
+    const float4 t = *reinterpret_cast<const float4*>(p);
+    r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+  } else {
+    r.v[0] = *p;
+  }
+  return r;
+}
+template <int V> __device__ __forceinline__ void stv(float* p, const VF<V>& r) {
+  if constexpr (V == 4) {
+    *reinterpret_cast<float4*>(p) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
+  } else {
+    *p = r.v[0];
+  }
+}
+template <int V> __device__ __forceinline__ VF<V> zerov() {
+  VF<V> r;
+#pragma unroll
+  for (int v = 0; v < V; ++v) r.v[v] = 0.0f;
+  return r;
+}
+
+// One Yee component update with its two CPML terms, in the canonical operation order (R3):
+//   x = fma(coef, d1 - d2, x);  slab a1: psi1 = fma(b1, psi1, c1*d1), x = fma(coef, fma(k1, d1, psi1), x);
+//   slab a2: psi2 = fma(b2, psi2, c2*d2), x = fma(-coef, fma(k2, d2, psi2), x).
+// E half-step: coef = ce.  H half-step: coef = -S.  (Compiled with -fmad=false: every fma here is explicit.)
+__device__ __forceinline__ float yee_update(float x, float coef, float d1, float d2, bool s1, float b1, float c1,
+                                            float k1, float& psi1, bool s2, float b2, float c2, float k2,
+                                            float& psi2) {
+  x = fmaf(coef, d1 - d2, x);
+  if (s1) {
+    const float ps = fmaf(b1, psi1, c1 * d1);
+    psi1 = ps;
+    x = fmaf(coef, fmaf(k1, d1, ps), x);
+  }
+  if (s2) {
+    const float ps = fmaf(b2, psi2, c2 * d2);
+    psi2 = ps;
+    x = fmaf(-coef, fmaf(k2, d2, ps), x);
+  }
+  return x;
+}
+
+// Transposed CPML term: g = cotangent reaching the (d/kappa + psi) sum; returns W = the cotangent of d beyond
+// the plain Yee part, and the new lambda_psi (R9 step 1/5).
+__device__ __forceinline__ float cpml_adjoint_term(float g, float lpsi_old, float bt, float ct, float kt,
+                                                   float& lpsi_new) {
+  const float phi = lpsi_old + g;
+  lpsi_new = bt * phi;
+  return fmaf(ct, phi, kt * g);
+}
+
+}  // namespace fdtd

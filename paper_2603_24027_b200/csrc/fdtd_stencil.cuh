@@ -1,0 +1,658 @@
+// fdtd_stencil.cuh — the bandwidth-bound stencil kernels: forward E / H half-steps with fused CPML, the
+// inverse half-steps of the reverse run, the adjoint half-steps with the transposed CPML, gradient accumulation.
+//
+// Thread mapping (all kernels): block = 32 lanes x TY rows; a lane owns V consecutive z cells (V = 4: 16-byte
+// coalesced accesses, a warp covers 128 contiguous z cells = 512 B), threadIdx.y selects the y row.  The forward
+// kernels march along x over a chunk of planes and carry the x-neighbour plane in registers; y/z neighbours
+// come from L1/L2 (the rows are loaded by the same block in the same iteration).
+#pragma once
+#include "fdtd_dev.cuh"
+
+namespace fdtd {
+
+constexpr int TY = 8;
+
+// ---------------------------------------------------------------------------------------------------------
+// Forward E half-step (SURVEY 8(a) rows A1 + A3):  E_c += ce * (d_a1^- H_b1 - d_a2^- H_b2) + CPML terms,
+// tangential E on the three low PEC walls held at zero.  DESIGN.md R1-R5.
+// ---------------------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_fwd_e(const __grid_constant__ Dev d, int xch) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = blockIdx.y * TY + threadIdx.y;
+  if (k0 >= nz || j >= ny) return;
+  const int i0 = blockIdx.z * xch;
+  const int i1 = min(nx, i0 + xch);
+  const long long sx = d.sx, sy = d.sy;
+
+  bool zs[V];
+  float bz[V], cz[V], kz[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    zs[v] = P > 0 && in_slab(k, nz, P);
+    bz[v] = zs[v] ? __ldg(d.tab[2][0] + k) : 0.0f;
+    cz[v] = zs[v] ? __ldg(d.tab[2][1] + k) : 0.0f;
+    kz[v] = zs[v] ? __ldg(d.tab[2][2] + k) : 0.0f;
+  }
+  const bool ys = P > 0 && in_slab(j, ny, P);
+  const float by = ys ? __ldg(d.tab[1][0] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][1] + j) : 0.0f,
+              ky = ys ? __ldg(d.tab[1][2] + j) : 0.0f;
+
+  long long q = ((long long)i0 * ny + j) * nz + k0;
+  VF<V> pHy = zerov<V>(), pHz = zerov<V>();
+  if (i0 > 0) {
+    pHy = ldv<V>(d.H[1] + q - sx);
+    pHz = ldv<V>(d.H[2] + q - sx);
+  }
+  for (int i = i0; i < i1; ++i, q += sx) {
+    const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+    VF<V> hx_ym = zerov<V>(), hz_ym = zerov<V>();
+    if (j > 0) {
+      hx_ym = ldv<V>(d.H[0] + q - sy);
+      hz_ym = ldv<V>(d.H[2] + q - sy);
+    }
+    float hx_z0 = 0.0f, hy_z0 = 0.0f;
+    if (k0 > 0) {
+      hx_z0 = d.H[0][q - 1];
+      hy_z0 = d.H[1][q - 1];
+    }
+    VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+    const VF<V> ce = ldv<V>(d.ce + q);
+
+    const bool xs = P > 0 && in_slab(i, nx, P);
+    const float bx = xs ? __ldg(d.tab[0][0] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][1] + i) : 0.0f,
+                kx = xs ? __ldg(d.tab[0][2] + i) : 0.0f;
+    // psi_E[c][t]: (0,0)=Ex/y (0,1)=Ex/z (1,0)=Ey/z (1,1)=Ey/x (2,0)=Ez/x (2,1)=Ez/y
+    VF<V> p_ey_x = zerov<V>(), p_ez_x = zerov<V>(), p_ex_y = zerov<V>(), p_ez_y = zerov<V>(),
+          p_ex_z = zerov<V>(), p_ey_z = zerov<V>();
+    long long qx = 0, qy = 0, qz = 0;
+    if (xs) {
+      qx = psi_index(d, 0, i, j, k0);
+      p_ey_x = ldv<V>(d.psiE[1][1] + qx);
+      p_ez_x = ldv<V>(d.psiE[2][0] + qx);
+    }
+    if (ys) {
+      qy = psi_index(d, 1, i, j, k0);
+      p_ex_y = ldv<V>(d.psiE[0][0] + qy);
+      p_ez_y = ldv<V>(d.psiE[2][1] + qy);
+    }
+    if (zs[0]) {
+      qz = psi_index(d, 2, i, j, k0);
+      p_ex_z = ldv<V>(d.psiE[0][1] + qz);
+      p_ey_z = ldv<V>(d.psiE[1][0] + qz);
+    }
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
+      const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+      const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+      // Ex: a1 = y (d_y^- Hz), a2 = z (d_z^- Hy)
+      if (j == 0 || k == 0) ex.v[v] = 0.0f;
+      else ex.v[v] = yee_update(ex.v[v], ce.v[v], hz.v[v] - hz_ym.v[v], hy.v[v] - hy_zm, ys, by, cy, ky, p_ex_y.v[v],
+                                zs[v], bz[v], cz[v], kz[v], p_ex_z.v[v]);
+      // Ey: a1 = z (d_z^- Hx), a2 = x (d_x^- Hz)
+      if (k == 0 || i == 0) ey.v[v] = 0.0f;
+      else ey.v[v] = yee_update(ey.v[v], ce.v[v], hx.v[v] - hx_zm, hz.v[v] - pHz.v[v], zs[v], bz[v], cz[v], kz[v],
+                                p_ey_z.v[v], xs, bx, cx, kx, p_ey_x.v[v]);
+      // Ez: a1 = x (d_x^- Hy), a2 = y (d_y^- Hx)
+      if (i == 0 || j == 0) ez.v[v] = 0.0f;
+      else ez.v[v] = yee_update(ez.v[v], ce.v[v], hy.v[v] - pHy.v[v], hx.v[v] - hx_ym.v[v], xs, bx, cx, kx,
+                                p_ez_x.v[v], ys, by, cy, ky, p_ez_y.v[v]);
+    }
+    stv<V>(d.E[0] + q, ex);
+    stv<V>(d.E[1] + q, ey);
+    stv<V>(d.E[2] + q, ez);
+    if (xs) {
+      stv<V>(d.psiE[1][1] + qx, p_ey_x);
+      stv<V>(d.psiE[2][0] + qx, p_ez_x);
+    }
+    if (ys) {
+      stv<V>(d.psiE[0][0] + qy, p_ex_y);
+      stv<V>(d.psiE[2][1] + qy, p_ez_y);
+    }
+    if (zs[0]) {
+      stv<V>(d.psiE[0][1] + qz, p_ex_z);
+      stv<V>(d.psiE[1][0] + qz, p_ey_z);
+    }
+    pHy = hy;
+    pHz = hz;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Forward H half-step (rows A2 + A4):  H_c -= S * (d_a1^+ E_b1 - d_a2^+ E_b2) + CPML terms; ghost E[n] = 0.
+// ---------------------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_fwd_h(const __grid_constant__ Dev d, int xch) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = blockIdx.y * TY + threadIdx.y;
+  if (k0 >= nz || j >= ny) return;
+  const int i0 = blockIdx.z * xch;
+  const int i1 = min(nx, i0 + xch);
+  const long long sx = d.sx, sy = d.sy;
+  const float mS = -d.S;
+
+  bool zs[V];
+  float bz[V], cz[V], kz[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    zs[v] = P > 0 && in_slab(k, nz, P);
+    bz[v] = zs[v] ? __ldg(d.tab[2][3] + k) : 0.0f;
+    cz[v] = zs[v] ? __ldg(d.tab[2][4] + k) : 0.0f;
+    kz[v] = zs[v] ? __ldg(d.tab[2][5] + k) : 0.0f;
+  }
+  const bool ys = P > 0 && in_slab(j, ny, P);
+  const float by = ys ? __ldg(d.tab[1][3] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][4] + j) : 0.0f,
+              ky = ys ? __ldg(d.tab[1][5] + j) : 0.0f;
+
+  long long q = ((long long)i0 * ny + j) * nz + k0;
+  VF<V> ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);   // plane i (carried), next plane loaded per iteration
+  for (int i = i0; i < i1; ++i, q += sx) {
+    const VF<V> ex = ldv<V>(d.E[0] + q);
+    VF<V> ey_xp = zerov<V>(), ez_xp = zerov<V>();
+    if (i + 1 < nx) {
+      ey_xp = ldv<V>(d.E[1] + q + sx);
+      ez_xp = ldv<V>(d.E[2] + q + sx);
+    }
+    VF<V> ex_yp = zerov<V>(), ez_yp = zerov<V>();
+    if (j + 1 < ny) {
+      ex_yp = ldv<V>(d.E[0] + q + sy);
+      ez_yp = ldv<V>(d.E[2] + q + sy);
+    }
+    float ex_zp = 0.0f, ey_zp = 0.0f;
+    if (k0 + V < nz) {
+      ex_zp = d.E[0][q + V];
+      ey_zp = d.E[1][q + V];
+    }
+    VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+
+    const bool xs = P > 0 && in_slab(i, nx, P);
+    const float bx = xs ? __ldg(d.tab[0][3] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][4] + i) : 0.0f,
+                kx = xs ? __ldg(d.tab[0][5] + i) : 0.0f;
+    // psi_H[c][t]: (0,0)=Hx/y (0,1)=Hx/z (1,0)=Hy/z (1,1)=Hy/x (2,0)=Hz/x (2,1)=Hz/y
+    VF<V> p_hy_x = zerov<V>(), p_hz_x = zerov<V>(), p_hx_y = zerov<V>(), p_hz_y = zerov<V>(),
+          p_hx_z = zerov<V>(), p_hy_z = zerov<V>();
+    long long qx = 0, qy = 0, qz = 0;
+    if (xs) {
+      qx = psi_index(d, 0, i, j, k0);
+      p_hy_x = ldv<V>(d.psiH[1][1] + qx);
+      p_hz_x = ldv<V>(d.psiH[2][0] + qx);
+    }
+    if (ys) {
+      qy = psi_index(d, 1, i, j, k0);
+      p_hx_y = ldv<V>(d.psiH[0][0] + qy);
+      p_hz_y = ldv<V>(d.psiH[2][1] + qy);
+    }
+    if (zs[0]) {
+      qz = psi_index(d, 2, i, j, k0);
+      p_hx_z = ldv<V>(d.psiH[0][1] + qz);
+      p_hy_z = ldv<V>(d.psiH[1][0] + qz);
+    }
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const float ey_zq = v == V - 1 ? ey_zp : ey.v[v < V - 1 ? v + 1 : v];
+      const float ex_zq = v == V - 1 ? ex_zp : ex.v[v < V - 1 ? v + 1 : v];
+      // Hx: a1 = y (d_y^+ Ez), a2 = z (d_z^+ Ey)
+      hx.v[v] = yee_update(hx.v[v], mS, ez_yp.v[v] - ez.v[v], ey_zq - ey.v[v], ys, by, cy, ky, p_hx_y.v[v], zs[v],
+                           bz[v], cz[v], kz[v], p_hx_z.v[v]);
+      // Hy: a1 = z (d_z^+ Ex), a2 = x (d_x^+ Ez)
+      hy.v[v] = yee_update(hy.v[v], mS, ex_zq - ex.v[v], ez_xp.v[v] - ez.v[v], zs[v], bz[v], cz[v], kz[v],
+                           p_hy_z.v[v], xs, bx, cx, kx, p_hy_x.v[v]);
+      // Hz: a1 = x (d_x^+ Ey), a2 = y (d_y^+ Ex)
+      hz.v[v] = yee_update(hz.v[v], mS, ey_xp.v[v] - ey.v[v], ex_yp.v[v] - ex.v[v], xs, bx, cx, kx, p_hz_x.v[v], ys,
+                           by, cy, ky, p_hz_y.v[v]);
+    }
+    stv<V>(d.H[0] + q, hx);
+    stv<V>(d.H[1] + q, hy);
+    stv<V>(d.H[2] + q, hz);
+    if (xs) {
+      stv<V>(d.psiH[1][1] + qx, p_hy_x);
+      stv<V>(d.psiH[2][0] + qx, p_hz_x);
+    }
+    if (ys) {
+      stv<V>(d.psiH[0][0] + qy, p_hx_y);
+      stv<V>(d.psiH[2][1] + qy, p_hz_y);
+    }
+    if (zs[0]) {
+      stv<V>(d.psiH[0][1] + qz, p_hx_z);
+      stv<V>(d.psiH[1][0] + qz, p_hy_z);
+    }
+    ey = ey_xp;
+    ez = ez_xp;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Reverse run, primal reconstruction on the inner interior (row R2).  One thread = one (i, j, z-group);
+// elements outside the inner interior keep their value.  Grid: x = z groups, y = rows from P+1, z = planes
+// from P+1.
+// ---------------------------------------------------------------------------------------------------------
+// inverse of the H half-step:  H^{m-1/2} = H^{m+1/2} + S * curl^+(E^m)
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int klo = P + 1, khi = nz - P - 1;
+  const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = P + 1 + blockIdx.y * TY + threadIdx.y;
+  const int i = P + 1 + blockIdx.z;
+  if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * ny + j) * nz + k0;
+  const float S = d.S;
+  const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  const VF<V> ey_xp = ldv<V>(d.E[1] + q + sx), ez_xp = ldv<V>(d.E[2] + q + sx);
+  const VF<V> ex_yp = ldv<V>(d.E[0] + q + sy), ez_yp = ldv<V>(d.E[2] + q + sy);
+  float ex_zp = 0.0f, ey_zp = 0.0f;
+  if (k0 + V < nz) {
+    ex_zp = d.E[0][q + V];
+    ey_zp = d.E[1][q + V];
+  }
+  VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    if (k < klo || k >= khi) continue;
+    const float ey_zq = v == V - 1 ? ey_zp : ey.v[v < V - 1 ? v + 1 : v];
+    const float ex_zq = v == V - 1 ? ex_zp : ex.v[v < V - 1 ? v + 1 : v];
+    hx.v[v] = fmaf(S, (ez_yp.v[v] - ez.v[v]) - (ey_zq - ey.v[v]), hx.v[v]);
+    hy.v[v] = fmaf(S, (ex_zq - ex.v[v]) - (ez_xp.v[v] - ez.v[v]), hy.v[v]);
+    hz.v[v] = fmaf(S, (ey_xp.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
+  }
+  stv<V>(d.H[0] + q, hx);
+  stv<V>(d.H[1] + q, hy);
+  stv<V>(d.H[2] + q, hz);
+}
+
+// gradient term (row R3) + inverse of the E half-step (row R2), fused since both need curl^-(H^{m-1/2}):
+//   acc += sum_c lE_c * curl_c  on design ∩ inner interior;   E^{m-1} = E^m - ce * curl
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_grad_inv_e(const __grid_constant__ Dev d) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int klo = P + 1, khi = nz - P - 1;
+  const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = P + 1 + blockIdx.y * TY + threadIdx.y;
+  const int i = P + 1 + blockIdx.z;
+  if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * ny + j) * nz + k0;
+  const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  const VF<V> hy_xm = ldv<V>(d.H[1] + q - sx), hz_xm = ldv<V>(d.H[2] + q - sx);
+  const VF<V> hx_ym = ldv<V>(d.H[0] + q - sy), hz_ym = ldv<V>(d.H[2] + q - sy);
+  float hx_z0 = 0.0f, hy_z0 = 0.0f;
+  if (k0 > 0) {
+    hx_z0 = d.H[0][q - 1];
+    hy_z0 = d.H[1][q - 1];
+  }
+  VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  const VF<V> ce = ldv<V>(d.ce + q);
+  const bool des_ij = d.has_design && i >= d.dlo[0] && i < d.dhi[0] && j >= d.dlo[1] && j < d.dhi[1] &&
+                      k0 + V > d.dlo[2] && k0 < d.dhi[2];
+  VF<V> lx = zerov<V>(), ly = zerov<V>(), lz = zerov<V>();
+  if (des_ij) {
+    lx = ldv<V>(d.lE[0] + q);
+    ly = ldv<V>(d.lE[1] + q);
+    lz = ldv<V>(d.lE[2] + q);
+  }
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    if (k < klo || k >= khi) continue;
+    const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+    const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+    const float cx = (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm);
+    const float cy = (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]);
+    const float cz = (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]);
+    if (des_ij && k >= d.dlo[2] && k < d.dhi[2]) {
+      double s = 0.0;
+      s += (double)lx.v[v] * (double)cx;
+      s += (double)ly.v[v] * (double)cy;
+      s += (double)lz.v[v] * (double)cz;
+      const long long e = ((long long)(i - d.dlo[0]) * (d.dhi[1] - d.dlo[1]) + (j - d.dlo[1])) * (d.dhi[2] - d.dlo[2]) +
+                          (k - d.dlo[2]);
+      d.acc[e] += s;
+    }
+    ex.v[v] = fmaf(-ce.v[v], cx, ex.v[v]);
+    ey.v[v] = fmaf(-ce.v[v], cy, ey.v[v]);
+    ez.v[v] = fmaf(-ce.v[v], cz, ez.v[v]);
+  }
+  stv<V>(d.E[0] + q, ex);
+  stv<V>(d.E[1] + q, ey);
+  stv<V>(d.E[2] + q, ez);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Adjoint of the H half-step (row R4): lE_e += -S * curl^-(lH)_e on all cells (PEC-masked nodes -> 0), plus the
+// transposed CPML: for the H term (c,t) with axis a and field b:  g = -S*s*lH_c, W = cH*(lpsiH + g) + kH*g,
+// lpsiH <- bH*(lpsiH + g), lE_b -= d_a^-(W).   lpsiH is ping-ponged (pb = buffer read, pb^1 = written), because
+// W at the low-side neighbour needs that neighbour's OLD lpsiH.
+// ---------------------------------------------------------------------------------------------------------
+struct WTerm {  // W(q) - W(q - stride_a) of one transposed H term, evaluated by the thread that owns q
+  float wq, wm;
+};
+
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_adj_h(const __grid_constant__ Dev d, int pb) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = blockIdx.y * TY + threadIdx.y;
+  const int i = blockIdx.z;
+  if (k0 >= nz || j >= ny) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * ny + j) * nz + k0;
+  const float S = d.S;
+  const VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
+  VF<V> lhy_xm = zerov<V>(), lhz_xm = zerov<V>(), lhx_ym = zerov<V>(), lhz_ym = zerov<V>();
+  if (i > 0) {
+    lhy_xm = ldv<V>(d.lH[1] + q - sx);
+    lhz_xm = ldv<V>(d.lH[2] + q - sx);
+  }
+  if (j > 0) {
+    lhx_ym = ldv<V>(d.lH[0] + q - sy);
+    lhz_ym = ldv<V>(d.lH[2] + q - sy);
+  }
+  float lhx_z0 = 0.0f, lhy_z0 = 0.0f;
+  if (k0 > 0) {
+    lhx_z0 = d.lH[0][q - 1];
+    lhy_z0 = d.lH[1][q - 1];
+  }
+  VF<V> lex = ldv<V>(d.lE[0] + q), ley = ldv<V>(d.lE[1] + q), lez = ldv<V>(d.lE[2] + q);
+
+  // --- slab state at this cell and at its low-side neighbours ---
+  const bool xs = P > 0 && in_slab(i, nx, P), xsm = P > 0 && i > 0 && in_slab(i - 1, nx, P);
+  const bool ys = P > 0 && in_slab(j, ny, P), ysm = P > 0 && j > 0 && in_slab(j - 1, ny, P);
+  float bx = 0, cx = 0, kx = 0, cxm = 0, kxm = 0, by = 0, cy = 0, ky = 0, cym = 0, kym = 0;
+  if (xs) { bx = __ldg(d.tab[0][3] + i); cx = __ldg(d.tab[0][4] + i); kx = __ldg(d.tab[0][5] + i); }
+  if (xsm) { cxm = __ldg(d.tab[0][4] + i - 1); kxm = __ldg(d.tab[0][5] + i - 1); }
+  if (ys) { by = __ldg(d.tab[1][3] + j); cy = __ldg(d.tab[1][4] + j); ky = __ldg(d.tab[1][5] + j); }
+  if (ysm) { cym = __ldg(d.tab[1][4] + j - 1); kym = __ldg(d.tab[1][5] + j - 1); }
+  // old lambda_psi_H at q and at the neighbour, per term
+  VF<V> o11 = zerov<V>(), o20 = zerov<V>(), o11m = zerov<V>(), o20m = zerov<V>();   // axis x: (c=1,t=1), (c=2,t=0)
+  VF<V> o00 = zerov<V>(), o21 = zerov<V>(), o00m = zerov<V>(), o21m = zerov<V>();   // axis y: (c=0,t=0), (c=2,t=1)
+  VF<V> o01 = zerov<V>(), o10 = zerov<V>();                                         // axis z: (c=0,t=1), (c=1,t=0)
+  long long qx = 0, qy = 0, qz = 0;
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    o11 = ldv<V>(d.lpsiH[pb][1][1] + qx);
+    o20 = ldv<V>(d.lpsiH[pb][2][0] + qx);
+  }
+  if (xsm) {
+    const long long qm = psi_index(d, 0, i - 1, j, k0);
+    o11m = ldv<V>(d.lpsiH[pb][1][1] + qm);
+    o20m = ldv<V>(d.lpsiH[pb][2][0] + qm);
+  }
+  if (ys) {
+    qy = psi_index(d, 1, i, j, k0);
+    o00 = ldv<V>(d.lpsiH[pb][0][0] + qy);
+    o21 = ldv<V>(d.lpsiH[pb][2][1] + qy);
+  }
+  if (ysm) {
+    const long long qm = psi_index(d, 1, i, j - 1, k0);
+    o00m = ldv<V>(d.lpsiH[pb][0][0] + qm);
+    o21m = ldv<V>(d.lpsiH[pb][2][1] + qm);
+  }
+  const bool zs0 = P > 0 && in_slab(k0, nz, P);           // V = 4: groups never straddle a slab edge (P % 4 == 0)
+  const bool zsm0 = P > 0 && k0 > 0 && in_slab(k0 - 1, nz, P);
+  float o01_z0 = 0.0f, o10_z0 = 0.0f;
+  if (zs0) {
+    qz = psi_index(d, 2, i, j, k0);
+    o01 = ldv<V>(d.lpsiH[pb][0][1] + qz);
+    o10 = ldv<V>(d.lpsiH[pb][1][0] + qz);
+  }
+  if (zsm0) {
+    const long long qm = psi_index(d, 2, i, j, k0 - 1);
+    o01_z0 = d.lpsiH[pb][0][1][qm];
+    o10_z0 = d.lpsiH[pb][1][0][qm];
+  }
+  VF<V> n11 = o11, n20 = o20, n00 = o00, n21 = o21, n01 = o01, n10 = o10;
+  float dummy;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    const float lhy_zm = v == 0 ? lhy_z0 : lhy.v[v > 0 ? v - 1 : 0];
+    const float lhx_zm = v == 0 ? lhx_z0 : lhx.v[v > 0 ? v - 1 : 0];
+    // --- W terms (coef: t = 0 -> -S, t = 1 -> +S) ---
+    float w11 = 0, w11m = 0, w20 = 0, w20m = 0, w00 = 0, w00m = 0, w21 = 0, w21m = 0, w01 = 0, w01m = 0, w10 = 0, w10m = 0;
+    if (xs) {
+      w11 = cpml_adjoint_term(S * lhy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);
+      w20 = cpml_adjoint_term(-S * lhz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);
+    }
+    if (xsm) {
+      w11m = cpml_adjoint_term(S * lhy_xm.v[v], o11m.v[v], 0.0f, cxm, kxm, dummy);
+      w20m = cpml_adjoint_term(-S * lhz_xm.v[v], o20m.v[v], 0.0f, cxm, kxm, dummy);
+    }
+    if (ys) {
+      w00 = cpml_adjoint_term(-S * lhx.v[v], o00.v[v], by, cy, ky, n00.v[v]);
+      w21 = cpml_adjoint_term(S * lhz.v[v], o21.v[v], by, cy, ky, n21.v[v]);
+    }
+    if (ysm) {
+      w00m = cpml_adjoint_term(-S * lhx_ym.v[v], o00m.v[v], 0.0f, cym, kym, dummy);
+      w21m = cpml_adjoint_term(S * lhz_ym.v[v], o21m.v[v], 0.0f, cym, kym, dummy);
+    }
+    const bool zs = P > 0 && in_slab(k, nz, P);
+    if (zs) {
+      const float bz = __ldg(d.tab[2][3] + k), cz = __ldg(d.tab[2][4] + k), kz = __ldg(d.tab[2][5] + k);
+      w01 = cpml_adjoint_term(S * lhx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);
+      w10 = cpml_adjoint_term(-S * lhy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);
+    }
+    if (P > 0 && k > 0 && in_slab(k - 1, nz, P)) {
+      const float czm = __ldg(d.tab[2][4] + k - 1), kzm = __ldg(d.tab[2][5] + k - 1);
+      const float p01 = v == 0 ? o01_z0 : o01.v[v > 0 ? v - 1 : 0];
+      const float p10 = v == 0 ? o10_z0 : o10.v[v > 0 ? v - 1 : 0];
+      w01m = cpml_adjoint_term(S * lhx_zm, p01, 0.0f, czm, kzm, dummy);
+      w10m = cpml_adjoint_term(-S * lhy_zm, p10, 0.0f, czm, kzm, dummy);
+    }
+    // --- lE_x: plain, then (c=1,t=0,a=z), then (c=2,t=1,a=y) ---
+    if (j == 0 || k == 0) lex.v[v] = 0.0f;
+    else {
+      float x = fmaf(-S, (lhz.v[v] - lhz_ym.v[v]) - (lhy.v[v] - lhy_zm), lex.v[v]);
+      x -= (w10 - w10m);
+      x -= (w21 - w21m);
+      lex.v[v] = x;
+    }
+    // --- lE_y: plain, then (c=0,t=1,a=z), then (c=2,t=0,a=x) ---
+    if (k == 0 || i == 0) ley.v[v] = 0.0f;
+    else {
+      float x = fmaf(-S, (lhx.v[v] - lhx_zm) - (lhz.v[v] - lhz_xm.v[v]), ley.v[v]);
+      x -= (w01 - w01m);
+      x -= (w20 - w20m);
+      ley.v[v] = x;
+    }
+    // --- lE_z: plain, then (c=0,t=0,a=y), then (c=1,t=1,a=x) ---
+    if (i == 0 || j == 0) lez.v[v] = 0.0f;
+    else {
+      float x = fmaf(-S, (lhy.v[v] - lhy_xm.v[v]) - (lhx.v[v] - lhx_ym.v[v]), lez.v[v]);
+      x -= (w00 - w00m);
+      x -= (w11 - w11m);
+      lez.v[v] = x;
+    }
+  }
+  stv<V>(d.lE[0] + q, lex);
+  stv<V>(d.lE[1] + q, ley);
+  stv<V>(d.lE[2] + q, lez);
+  const int nb = pb ^ 1;
+  if (xs) {
+    stv<V>(d.lpsiH[nb][1][1] + qx, n11);
+    stv<V>(d.lpsiH[nb][2][0] + qx, n20);
+  }
+  if (ys) {
+    stv<V>(d.lpsiH[nb][0][0] + qy, n00);
+    stv<V>(d.lpsiH[nb][2][1] + qy, n21);
+  }
+  if (zs0) {
+    stv<V>(d.lpsiH[nb][0][1] + qz, n01);
+    stv<V>(d.lpsiH[nb][1][0] + qz, n10);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Adjoint of the E half-step (row R4): with G_c = ce*lE_c,  lH_h += curl^+(G)_h on all cells, plus the transposed
+// CPML: for the E term (c,t) with axis a and field b: g = s*G_c, W = cE*(lpsiE + g) + kE*g, lpsiE <- bE*(lpsiE+g)
+// (skipped on PEC-masked E_c nodes), lH_b -= d_a^+(W).
+// ---------------------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_adj_e(const __grid_constant__ Dev d, int pb) {
+  const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
+  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
+  const int j = blockIdx.y * TY + threadIdx.y;
+  const int i = blockIdx.z;
+  if (k0 >= nz || j >= ny) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * ny + j) * nz + k0;
+  const VF<V> ce = ldv<V>(d.ce + q);
+  VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
+  VF<V> gy_xp = zerov<V>(), gz_xp = zerov<V>(), gx_yp = zerov<V>(), gz_yp = zerov<V>();
+  float gx_zp = 0.0f, gy_zp = 0.0f;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    gx.v[v] = ce.v[v] * gx.v[v];
+    gy.v[v] = ce.v[v] * gy.v[v];
+    gz.v[v] = ce.v[v] * gz.v[v];
+  }
+  if (i + 1 < nx) {
+    const VF<V> c2 = ldv<V>(d.ce + q + sx);
+    gy_xp = ldv<V>(d.lE[1] + q + sx);
+    gz_xp = ldv<V>(d.lE[2] + q + sx);
+#pragma unroll
+    for (int v = 0; v < V; ++v) { gy_xp.v[v] = c2.v[v] * gy_xp.v[v]; gz_xp.v[v] = c2.v[v] * gz_xp.v[v]; }
+  }
+  if (j + 1 < ny) {
+    const VF<V> c2 = ldv<V>(d.ce + q + sy);
+    gx_yp = ldv<V>(d.lE[0] + q + sy);
+    gz_yp = ldv<V>(d.lE[2] + q + sy);
+#pragma unroll
+    for (int v = 0; v < V; ++v) { gx_yp.v[v] = c2.v[v] * gx_yp.v[v]; gz_yp.v[v] = c2.v[v] * gz_yp.v[v]; }
+  }
+  if (k0 + V < nz) {
+    const float c2 = d.ce[q + V];
+    gx_zp = c2 * d.lE[0][q + V];
+    gy_zp = c2 * d.lE[1][q + V];
+  }
+  VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
+
+  const bool xs = P > 0 && in_slab(i, nx, P), xsp = P > 0 && i + 1 < nx && in_slab(i + 1, nx, P);
+  const bool ys = P > 0 && in_slab(j, ny, P), ysp = P > 0 && j + 1 < ny && in_slab(j + 1, ny, P);
+  float bx = 0, cx = 0, kx = 0, cxp = 0, kxp = 0, by = 0, cy = 0, ky = 0, cyp = 0, kyp = 0;
+  if (xs) { bx = __ldg(d.tab[0][0] + i); cx = __ldg(d.tab[0][1] + i); kx = __ldg(d.tab[0][2] + i); }
+  if (xsp) { cxp = __ldg(d.tab[0][1] + i + 1); kxp = __ldg(d.tab[0][2] + i + 1); }
+  if (ys) { by = __ldg(d.tab[1][0] + j); cy = __ldg(d.tab[1][1] + j); ky = __ldg(d.tab[1][2] + j); }
+  if (ysp) { cyp = __ldg(d.tab[1][1] + j + 1); kyp = __ldg(d.tab[1][2] + j + 1); }
+  // old lambda_psi_E: axis x terms (c=1,t=1: Ey) (c=2,t=0: Ez); axis y (c=0,t=0: Ex) (c=2,t=1: Ez); axis z (c=0,t=1: Ex) (c=1,t=0: Ey)
+  VF<V> o11 = zerov<V>(), o20 = zerov<V>(), o11p = zerov<V>(), o20p = zerov<V>();
+  VF<V> o00 = zerov<V>(), o21 = zerov<V>(), o00p = zerov<V>(), o21p = zerov<V>();
+  VF<V> o01 = zerov<V>(), o10 = zerov<V>();
+  long long qx = 0, qy = 0, qz = 0;
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    o11 = ldv<V>(d.lpsiE[pb][1][1] + qx);
+    o20 = ldv<V>(d.lpsiE[pb][2][0] + qx);
+  }
+  if (xsp) {
+    const long long qp = psi_index(d, 0, i + 1, j, k0);
+    o11p = ldv<V>(d.lpsiE[pb][1][1] + qp);
+    o20p = ldv<V>(d.lpsiE[pb][2][0] + qp);
+  }
+  if (ys) {
+    qy = psi_index(d, 1, i, j, k0);
+    o00 = ldv<V>(d.lpsiE[pb][0][0] + qy);
+    o21 = ldv<V>(d.lpsiE[pb][2][1] + qy);
+  }
+  if (ysp) {
+    const long long qp = psi_index(d, 1, i, j + 1, k0);
+    o00p = ldv<V>(d.lpsiE[pb][0][0] + qp);
+    o21p = ldv<V>(d.lpsiE[pb][2][1] + qp);
+  }
+  const bool zs0 = P > 0 && in_slab(k0, nz, P);
+  const bool zsp0 = P > 0 && k0 + V < nz && in_slab(k0 + V, nz, P);
+  float o01_zp = 0.0f, o10_zp = 0.0f;
+  if (zs0) {
+    qz = psi_index(d, 2, i, j, k0);
+    o01 = ldv<V>(d.lpsiE[pb][0][1] + qz);
+    o10 = ldv<V>(d.lpsiE[pb][1][0] + qz);
+  }
+  if (zsp0) {
+    const long long qp = psi_index(d, 2, i, j, k0 + V);
+    o01_zp = d.lpsiE[pb][0][1][qp];
+    o10_zp = d.lpsiE[pb][1][0][qp];
+  }
+  VF<V> n11 = o11, n20 = o20, n00 = o00, n21 = o21, n01 = o01, n10 = o10;   // masked nodes keep lambda_psi
+  float dummy;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int k = k0 + v;
+    const float gx_zq = v == V - 1 ? gx_zp : gx.v[v < V - 1 ? v + 1 : v];
+    const float gy_zq = v == V - 1 ? gy_zp : gy.v[v < V - 1 ? v + 1 : v];
+    // PEC masks of E_c at q: Ex: j==0||k==0, Ey: k==0||i==0, Ez: i==0||j==0 ; at the +a neighbour only the other axis counts
+    float w11 = 0, w11p = 0, w20 = 0, w20p = 0, w00 = 0, w00p = 0, w21 = 0, w21p = 0, w01 = 0, w01p = 0, w10 = 0, w10p = 0;
+    if (xs) {
+      if (!(k == 0 || i == 0)) w11 = cpml_adjoint_term(-gy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);   // (c=1,t=1): g = -G_y
+      if (!(i == 0 || j == 0)) w20 = cpml_adjoint_term(gz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);    // (c=2,t=0): g = +G_z
+    }
+    if (xsp) {
+      if (k != 0) w11p = cpml_adjoint_term(-gy_xp.v[v], o11p.v[v], 0.0f, cxp, kxp, dummy);
+      if (j != 0) w20p = cpml_adjoint_term(gz_xp.v[v], o20p.v[v], 0.0f, cxp, kxp, dummy);
+    }
+    if (ys) {
+      if (!(j == 0 || k == 0)) w00 = cpml_adjoint_term(gx.v[v], o00.v[v], by, cy, ky, n00.v[v]);    // (c=0,t=0): g = +G_x
+      if (!(i == 0 || j == 0)) w21 = cpml_adjoint_term(-gz.v[v], o21.v[v], by, cy, ky, n21.v[v]);   // (c=2,t=1): g = -G_z
+    }
+    if (ysp) {
+      if (k != 0) w00p = cpml_adjoint_term(gx_yp.v[v], o00p.v[v], 0.0f, cyp, kyp, dummy);
+      if (i != 0) w21p = cpml_adjoint_term(-gz_yp.v[v], o21p.v[v], 0.0f, cyp, kyp, dummy);
+    }
+    if (P > 0 && in_slab(k, nz, P)) {
+      const float bz = __ldg(d.tab[2][0] + k), cz = __ldg(d.tab[2][1] + k), kz = __ldg(d.tab[2][2] + k);
+      if (!(j == 0 || k == 0)) w01 = cpml_adjoint_term(-gx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);   // (c=0,t=1): g = -G_x
+      if (!(k == 0 || i == 0)) w10 = cpml_adjoint_term(gy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);    // (c=1,t=0): g = +G_y
+    }
+    if (P > 0 && k + 1 < nz && in_slab(k + 1, nz, P)) {
+      const float czp = __ldg(d.tab[2][1] + k + 1), kzp = __ldg(d.tab[2][2] + k + 1);
+      const float p01 = v == V - 1 ? o01_zp : o01.v[v < V - 1 ? v + 1 : v];
+      const float p10 = v == V - 1 ? o10_zp : o10.v[v < V - 1 ? v + 1 : v];
+      if (j != 0) w01p = cpml_adjoint_term(-gx_zq, p01, 0.0f, czp, kzp, dummy);
+      if (i != 0) w10p = cpml_adjoint_term(gy_zq, p10, 0.0f, czp, kzp, dummy);
+    }
+    // lH_x: d1 = d_y^+ G_z, d2 = d_z^+ G_y ; then (c=1,t=0,a=z), then (c=2,t=1,a=y)
+    {
+      float x = lhx.v[v] + ((gz_yp.v[v] - gz.v[v]) - (gy_zq - gy.v[v]));
+      x -= (w10p - w10);
+      x -= (w21p - w21);
+      lhx.v[v] = x;
+    }
+    // lH_y: d1 = d_z^+ G_x, d2 = d_x^+ G_z ; then (c=0,t=1,a=z), then (c=2,t=0,a=x)
+    {
+      float x = lhy.v[v] + ((gx_zq - gx.v[v]) - (gz_xp.v[v] - gz.v[v]));
+      x -= (w01p - w01);
+      x -= (w20p - w20);
+      lhy.v[v] = x;
+    }
+    // lH_z: d1 = d_x^+ G_y, d2 = d_y^+ G_x ; then (c=0,t=0,a=y), then (c=1,t=1,a=x)
+    {
+      float x = lhz.v[v] + ((gy_xp.v[v] - gy.v[v]) - (gx_yp.v[v] - gx.v[v]));
+      x -= (w00p - w00);
+      x -= (w11p - w11);
+      lhz.v[v] = x;
+    }
+  }
+  stv<V>(d.lH[0] + q, lhx);
+  stv<V>(d.lH[1] + q, lhy);
+  stv<V>(d.lH[2] + q, lhz);
+  const int nb = pb ^ 1;
+  if (xs) {
+    stv<V>(d.lpsiE[nb][1][1] + qx, n11);
+    stv<V>(d.lpsiE[nb][2][0] + qx, n20);
+  }
+  if (ys) {
+    stv<V>(d.lpsiE[nb][0][0] + qy, n00);
+    stv<V>(d.lpsiE[nb][2][1] + qy, n21);
+  }
+  if (zs0) {
+    stv<V>(d.lpsiE[nb][0][1] + qz, n01);
+    stv<V>(d.lpsiE[nb][1][0] + qz, n10);
+  }
+}
+
+}  // namespace fdtd

@@ -27,7 +27,7 @@ WAVELENGTH = 1550e-9
 OMEGA_DT = 2.0 * np.pi * C0 * DT / WAVELENGTH  # rad per step; 2*pi/135.59 ("approximately 136")
 EPS_SI, EPS_SIO2 = 12.25, 2.085
 
-# store dtypes / interpolation (same ids as include/fdtd.h and oracle/fdtd_oracle.py)
+# store dtypes / interpolation (the ids of include/fdtd.h)
 F32, F16, BF16, F8E4M3_SCALED = 0, 1, 2, 3
 LINEAR, CUBIC = 0, 1
 DTYPE_NAMES = {F32: "float32", F16: "float16", BF16: "bfloat16", F8E4M3_SCALED: "float8_e4m3+scale"}

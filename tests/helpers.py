@@ -35,3 +35,25 @@ def rel_l2(a, b):
     a = np.asarray(a, dtype=np.float64)
     b = np.asarray(b, dtype=np.float64)
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+# ---- CUDA path (imported lazily so that CPU-only test runs never touch torch.cuda) ----
+def gpu_sim(w, cpml=None):
+    import torch
+    from paper_2603_24027_b200 import fdtd
+    eps = torch.from_numpy(np.ascontiguousarray(w.eps, dtype=np.float32)).cuda()
+    return fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor, cpml=cpml)
+
+
+def gpu_gradient(w, dtype, k, interp=0, extra=None, sim=None):
+    """forward -> loss (harness, numpy on the monitor record) -> reverse, all through the C ABI."""
+    import torch
+    s = sim or gpu_sim(w)
+    mon = s.forward(w.nsteps, w.sources, dtype, k)
+    final = s.fields().cpu().numpy().astype(np.float64)
+    mon_np = mon.cpu().numpy().astype(np.float64)
+    L, d = W.loss_and_cotangent(w, mon_np, extra)
+    dmon = torch.from_numpy(d.astype(np.float32)).cuda()
+    g = s.reverse(None, dmon, interp)
+    state0 = s.fields().cpu().numpy().astype(np.float64)
+    return dict(L=L, grad=g.cpu().numpy().astype(np.float64), final=final, state0=state0, mon=mon_np, sim=s, dmon=d)

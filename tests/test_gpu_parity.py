@@ -1,0 +1,288 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): codec / interpolation bit-exact on identical slices; end-to-end float32 fields
+rel-L2 <= 1e-5 and gradients <= 1e-4 against the float32 oracle under identical compression settings.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from oracle import fdtd_oracle as orc
+from paper_2603_24027_b200 import workloads as W
+from tests.helpers import gpu_gradient, gpu_sim, make_oracle, oracle_gradient, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+FIELD_TOL = 1e-5
+GRAD_TOL = 1e-4
+
+
+def _fdtd():
+    from paper_2603_24027_b200 import fdtd
+    return fdtd
+
+
+def _report(name, g, o):
+    f_err = rel_l2(g["final"], o["final"])
+    g_err = rel_l2(g["grad"], o["grad"])
+    s_err = np.abs(g["state0"] - o["state0"]).max() / max(np.abs(o["final"]).max(), 1e-30)
+    ident = np.array_equal(g["final"], o["final"])
+    print(f"[parity] {name}: fields rel-L2 {f_err:.3e} (bit-identical: {ident}), grad rel-L2 {g_err:.3e}, "
+          f"state0 max-abs/peak {s_err:.3e}, cos {W.cosine_similarity(g['grad'], o['grad']):.9f}")
+    return f_err, g_err
+
+
+def mid_workload(shape=(40, 52, 136), P=8, nsteps=48, seed=21, dtype=W.F32, k=1):
+    """Several tiles with ragged tails in y (52 = 6*8+4) and z (136 = 128+8), x chunks, V = 4 path."""
+    rng = np.random.default_rng(seed)
+    eps = rng.uniform(1.0, 12.25, shape).astype(np.float32)
+    c = tuple(s // 2 for s in shape)
+    wave = W.gauss_sine(nsteps, 14, 5)
+    amp = rng.uniform(0.5, 1.5, (3, 2, 4)).astype(np.float32)
+    srcs = [W.Source(1, c, (c[0] + 3, c[1] + 2, c[2] + 4), amp, wave),
+            W.Source(2, (P, P, P), (P + 1, P + 1, P + 1), None, (0.3 * wave).astype(np.float32))]
+    design = ((P, P + 2, P), (P + 9, shape[1] - P, P + 21))
+    mon = ((shape[0] - P - 3, P, P), (shape[0] - P - 2, shape[1] - P, shape[2] - P), 0b110110)
+    return W.Workload("mid", shape, P, nsteps, eps, design, srcs, mon, "flux_x", dtype, k)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# codec / interpolation: bit-exact on identical slices
+# ---------------------------------------------------------------------------------------------------------
+def _slice(n, seed, amp=1.0):
+    rng = np.random.default_rng(seed)
+    x = (amp * rng.standard_normal(n) * np.exp(rng.uniform(-8, 2, n))).astype(np.float32)
+    x[:8] = [0.0, -0.0, 1e-45, -3e-39, 6.1e-5, -5.9e-8, 65504.0 if amp >= 1 else 1e-3, 1.0]
+    return x
+
+
+@pytest.mark.parametrize("dtype", [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED])
+@pytest.mark.parametrize("n,amp", [(1, 1.0), (257, 1.0), (70001, 1e-3), (4096, 3e4)])
+def test_quantise_bit_exact(dtype, n, amp):
+    import torch
+    fdtd = _fdtd()
+    x = _slice(max(n, 8), 100 + n, amp)[:n]
+    codes, scale = fdtd.codec_encode(dtype, torch.from_numpy(x).cuda())
+    ref_codes, ref_scale = orc.encode(dtype, x)
+    assert np.array_equal(codes.cpu().numpy(), ref_codes)
+    assert np.float32(scale) == np.float32(ref_scale)
+
+
+def test_quantise_zero_slice_fp8():
+    import torch
+    fdtd = _fdtd()
+    codes, scale = fdtd.codec_encode(W.F8E4M3_SCALED, torch.zeros(1000, device="cuda"))
+    assert scale == 0.0 and not codes.any().item()
+
+
+@pytest.mark.parametrize("dtype", [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED])
+@pytest.mark.parametrize("interp", [W.LINEAR, W.CUBIC])
+def test_dequantise_interpolate_bit_exact(dtype, interp):
+    import torch
+    fdtd = _fdtd()
+    n = 3001
+    xs = [_slice(n, 7 + j, 1e-2) for j in range(4)]
+    enc = [orc.encode(dtype, x) for x in xs]
+    dec = [orc.decode(dtype, c, s) for c, s in enc]
+    codes = [torch.from_numpy(c).cuda() for c, _ in enc]
+    scales = [float(s) for _, s in enc]
+    for num, den in [(0, 4), (1, 4), (3, 4), (5, 8), (1, 3), (31, 32), (1, 2)]:
+        got = fdtd.codec_fetch(dtype, interp, codes, scales, num, den).cpu().numpy()
+        if num == 0:
+            ref = dec[1]
+        elif interp == W.LINEAR:
+            ref = np.array([orc.lerp(float(a), float(b), num, den) for a, b in zip(dec[1], dec[2])], dtype=np.float32)
+        else:
+            ref = np.array([orc.cubic(float(a), float(b), float(c), float(d), num, den)
+                            for a, b, c, d in zip(dec[0], dec[1], dec[2], dec[3])], dtype=np.float32)
+        assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (dtype, interp, num, den)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# end-to-end parity
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,k,interp", [(W.F32, 1, W.LINEAR), (W.BF16, 4, W.LINEAR), (W.F16, 3, W.CUBIC),
+                                            (W.F8E4M3_SCALED, 5, W.LINEAR)])
+def test_tiny_scalar_path(dtype, k, interp):
+    """Odd shape (14,13,12), P = 3: the V = 1 kernels, edge/corner design cells, nsteps % k != 0."""
+    w = W.tiny(nsteps=22)
+    o = oracle_gradient(w, 32, dtype, k, interp)
+    g = gpu_gradient(w, dtype, k, interp)
+    f_err, g_err = _report(f"tiny dtype={dtype} k={k} interp={interp}", g, o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    assert rel_l2(g["mon"], o["mon"]) <= FIELD_TOL
+    assert g["sim"].store_bytes() == o["sim"].store_bytes()
+    assert g["sim"].num_slots() == o["sim"].num_slots()
+
+
+@pytest.mark.parametrize("dtype,k,interp", [(W.F32, 1, W.LINEAR), (W.BF16, 4, W.LINEAR), (W.F16, 8, W.LINEAR),
+                                            (W.F8E4M3_SCALED, 8, W.LINEAR), (W.F16, 8, W.CUBIC)])
+def test_c1_gradient_parity(dtype, k, interp):
+    """BASELINE.json configs[0] (32^3, P = 8, 200 steps) under each store setting."""
+    w = W.c1()
+    o = oracle_gradient(w, 32, dtype, k, interp)
+    g = gpu_gradient(w, dtype, k, interp)
+    f_err, g_err = _report(f"C1 dtype={dtype} k={k} interp={interp}", g, o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    P = w.pml
+    peak = np.abs(o["final"]).max()
+    assert np.abs((g["state0"] - o["state0"])[:, P:-P, P:-P, P:-P]).max() <= 1e-5 * peak
+    assert g["sim"].store_bytes() == o["sim"].store_bytes()
+
+
+def test_c1_against_f64_oracle_reported():
+    """GPU f32 vs the f64 oracle: reported, gated only loosely (f32 vs f64 alone is ~1e-5 in the fields)."""
+    w = W.c1()
+    o = oracle_gradient(w, 64, orc.NATIVE, 1)
+    g = gpu_gradient(w, W.F32, 1)
+    f_err, g_err = _report("C1 vs f64 oracle", g, o)
+    assert f_err <= 5e-5 and g_err <= GRAD_TOL
+
+
+@pytest.mark.parametrize("dtype,k", [(W.F32, 1), (W.BF16, 4)])
+def test_mid_grid_several_tiles_ragged(dtype, k):
+    w = mid_workload(dtype=dtype, k=k)
+    o = oracle_gradient(w, 32, dtype, k)
+    g = gpu_gradient(w, dtype, k)
+    f_err, g_err = _report(f"mid dtype={dtype} k={k}", g, o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    assert rel_l2(g["mon"], o["mon"]) <= FIELD_TOL
+
+
+def test_store_slots_bit_exact_when_fields_agree():
+    """Record kernel vs oracle record: every slot, byte for byte, for each dtype (fields are bit-identical in practice;
+    if they are not, compare the decoded values within the field tolerance instead)."""
+    import torch
+    w = W.c1(nsteps=40)
+    for dtype, k in [(W.F32, 1), (W.F16, 4), (W.BF16, 4), (W.F8E4M3_SCALED, 8)]:
+        o = make_oracle(w, 32)
+        o.forward(w.nsteps, dtype, k)
+        s = gpu_sim(w)
+        s.forward(w.nsteps, w.sources, dtype, k)
+        same_fields = np.array_equal(s.fields().cpu().numpy().astype(np.float64), o.fields())
+        assert s.num_slots() == o.num_slots() and s.slot_values() == o.slot_values()
+        for j in range(o.num_slots()):
+            data, scales = s.slot(j, dtype)
+            od, osc = o.slot(j, dtype)
+            if same_fields:
+                assert np.array_equal(data.cpu().numpy(), od), (dtype, j)
+                if dtype == W.F8E4M3_SCALED:
+                    assert np.array_equal(scales.cpu().numpy(), osc), (dtype, j)
+            else:
+                sc_g = scales.cpu().numpy() if dtype == W.F8E4M3_SCALED else np.ones(36, np.float32)
+                fs = o.slot_values() // 36
+                # decode slice by slice (all faces equal-sized here)
+                for sl in range(36):
+                    eb = orc.elem_bytes(dtype) if dtype != W.F32 else 4
+                    a = orc.decode(dtype, data.cpu().numpy()[sl * fs * eb:(sl + 1) * fs * eb], sc_g[sl])
+                    b = orc.decode(dtype, od[sl * fs * eb:(sl + 1) * fs * eb], osc[sl] if dtype == W.F8E4M3_SCALED else 1.0)
+                    assert np.abs(a - b).max() <= 0.07 * max(np.abs(b).max(), 1e-30)
+        print(f"[parity] store slots dtype={dtype} k={k}: fields bit-identical={same_fields}")
+
+
+def test_c2_shaped_short_run_sampled_parity():
+    """BASELINE.json configs[1] grid and launch configuration (128^3, P = 12, bf16, k = 4) on a run short enough for the
+    oracle; fields compared on sampled planes, gradient on the whole design patch."""
+    w = W.c2(nsteps=120)
+    o = oracle_gradient(w, 32, w.store_dtype, w.k)
+    g = gpu_gradient(w, w.store_dtype, w.k)
+    f_err, g_err = _report("C2-shaped 120 steps", g, o)
+    for sl in (np.s_[:, 64], np.s_[:, :, 40], np.s_[:, :, :, 63]):
+        assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+
+
+def test_final_state_cotangent_box_and_get_box():
+    """dL/dfinal given as a box cotangent (fdtd_cotangent) instead of a monitor cotangent gives the same gradient."""
+    import torch
+    w = W.c1(nsteps=60)
+    o = oracle_gradient(w, 32, W.F32, 1)
+    s = gpu_sim(w)
+    s.forward(w.nsteps, w.sources, W.F32, 1)
+    lo, hi, mask = w.monitor
+    box = s.box(lo, hi, mask)
+    g = s.reverse((lo, hi, mask, (2.0 * box).contiguous()), None, W.LINEAR)
+    assert rel_l2(g.cpu().numpy(), o["grad"]) <= GRAD_TOL
+    full = s.fields()
+    assert full.shape == (6, 32, 32, 32)
+
+
+def test_repeated_runs_and_new_eps_are_deterministic():
+    w = W.c1(nsteps=50)
+    s = gpu_sim(w)
+    a = gpu_gradient(w, W.BF16, 4, sim=s)
+    b = gpu_gradient(w, W.BF16, 4, sim=s)
+    assert np.array_equal(a["grad"], b["grad"]) and np.array_equal(a["final"], b["final"])
+    import torch
+    w2 = W.c1(nsteps=50, seed=77)
+    s.set_eps(torch.from_numpy(w2.eps).cuda())
+    c = gpu_gradient(w2, W.BF16, 4, sim=s)
+    o = oracle_gradient(w2, 32, W.BF16, 4)
+    assert rel_l2(c["grad"], o["grad"]) <= GRAD_TOL
+
+
+def test_host_buffer_path_matches_device_path():
+    import torch
+    fdtd = _fdtd()
+    w = W.c1(nsteps=64)
+    ref = gpu_gradient(w, W.F16, 4)
+    s = gpu_sim(w)
+    s.set_workspace(w.nsteps, W.F16, 4, fdtd.WS_REVERSE | fdtd.WS_HOST_IO)
+    s.set_eps_host(torch.from_numpy(w.eps).pin_memory())
+    mon = torch.empty(w.monitor_shape(), dtype=torch.float32).pin_memory()
+    s.forward_host(w.nsteps, w.sources, W.F16, 4, mon)
+    L, d = W.loss_and_cotangent(w, mon.numpy())
+    grad = torch.empty(16, 16, 16, dtype=torch.float32).pin_memory()
+    s.reverse_host(torch.from_numpy(d.astype(np.float32)).pin_memory(), W.LINEAR, grad)
+    assert abs(L - ref["L"]) <= 1e-12 * abs(ref["L"])
+    assert np.array_equal(grad.numpy().astype(np.float64), ref["grad"])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# error behaviour and memory claims
+# ---------------------------------------------------------------------------------------------------------
+def test_error_codes():
+    import torch
+    fdtd = _fdtd()
+    w = W.tiny()
+    with pytest.raises(fdtd.FdtdError) as e:
+        fdtd.Sim(torch.ones(8, 8, 8, device="cuda"), W.DX, 2 * W.DT, 2)          # above the CFL limit
+    assert e.value.status == 1
+    with pytest.raises(fdtd.FdtdError):
+        fdtd.Sim(torch.ones(8, 8, 8, device="cuda"), W.DX, W.DT, 4)              # no interior left
+    s = gpu_sim(w)
+    with pytest.raises(fdtd.FdtdError) as e:
+        s.reverse()                                                              # reverse before forward
+    assert e.value.status == 4
+    with pytest.raises(fdtd.FdtdError) as e:
+        s.set_workspace(100, W.F32, 1, bytes_override=1 << 16)                   # workspace too small
+    assert e.value.status == 2
+    s.set_workspace(10, W.F32, 1)
+    arr = s._sources(w.sources, 20, False)
+    assert s._L.fdtd_forward(s._h, 20, arr, len(w.sources), W.F32, 1) == 2       # run longer than the workspace allows
+    assert s._L.fdtd_forward(s._h, 10, arr, len(w.sources), W.F32, 0) == 1       # k < 1
+    bad = dataclasses.replace(w.sources[0], lo=(0, 0, 0), hi=(1, 1, 1))
+    arr = s._sources([bad], 10, False)
+    assert s._L.fdtd_forward(s._h, 10, arr, 1, W.F32, 1) == 1                    # source outside the interior
+    low = gpu_sim(dataclasses.replace(w, eps=np.full(w.shape, 0.5, np.float32)))
+    with pytest.raises(fdtd.FdtdError) as e:
+        low.set_workspace(10, W.F32, 1)                                          # eps < 1
+    assert e.value.status == 1
+
+
+def test_512_cubed_long_run_fits_only_compressed():
+    """BASELINE.json configs[3]: the uncompressed float32 k = 1 store of the 512^3 / 10000-step run exceeds HBM,
+    bf16 k = 4 and fp8 k = 8 fit (sizes only; nothing is allocated)."""
+    import torch
+    fdtd = _fdtd()
+    eps = torch.ones(512, 512, 512, device="cuda")
+    s = fdtd.Sim(eps, W.DX, W.DT, 16, design=((128, 128, 128), (384, 384, 384)))
+    hbm = torch.cuda.get_device_properties(0).total_memory
+    f32 = s.workspace_bytes(10000, W.F32, 1)
+    bf16 = s.workspace_bytes(10000, W.BF16, 4)
+    fp8 = s.workspace_bytes(10000, W.F8E4M3_SCALED, 8)
+    assert f32 > hbm > bf16 > fp8
+    assert abs(f32 - bf16 - (10001 * 4 - 2501 * 2) * s.slot_values()) < (1 << 24)
+    print(f"[memory] 512^3 x 10000 steps: f32,k=1 {f32 / 1e9:.1f} GB (HBM {hbm / 1e9:.1f} GB), bf16,k=4 {bf16 / 1e9:.1f} GB, "
+          f"fp8,k=8 {fp8 / 1e9:.1f} GB")
