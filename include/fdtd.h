@@ -164,6 +164,13 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dtype, fdtd_interp interp, const void* c
 fdtd_status fdtd_sync(fdtd_sim*);
 const char* fdtd_last_error(const fdtd_sim*);
 void fdtd_destroy(fdtd_sim*);
+/* Measurement aid for bench.py's roofline: launch stencil kernel `kernel_id` reps times back to back on the current
+ * buffers between two CUDA events (after `warm` untimed launches) and return the mean milliseconds per launch.
+ * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e.  Needs a reverse
+ * workspace and a completed forward for ids >= 2.  The field contents are garbage afterwards: call fdtd_reset.
+ * Synchronises.  algo_bytes (may be NULL) receives the algorithmic bytes one launch moves. */
+fdtd_status fdtd_profile_kernel(fdtd_sim*, int kernel_id, int warm, int reps, double* ms_per_launch, double* algo_bytes);
+
 /* Number of kernels this library has launched on behalf of the handle since create (bench.py's gpu_launches). */
 unsigned long long fdtd_launch_count(const fdtd_sim*);
 

@@ -62,8 +62,12 @@ struct fdtd_sim {
   std::vector<SrcDev> src_host;
   std::vector<float> waves_host;
   int nsrc = 0;
-  int V = 1;
-  int xch = 8;
+  int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
+  int VG = 1;   // ... of the general kernels (2 in vector mode)
+  // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
+  Region reg[4]{};
+  bool has_lean[4] = {false, false, false, false};
+  BoxList boxes[4]{};
   // run state
   int nsteps = 0, k = 1, dtype = 0;
   bool forward_done = false, state_final = false;
@@ -207,8 +211,51 @@ bool in_grid(const fdtd_sim* s, const int lo[3], const int hi[3]) {
   return box_ok(lo, hi, ilo, s->n);
 }
 
-dim3 grid_all(const fdtd_sim* s, int zdim) {
-  return dim3((unsigned)((s->n[2] + 32 * s->V - 1) / (32 * s->V)), (unsigned)((s->n[1] + TY - 1) / TY), (unsigned)zdim);
+// Lean region [lo, hi) of split half-step `which` and the disjoint boxes covering the rest of the grid.
+void make_split(fdtd_sim* s, int which) {
+  const int P = s->P, V = s->V, VG = s->VG;
+  Region& r = s->reg[which];
+  for (int a = 0; a < 3; ++a) {
+    const int n = s->n[a];
+    int lo, hi;
+    switch (which) {
+      case 0: lo = std::max(P, 1); hi = n - P; break;                 // fwd E: needs the -1 neighbours, no PEC-masked node
+      case 1: lo = P; hi = std::min(n - P, n - 1); break;             // fwd H: needs the +1 neighbours
+      case 2: lo = P + 1; hi = n - P; break;                          // adj H: the -1 neighbour must not be a slab cell
+      default: lo = P; hi = std::min(n - P - 1, n - 1); break;        // adj E: the +1 neighbour must not be a slab cell
+    }
+    if (a == 2) { lo = (lo + V - 1) / V * V; hi = hi / V * V; }
+    r.lo[a] = lo; r.hi[a] = hi;
+  }
+  s->has_lean[which] = r.hi[0] > r.lo[0] && r.hi[1] > r.lo[1] && r.hi[2] > r.lo[2];
+  BoxList& B = s->boxes[which];
+  B = BoxList{};
+  auto add = [&](int x0, int x1, int y0, int y1, int z0, int z1) {
+    if (x1 <= x0 || y1 <= y0 || z1 <= z0) return;
+    const int b = B.nb++;
+    B.lo[b][0] = x0; B.hi[b][0] = x1; B.lo[b][1] = y0; B.hi[b][1] = y1; B.lo[b][2] = z0; B.hi[b][2] = z1;
+    const int groups = (z1 - z0 + VG - 1) / VG;
+    int lzs = 0;
+    while ((1 << lzs) < groups && lzs < 5) ++lzs;
+    B.lzs[b] = lzs;
+    B.nbx[b] = (groups + (1 << lzs) - 1) >> lzs;
+    const int rows_per_block = TY << (5 - lzs);
+    B.nby[b] = (y1 - y0 + rows_per_block - 1) / rows_per_block;
+    B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b] * (x1 - x0);
+  };
+  const int nx = s->n[0], ny = s->n[1], nz = s->n[2];
+  if (!s->has_lean[which]) { add(0, nx, 0, ny, 0, nz); return; }
+  add(0, r.lo[0], 0, ny, 0, nz);
+  add(r.hi[0], nx, 0, ny, 0, nz);
+  add(r.lo[0], r.hi[0], 0, r.lo[1], 0, nz);
+  add(r.lo[0], r.hi[0], r.hi[1], ny, 0, nz);
+  add(r.lo[0], r.hi[0], r.lo[1], r.hi[1], 0, r.lo[2]);
+  add(r.lo[0], r.hi[0], r.lo[1], r.hi[1], r.hi[2], nz);
+}
+dim3 grid_lean(const fdtd_sim* s, int which) {
+  const Region& r = s->reg[which];
+  return dim3((unsigned)((r.hi[2] - r.lo[2] + 32 * s->V - 1) / (32 * s->V)), (unsigned)((r.hi[1] - r.lo[1] + TY - 1) / TY),
+              (unsigned)(r.hi[0] - r.lo[0]));
 }
 bool grid_inner(const fdtd_sim* s, dim3* g) {
   const int P = s->P, V = s->V;
@@ -226,16 +273,49 @@ bool grid_inner(const fdtd_sim* s, dim3* g) {
     ++(s)->launches;                                 \
   } while (0)
 
-void launch_fwd_e(fdtd_sim* s) {
-  const dim3 g = grid_all(s, (s->n[0] + s->xch - 1) / s->xch), b(32, TY);
-  if (s->V == 4) LAUNCH(s, k_fwd_e<4>, g, b, s->d, s->xch);
-  else LAUNCH(s, k_fwd_e<1>, g, b, s->d, s->xch);
+// The four split half-steps: lean kernel on the plain cells + general kernel on the rest (disjoint writes).
+void launch_split(fdtd_sim* s, int which, int pb) {
+  const dim3 b(32, TY);
+  if (s->has_lean[which]) {
+    const dim3 g = grid_lean(s, which);
+    const Region& r = s->reg[which];
+    if (s->V == 4) {
+      switch (which) {
+        case 0: LAUNCH(s, (k_lean_curlm<4, false>), g, b, s->d, r); break;
+        case 1: LAUNCH(s, k_lean_h<4>, g, b, s->d, r); break;
+        case 2: LAUNCH(s, (k_lean_curlm<4, true>), g, b, s->d, r); break;
+        default: LAUNCH(s, k_lean_adj_e<4>, g, b, s->d, r);
+      }
+    } else {
+      switch (which) {
+        case 0: LAUNCH(s, (k_lean_curlm<1, false>), g, b, s->d, r); break;
+        case 1: LAUNCH(s, k_lean_h<1>, g, b, s->d, r); break;
+        case 2: LAUNCH(s, (k_lean_curlm<1, true>), g, b, s->d, r); break;
+        default: LAUNCH(s, k_lean_adj_e<1>, g, b, s->d, r);
+      }
+    }
+  }
+  const BoxList& B = s->boxes[which];
+  const unsigned g = (unsigned)B.off[B.nb];
+  if (g == 0) return;
+  if (s->VG == 2) {
+    switch (which) {
+      case 0: LAUNCH(s, k_gen_e<2>, g, b, s->d, B); break;
+      case 1: LAUNCH(s, k_gen_h<2>, g, b, s->d, B); break;
+      case 2: LAUNCH(s, k_gen_adj_h<2>, g, b, s->d, B, pb); break;
+      default: LAUNCH(s, k_gen_adj_e<2>, g, b, s->d, B, pb);
+    }
+  } else {
+    switch (which) {
+      case 0: LAUNCH(s, k_gen_e<1>, g, b, s->d, B); break;
+      case 1: LAUNCH(s, k_gen_h<1>, g, b, s->d, B); break;
+      case 2: LAUNCH(s, k_gen_adj_h<1>, g, b, s->d, B, pb); break;
+      default: LAUNCH(s, k_gen_adj_e<1>, g, b, s->d, B, pb);
+    }
+  }
 }
-void launch_fwd_h(fdtd_sim* s) {
-  const dim3 g = grid_all(s, (s->n[0] + s->xch - 1) / s->xch), b(32, TY);
-  if (s->V == 4) LAUNCH(s, k_fwd_h<4>, g, b, s->d, s->xch);
-  else LAUNCH(s, k_fwd_h<1>, g, b, s->d, s->xch);
-}
+void launch_fwd_e(fdtd_sim* s) { launch_split(s, 0, 0); }
+void launch_fwd_h(fdtd_sim* s) { launch_split(s, 1, 0); }
 void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
   if (s->nsrc == 0) return;
   long long maxc = 1;
@@ -293,9 +373,7 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
     if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
     else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
   }
-  const dim3 ga = grid_all(s, s->n[0]);
-  if (s->V == 4) LAUNCH(s, k_adj_h<4>, ga, b, s->d, pb);
-  else LAUNCH(s, k_adj_h<1>, ga, b, s->d, pb);
+  launch_split(s, 2, pb);
   launch_inject(s, m_base, step_dev, 1, interp);
   launch_sources(s, m_base, step_dev, -1.0f);
   if (inner) {
@@ -303,8 +381,7 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
     else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d);
   }
   launch_inject(s, m_base, step_dev, 0, interp);
-  if (s->V == 4) LAUNCH(s, k_adj_e<4>, ga, b, s->d, pb);
-  else LAUNCH(s, k_adj_e<1>, ga, b, s->d, pb);
+  launch_split(s, 3, pb);
 }
 
 fdtd_status zero_state(fdtd_sim* s) {
@@ -563,14 +640,9 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
   }
   s->V = (s->n[2] % 4 == 0 && s->P % 4 == 0) ? 4 : 1;
-  {
-    // x chunk per block of the marching forward kernels: enough blocks to fill 148 SMs several times over
-    const long long gxy = (long long)((s->n[2] + 32 * s->V - 1) / (32 * s->V)) * ((s->n[1] + TY - 1) / TY);
-    long long chunks = std::max<long long>(1, (148LL * 8 + gxy - 1) / gxy);
-    int xch = (int)std::max<long long>(4, (s->n[0] + chunks - 1) / chunks);
-    if (const char* e = std::getenv("FDTD_XCH")) xch = std::max(1, atoi(e));
-    s->xch = std::min(xch, s->n[0]);
-  }
+  s->VG = s->V == 4 ? 2 : 1;
+  if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2) && s->V == 4) s->VG = v; }
+  for (int which = 0; which < 4; ++which) make_split(s, which);
   build_tables(s);
   CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
   CUDA_TRY(s, cudaMemsetAsync(w + L.step, 0, 16, s->stream));
@@ -733,6 +805,73 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* cons
     default: k_codec_fetch<DT_E4M3S><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev);
   }
   return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
+}
+
+fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
+  if (!s || id < 0 || id > 8 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
+  if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
+  if (id >= 6 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
+  const dim3 b(32, TY);
+  dim3 gi;
+  const bool inner = grid_inner(s, &gi);
+  const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
+  auto once = [&]() {
+    switch (id) {
+      case 0: launch_fwd_e(s); break;
+      case 1: launch_fwd_h(s); break;
+      case 2: if (inner) { if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d); else LAUNCH(s, k_inv_h<1>, gi, b, s->d); } break;
+      case 3: launch_split(s, 2, 0); break;
+      case 4: if (inner) { if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d); else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d); } break;
+      case 5: launch_split(s, 3, 0); break;
+      case 6: launch_record(s, s->nsteps, nullptr); break;
+      case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
+      default: launch_inject(s, mrev, nullptr, 0, 0); break;
+    }
+  };
+  cudaEvent_t e0, e1;
+  CUDA_TRY(s, cudaEventCreate(&e0));
+  CUDA_TRY(s, cudaEventCreate(&e1));
+  for (int r = 0; r < warm; ++r) once();
+  CUDA_TRY(s, cudaEventRecord(e0, s->stream));
+  for (int r = 0; r < reps; ++r) once();
+  CUDA_TRY(s, cudaEventRecord(e1, s->stream));
+  CUDA_TRY(s, cudaEventSynchronize(e1));
+  float ms = 0;
+  CUDA_TRY(s, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  CUDA_TRY(s, cudaGetLastError());
+  *ms_out = (double)ms / reps;
+  s->forward_done = s->state_final = false;
+  if (bytes_out) {
+    // algorithmic bytes per launch: f32 arrays read / written once, psi read+written in the slabs
+    const double N = (double)s->d.N;
+    double slab = 0;
+    for (int a = 0; a < 3; ++a) slab += (double)psi_elems(s, a);
+    double Ninner = 1;
+    for (int a = 0; a < 3; ++a) Ninner *= std::max(0, s->n[a] - 2 * s->P - 2);
+    double dcells = 0;
+    if (s->has_design) {
+      dcells = 1;
+      for (int a = 0; a < 3; ++a) dcells *= std::max(0, std::min(s->dhi[a], s->n[a] - s->P - 1) - std::max(s->dlo[a], s->P + 1));
+    }
+    const double eb = elem_bytes_host(s->dtype);
+    double shell = (double)s->st.cell_off[6];
+    double v = 0;
+    switch (id) {
+      case 0: v = 40 * N + 16 * slab; break;          // E rw (24) + H (12) + ce (4); 2 psi arrays rw per slab-cell-axis
+      case 1: v = 36 * N + 16 * slab; break;          // H rw (24) + E (12)
+      case 2: v = 36 * Ninner; break;
+      case 3: v = 36 * N + 16 * slab; break;          // lE rw + lH; lpsiH read (old) + written (new)
+      case 4: v = 40 * Ninner + 28 * dcells; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
+      case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
+      case 6: v = (double)s->st.slot_values * (4 + eb); break;
+      default: v = 3 * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+    }
+    *bytes_out = v;
+  }
+  return FDTD_OK;
 }
 
 fdtd_status fdtd_sync(fdtd_sim* s) {

@@ -32,6 +32,17 @@ struct Dev {
   int has_design;
 };
 
+// A lean kernel's region (plain Yee cells) and the list of boxes that make up its complement (slab cells and the
+// layers that touch them), each with its own lane shape: LZ = 1 << lzs lanes along z, 32/LZ rows per warp.
+struct Region { int lo[3], hi[3]; };
+struct BoxList {
+  int nb;
+  int lo[6][3], hi[6][3];
+  int lzs[6];
+  int nbx[6], nby[6];
+  int off[7];
+};
+
 __device__ __forceinline__ bool in_slab(int i, int n, int P) { return i < P || i >= n - P; }
 __device__ __forceinline__ int slab_s(int i, int n, int P) { return i < P ? i : i - (n - 2 * P); }
 __device__ __forceinline__ long long psi_index(const Dev& d, int a, int i, int j, int k) {
@@ -48,6 +59,9 @@ template <int V> __device__ __forceinline__ VF<V> ldv(const float* p) {
   if constexpr (V == 4) {
     const float4 t = *reinterpret_cast<const float4*>(p);
     r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w;
+  } else if constexpr (V == 2) {
+    const float2 t = *reinterpret_cast<const float2*>(p);
+    r.v[0] = t.x; r.v[1] = t.y;
   } else {
     r.v[0] = *p;
   }
@@ -56,6 +70,8 @@ template <int V> __device__ __forceinline__ VF<V> ldv(const float* p) {
 template <int V> __device__ __forceinline__ void stv(float* p, const VF<V>& r) {
   if constexpr (V == 4) {
     *reinterpret_cast<float4*>(p) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
+  } else if constexpr (V == 2) {
+    *reinterpret_cast<float2*>(p) = make_float2(r.v[0], r.v[1]);
   } else {
     *p = r.v[0];
   }

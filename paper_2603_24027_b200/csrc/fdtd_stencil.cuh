@@ -1,10 +1,13 @@
 // fdtd_stencil.cuh — the bandwidth-bound stencil kernels: forward E / H half-steps with fused CPML, the
 // inverse half-steps of the reverse run, the adjoint half-steps with the transposed CPML, gradient accumulation.
 //
-// Thread mapping (all kernels): block = 32 lanes x TY rows; a lane owns V consecutive z cells (V = 4: 16-byte
-// coalesced accesses, a warp covers 128 contiguous z cells = 512 B), threadIdx.y selects the y row.  The forward
-// kernels march along x over a chunk of planes and carry the x-neighbour plane in registers; y/z neighbours
-// come from L1/L2 (the rows are loaded by the same block in the same iteration).
+// Work split: every half-step is two launches that touch disjoint cells.
+//  * a LEAN kernel over the box of plain Yee cells (no CPML term, no wall): few registers, high occupancy,
+//    one thread = V = 4 consecutive z cells (16-byte accesses, a warp covers 512 contiguous bytes), TY rows per block,
+//    one x plane per block; x/y/z neighbours come from L1/L2 (DRAM traffic measured = algorithmic bytes);
+//  * a GENERAL kernel over the complement (the six slab boxes plus the layers that touch them): the same update
+//    with the CPML psi recursion fused in, V = 2 to halve its register footprint, and a per-box lane shape so that
+//    the thin z slabs still fill their warps.
 #pragma once
 #include "fdtd_dev.cuh"
 
@@ -12,18 +15,34 @@ namespace fdtd {
 
 constexpr int TY = 8;
 
+// block / thread -> (i, j, first k) inside the box list of a GENERAL kernel
+template <int V>
+__device__ __forceinline__ bool box_decode(const BoxList& B, int& i, int& j, int& k0) {
+  const int blk = blockIdx.x;
+  int b = 0;
+#pragma unroll
+  for (int g = 1; g < 6; ++g) b += (g < B.nb && blk >= B.off[g]);
+  const int local = blk - B.off[b];
+  const int bx = local % B.nbx[b];
+  const int t = local / B.nbx[b];
+  const int by = t % B.nby[b], bz = t / B.nby[b];
+  const int lzs = B.lzs[b];
+  const int zl = threadIdx.x & ((1 << lzs) - 1), yl = threadIdx.x >> lzs;
+  j = B.lo[b][1] + ((by * TY + threadIdx.y) << (5 - lzs)) + yl;
+  k0 = B.lo[b][2] + ((bx << lzs) + zl) * V;
+  i = B.lo[b][0] + bz;
+  return j < B.hi[b][1] && k0 < B.hi[b][2];
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Forward E half-step (SURVEY 8(a) rows A1 + A3):  E_c += ce * (d_a1^- H_b1 - d_a2^- H_b2) + CPML terms,
 // tangential E on the three low PEC walls held at zero.  DESIGN.md R1-R5.
 // ---------------------------------------------------------------------------------------------------------
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_fwd_e(const __grid_constant__ Dev d, int xch) {
+__global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
-  const int j = blockIdx.y * TY + threadIdx.y;
-  if (k0 >= nz || j >= ny) return;
-  const int i0 = blockIdx.z * xch;
-  const int i1 = min(nx, i0 + xch);
+  int i, j, k0;
+  if (!box_decode<V>(B, i, j, k0)) return;
   const long long sx = d.sx, sy = d.sy;
 
   bool zs[V];
@@ -40,13 +59,13 @@ __global__ void __launch_bounds__(32 * TY) k_fwd_e(const __grid_constant__ Dev d
   const float by = ys ? __ldg(d.tab[1][0] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][1] + j) : 0.0f,
               ky = ys ? __ldg(d.tab[1][2] + j) : 0.0f;
 
-  long long q = ((long long)i0 * ny + j) * nz + k0;
+  const long long q = ((long long)i * ny + j) * nz + k0;
   VF<V> pHy = zerov<V>(), pHz = zerov<V>();
-  if (i0 > 0) {
+  if (i > 0) {
     pHy = ldv<V>(d.H[1] + q - sx);
     pHz = ldv<V>(d.H[2] + q - sx);
   }
-  for (int i = i0; i < i1; ++i, q += sx) {
+  {
     const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
     VF<V> hx_ym = zerov<V>(), hz_ym = zerov<V>();
     if (j > 0) {
@@ -116,8 +135,6 @@ __global__ void __launch_bounds__(32 * TY) k_fwd_e(const __grid_constant__ Dev d
       stv<V>(d.psiE[0][1] + qz, p_ex_z);
       stv<V>(d.psiE[1][0] + qz, p_ey_z);
     }
-    pHy = hy;
-    pHz = hz;
   }
 }
 
@@ -125,13 +142,10 @@ __global__ void __launch_bounds__(32 * TY) k_fwd_e(const __grid_constant__ Dev d
 // Forward H half-step (rows A2 + A4):  H_c -= S * (d_a1^+ E_b1 - d_a2^+ E_b2) + CPML terms; ghost E[n] = 0.
 // ---------------------------------------------------------------------------------------------------------
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_fwd_h(const __grid_constant__ Dev d, int xch) {
+__global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
-  const int j = blockIdx.y * TY + threadIdx.y;
-  if (k0 >= nz || j >= ny) return;
-  const int i0 = blockIdx.z * xch;
-  const int i1 = min(nx, i0 + xch);
+  int i, j, k0;
+  if (!box_decode<V>(B, i, j, k0)) return;
   const long long sx = d.sx, sy = d.sy;
   const float mS = -d.S;
 
@@ -149,9 +163,9 @@ __global__ void __launch_bounds__(32 * TY) k_fwd_h(const __grid_constant__ Dev d
   const float by = ys ? __ldg(d.tab[1][3] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][4] + j) : 0.0f,
               ky = ys ? __ldg(d.tab[1][5] + j) : 0.0f;
 
-  long long q = ((long long)i0 * ny + j) * nz + k0;
-  VF<V> ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);   // plane i (carried), next plane loaded per iteration
-  for (int i = i0; i < i1; ++i, q += sx) {
+  const long long q = ((long long)i * ny + j) * nz + k0;
+  const VF<V> ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  {
     const VF<V> ex = ldv<V>(d.E[0] + q);
     VF<V> ey_xp = zerov<V>(), ez_xp = zerov<V>();
     if (i + 1 < nx) {
@@ -221,8 +235,6 @@ __global__ void __launch_bounds__(32 * TY) k_fwd_h(const __grid_constant__ Dev d
       stv<V>(d.psiH[0][1] + qz, p_hx_z);
       stv<V>(d.psiH[1][0] + qz, p_hy_z);
     }
-    ey = ey_xp;
-    ez = ez_xp;
   }
 }
 
@@ -335,12 +347,10 @@ struct WTerm {  // W(q) - W(q - stride_a) of one transposed H term, evaluated by
 };
 
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_adj_h(const __grid_constant__ Dev d, int pb) {
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
-  const int j = blockIdx.y * TY + threadIdx.y;
-  const int i = blockIdx.z;
-  if (k0 >= nz || j >= ny) return;
+  int i, j, k0;
+  if (!box_decode<V>(B, i, j, k0)) return;
   const long long sx = d.sx, sy = d.sy;
   const long long q = ((long long)i * ny + j) * nz + k0;
   const float S = d.S;
@@ -494,12 +504,10 @@ __global__ void __launch_bounds__(32 * TY) k_adj_h(const __grid_constant__ Dev d
 // (skipped on PEC-masked E_c nodes), lH_b -= d_a^+(W).
 // ---------------------------------------------------------------------------------------------------------
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_adj_e(const __grid_constant__ Dev d, int pb) {
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  const int k0 = (blockIdx.x * 32 + threadIdx.x) * V;
-  const int j = blockIdx.y * TY + threadIdx.y;
-  const int i = blockIdx.z;
-  if (k0 >= nz || j >= ny) return;
+  int i, j, k0;
+  if (!box_decode<V>(B, i, j, k0)) return;
   const long long sx = d.sx, sy = d.sy;
   const long long q = ((long long)i * ny + j) * nz + k0;
   const VF<V> ce = ldv<V>(d.ce + q);
@@ -653,6 +661,114 @@ __global__ void __launch_bounds__(32 * TY) k_adj_e(const __grid_constant__ Dev d
     stv<V>(d.lpsiE[nb][0][1] + qz, n01);
     stv<V>(d.lpsiE[nb][1][0] + qz, n10);
   }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// LEAN kernels: plain Yee cells only (region chosen by the host so that no CPML term, no PEC mask and no ghost
+// applies, and — for the adjoint — no neighbour W term either).  Grid: x = z groups, y = row tiles, z = planes.
+// Same canonical arithmetic as the general kernels (R3), so results are bit-identical to them.
+// ---------------------------------------------------------------------------------------------------------
+template <int V>
+__device__ __forceinline__ bool lean_decode(const Region& r, int& i, int& j, int& k0) {
+  k0 = r.lo[2] + (blockIdx.x * 32 + threadIdx.x) * V;
+  j = r.lo[1] + blockIdx.y * TY + threadIdx.y;
+  i = r.lo[0] + blockIdx.z;
+  return k0 < r.hi[2] && j < r.hi[1];
+}
+
+// ADJ = false: forward E half-step   E_c  = fma(ce, curl^-(H)_c,  E_c)      (row A1)
+// ADJ = true : adjoint of H half-step lE_c = fma(-S, curl^-(lH)_c, lE_c)     (row R4)
+template <int V, bool ADJ>
+__global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V>(r, i, j, k0)) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const float* const* in = ADJ ? d.lH : d.H;
+  float* const* out = ADJ ? d.lE : d.E;
+  const VF<V> hx = ldv<V>(in[0] + q), hy = ldv<V>(in[1] + q), hz = ldv<V>(in[2] + q);
+  const VF<V> hy_xm = ldv<V>(in[1] + q - sx), hz_xm = ldv<V>(in[2] + q - sx);
+  const VF<V> hx_ym = ldv<V>(in[0] + q - sy), hz_ym = ldv<V>(in[2] + q - sy);
+  const float hx_z0 = in[0][q - 1], hy_z0 = in[1][q - 1];
+  VF<V> ex = ldv<V>(out[0] + q), ey = ldv<V>(out[1] + q), ez = ldv<V>(out[2] + q);
+  VF<V> ce;
+  if (!ADJ) ce = ldv<V>(d.ce + q);
+  const float mS = -d.S;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+    const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+    const float c = ADJ ? mS : ce.v[v];
+    ex.v[v] = fmaf(c, (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex.v[v]);
+    ey.v[v] = fmaf(c, (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey.v[v]);
+    ez.v[v] = fmaf(c, (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez.v[v]);
+  }
+  stv<V>(out[0] + q, ex);
+  stv<V>(out[1] + q, ey);
+  stv<V>(out[2] + q, ez);
+}
+
+// forward H half-step on plain cells:  H_c = fma(-S, curl^+(E)_c, H_c)   (row A2)
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V>(r, i, j, k0)) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  const VF<V> ey_xp = ldv<V>(d.E[1] + q + sx), ez_xp = ldv<V>(d.E[2] + q + sx);
+  const VF<V> ex_yp = ldv<V>(d.E[0] + q + sy), ez_yp = ldv<V>(d.E[2] + q + sy);
+  const float ex_zp = d.E[0][q + V], ey_zp = d.E[1][q + V];
+  VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  const float mS = -d.S;
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const float ey_zq = v == V - 1 ? ey_zp : ey.v[v < V - 1 ? v + 1 : v];
+    const float ex_zq = v == V - 1 ? ex_zp : ex.v[v < V - 1 ? v + 1 : v];
+    hx.v[v] = fmaf(mS, (ez_yp.v[v] - ez.v[v]) - (ey_zq - ey.v[v]), hx.v[v]);
+    hy.v[v] = fmaf(mS, (ex_zq - ex.v[v]) - (ez_xp.v[v] - ez.v[v]), hy.v[v]);
+    hz.v[v] = fmaf(mS, (ey_xp.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
+  }
+  stv<V>(d.H[0] + q, hx);
+  stv<V>(d.H[1] + q, hy);
+  stv<V>(d.H[2] + q, hz);
+}
+
+// adjoint of the E half-step on plain cells:  lH_h = lH_h + curl^+(ce*lE)_h   (row R4)
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V>(r, i, j, k0)) return;
+  const long long sx = d.sx, sy = d.sy;
+  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const VF<V> ce = ldv<V>(d.ce + q), ce_xp = ldv<V>(d.ce + q + sx), ce_yp = ldv<V>(d.ce + q + sy);
+  const float ce_zp = d.ce[q + V];
+  VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
+  VF<V> gy_xp = ldv<V>(d.lE[1] + q + sx), gz_xp = ldv<V>(d.lE[2] + q + sx);
+  VF<V> gx_yp = ldv<V>(d.lE[0] + q + sy), gz_yp = ldv<V>(d.lE[2] + q + sy);
+  const float gx_zp = ce_zp * d.lE[0][q + V], gy_zp = ce_zp * d.lE[1][q + V];
+  VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    gx.v[v] = ce.v[v] * gx.v[v];
+    gy.v[v] = ce.v[v] * gy.v[v];
+    gz.v[v] = ce.v[v] * gz.v[v];
+    gy_xp.v[v] = ce_xp.v[v] * gy_xp.v[v];
+    gz_xp.v[v] = ce_xp.v[v] * gz_xp.v[v];
+    gx_yp.v[v] = ce_yp.v[v] * gx_yp.v[v];
+    gz_yp.v[v] = ce_yp.v[v] * gz_yp.v[v];
+  }
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const float gx_zq = v == V - 1 ? gx_zp : gx.v[v < V - 1 ? v + 1 : v];
+    const float gy_zq = v == V - 1 ? gy_zp : gy.v[v < V - 1 ? v + 1 : v];
+    lhx.v[v] = lhx.v[v] + ((gz_yp.v[v] - gz.v[v]) - (gy_zq - gy.v[v]));
+    lhy.v[v] = lhy.v[v] + ((gx_zq - gx.v[v]) - (gz_xp.v[v] - gz.v[v]));
+    lhz.v[v] = lhz.v[v] + ((gy_xp.v[v] - gy.v[v]) - (gx_yp.v[v] - gx.v[v]));
+  }
+  stv<V>(d.lH[0] + q, lhx);
+  stv<V>(d.lH[1] + q, lhy);
+  stv<V>(d.lH[2] + q, lhz);
 }
 
 }  // namespace fdtd

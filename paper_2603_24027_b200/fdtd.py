@@ -73,6 +73,7 @@ def lib():
     L.fdtd_reverse_host.argtypes = [vp, vp, C.c_int, vp]
     L.fdtd_codec_encode.argtypes = [C.c_int, vp, C.c_size_t, vp, vp, vp, vp]
     L.fdtd_codec_fetch.argtypes = [C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_float), C.c_int, C.c_int, C.c_size_t, vp, vp]
+    L.fdtd_profile_kernel.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.fdtd_sync.argtypes = [vp]
     L.fdtd_last_error.restype = C.c_char_p
     L.fdtd_last_error.argtypes = [vp]
@@ -87,7 +88,7 @@ EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
             "fdtd_set_graphs", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
-            "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
+            "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count"]
 
 
@@ -311,6 +312,14 @@ class Sim:
 
     def sync(self):
         self._check(self._L.fdtd_sync(self._h))
+
+    KERNELS = ["fwd_e", "fwd_h", "inv_h", "adj_h", "grad_inv_e", "adj_e", "record", "inject_h", "inject_e"]
+
+    def profile_kernel(self, kernel_id, warm=5, reps=50):
+        """(mean ms per launch, algorithmic bytes per launch) of one kernel timed alone, back to back (fdtd_profile_kernel)."""
+        ms, by = C.c_double(), C.c_double()
+        self._check(self._L.fdtd_profile_kernel(self._h, int(kernel_id), int(warm), int(reps), C.byref(ms), C.byref(by)))
+        return ms.value, by.value
 
     def launch_count(self):
         return int(self._L.fdtd_launch_count(self._h))
