@@ -42,6 +42,12 @@ struct fdtd_sim {
   int P = 0;
   double dx = 0, dt = 0, Sd = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t cur = nullptr;          // stream the next LAUNCH goes to (fork / on / join)
+  cudaStream_t aux[3] = {nullptr, nullptr, nullptr};
+  cudaStream_t cap = nullptr;          // origin stream of graph captures (the caller's stream may be the legacy default)
+  cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+  bool parallel = false;               // auxiliary streams available
+  std::vector<cudaGraphExec_t> dead_graphs;
   mutable std::string err;
   const float* eps_dev = nullptr;
   double cpml[4] = {0.8, 1.0, 0.01, 3.0};
@@ -269,32 +275,51 @@ bool grid_inner(const fdtd_sim* s, dim3* g) {
 
 #define LAUNCH(s, kern, grid, block, ...)            \
   do {                                               \
-    kern<<<grid, block, 0, (s)->stream>>>(__VA_ARGS__); \
+    kern<<<grid, block, 0, (s)->cur>>>(__VA_ARGS__); \
     ++(s)->launches;                                 \
   } while (0)
 
-// The four split half-steps: lean kernel on the plain cells + general kernel on the rest (disjoint writes).
-void launch_split(fdtd_sim* s, int which, int pb) {
+// ---- fork / join over the handle's auxiliary streams: kernels of one phase that touch disjoint data run side by
+// side.  Under stream capture these become parallel branches of the CUDA graph; outside they are plain streams. ----
+void fork(fdtd_sim* s, int branches) {
+  s->cur = s->stream;
+  if (!s->parallel) return;
+  cudaEventRecord(s->ev_fork, s->stream);
+  for (int b = 1; b < branches; ++b) cudaStreamWaitEvent(s->aux[b - 1], s->ev_fork, 0);
+}
+void on(fdtd_sim* s, int branch) { s->cur = (s->parallel && branch > 0) ? s->aux[branch - 1] : s->stream; }
+void join(fdtd_sim* s, int branches) {
+  s->cur = s->stream;
+  if (!s->parallel) return;
+  for (int b = 1; b < branches; ++b) {
+    cudaEventRecord(s->ev_join[b - 1], s->aux[b - 1]);
+    cudaStreamWaitEvent(s->stream, s->ev_join[b - 1], 0);
+  }
+}
+
+void launch_lean(fdtd_sim* s, int which) {
+  if (!s->has_lean[which]) return;
   const dim3 b(32, TY);
-  if (s->has_lean[which]) {
-    const dim3 g = grid_lean(s, which);
-    const Region& r = s->reg[which];
-    if (s->V == 4) {
-      switch (which) {
-        case 0: LAUNCH(s, (k_lean_curlm<4, false>), g, b, s->d, r); break;
-        case 1: LAUNCH(s, k_lean_h<4>, g, b, s->d, r); break;
-        case 2: LAUNCH(s, (k_lean_curlm<4, true>), g, b, s->d, r); break;
-        default: LAUNCH(s, k_lean_adj_e<4>, g, b, s->d, r);
-      }
-    } else {
-      switch (which) {
-        case 0: LAUNCH(s, (k_lean_curlm<1, false>), g, b, s->d, r); break;
-        case 1: LAUNCH(s, k_lean_h<1>, g, b, s->d, r); break;
-        case 2: LAUNCH(s, (k_lean_curlm<1, true>), g, b, s->d, r); break;
-        default: LAUNCH(s, k_lean_adj_e<1>, g, b, s->d, r);
-      }
+  const dim3 g = grid_lean(s, which);
+  const Region& r = s->reg[which];
+  if (s->V == 4) {
+    switch (which) {
+      case 0: LAUNCH(s, (k_lean_curlm<4, false>), g, b, s->d, r); break;
+      case 1: LAUNCH(s, k_lean_h<4>, g, b, s->d, r); break;
+      case 2: LAUNCH(s, (k_lean_curlm<4, true>), g, b, s->d, r); break;
+      default: LAUNCH(s, k_lean_adj_e<4>, g, b, s->d, r);
+    }
+  } else {
+    switch (which) {
+      case 0: LAUNCH(s, (k_lean_curlm<1, false>), g, b, s->d, r); break;
+      case 1: LAUNCH(s, k_lean_h<1>, g, b, s->d, r); break;
+      case 2: LAUNCH(s, (k_lean_curlm<1, true>), g, b, s->d, r); break;
+      default: LAUNCH(s, k_lean_adj_e<1>, g, b, s->d, r);
     }
   }
+}
+void launch_gen(fdtd_sim* s, int which, int pb) {
+  const dim3 b(32, TY);
   const BoxList& B = s->boxes[which];
   const unsigned g = (unsigned)B.off[B.nb];
   if (g == 0) return;
@@ -314,8 +339,27 @@ void launch_split(fdtd_sim* s, int which, int pb) {
     }
   }
 }
+// The four split half-steps: lean kernel on the plain cells + general kernel on the rest (disjoint writes).
+void launch_split(fdtd_sim* s, int which, int pb) {
+  launch_lean(s, which);
+  launch_gen(s, which, pb);
+}
 void launch_fwd_e(fdtd_sim* s) { launch_split(s, 0, 0); }
 void launch_fwd_h(fdtd_sim* s) { launch_split(s, 1, 0); }
+void launch_inv_h(fdtd_sim* s) {
+  dim3 gi;
+  if (!grid_inner(s, &gi)) return;
+  const dim3 b(32, TY);
+  if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
+  else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
+}
+void launch_grad_inv_e(fdtd_sim* s) {
+  dim3 gi;
+  if (!grid_inner(s, &gi)) return;
+  const dim3 b(32, TY);
+  if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d);
+  else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d);
+}
 void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
   if (s->nsrc == 0) return;
   long long maxc = 1;
@@ -333,15 +377,17 @@ void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int*
   if (tot <= 0) return;
   LAUNCH(s, k_box, (unsigned)((tot + 255) / 256), 256, s->d, b, rec, m_base, step_dev, mode);
 }
-void launch_record(fdtd_sim* s, int m_base, const int* step_dev) {
-  const unsigned g = (unsigned)((s->st.slot_values + 255) / 256);
+// half: 0 = E components, 1 = H components, 2 = all six
+void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
+  const long long items = s->st.cell_off[6] * (half == 2 ? 6 : 3);
+  const unsigned g = (unsigned)((items + 255) / 256);
   switch (s->dtype) {
-    case DT_F32: LAUNCH(s, k_record<DT_F32>, g, 256, s->d, s->st, m_base, step_dev); break;
-    case DT_F16: LAUNCH(s, k_record<DT_F16>, g, 256, s->d, s->st, m_base, step_dev); break;
-    case DT_BF16: LAUNCH(s, k_record<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev); break;
+    case DT_F32: LAUNCH(s, k_record<DT_F32>, g, 256, s->d, s->st, m_base, step_dev, half); break;
+    case DT_F16: LAUNCH(s, k_record<DT_F16>, g, 256, s->d, s->st, m_base, step_dev, half); break;
+    case DT_BF16: LAUNCH(s, k_record<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev, half); break;
     default:
-      LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev);
-      LAUNCH(s, k_record<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev);
+      LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
+      LAUNCH(s, k_record<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev, half);
   }
 }
 void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp) {
@@ -355,33 +401,75 @@ void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, i
 }
 
 // One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
-void forward_step(fdtd_sim* s, int m_base, const int* step_dev, bool record) {
-  launch_fwd_e(s);
+// Phase E: {lean E, general E, record of the H half of the previous state if one is pending (H is read-only here)}.
+// Phase H: {lean H, general H, record of the E half of state m if due (E is read-only here)}.
+// pending_h carries "state m-1 still needs its H half recorded" in and "state m ..." out.
+void forward_step(fdtd_sim* s, int m_base, const int* step_dev, bool record, bool* pending_h) {
+  fork(s, 3);
+  on(s, 0); launch_lean(s, 0);
+  on(s, 1); launch_gen(s, 0, 0);
+  if (*pending_h) { on(s, 2); launch_record(s, m_base - 1, step_dev, 1); }
+  join(s, 3);
   launch_sources(s, m_base, step_dev, 1.0f);
-  launch_fwd_h(s);
+  fork(s, 3);
+  on(s, 0); launch_lean(s, 1);
+  on(s, 1); launch_gen(s, 1, 0);
+  if (record) { on(s, 2); launch_record(s, m_base, step_dev, 0); }
+  join(s, 3);
   if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0);
-  if (record) launch_record(s, m_base, step_dev);
+  *pending_h = record;
 }
 
-// One reverse step m -> m-1 (R9).
+// One reverse step m -> m-1 (R9), as two phases of mutually independent kernels:
+//  1: {adjoint-H lean, adjoint-H general, inverse-H (inner interior), inject H (shell)}
+//  2: {adjoint-E lean, adjoint-E general, gradient + inverse-E (inner interior), inject E + shell gradient}
 void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
-  const dim3 b(32, TY);
   if (dmon && s->has_mon) launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
-  dim3 gi;
-  const bool inner = grid_inner(s, &gi);
-  if (inner) {
-    if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
-    else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
-  }
-  launch_split(s, 2, pb);
-  launch_inject(s, m_base, step_dev, 1, interp);
+  fork(s, 4);
+  on(s, 0); launch_lean(s, 2);
+  on(s, 1); launch_gen(s, 2, pb);
+  on(s, 2); launch_inv_h(s);
+  on(s, 3); launch_inject(s, m_base, step_dev, 1, interp);
+  join(s, 4);
   launch_sources(s, m_base, step_dev, -1.0f);
-  if (inner) {
-    if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d);
-    else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d);
+  fork(s, 4);
+  on(s, 0); launch_lean(s, 3);
+  on(s, 1); launch_gen(s, 3, pb);
+  on(s, 2); launch_grad_inv_e(s);
+  on(s, 3); launch_inject(s, m_base, step_dev, 0, interp);
+  join(s, 4);
+}
+
+// Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.
+template <class F>
+fdtd_status run_graph(fdtd_sim* s, int times, F body) {
+  if (times <= 0) return FDTD_OK;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  const unsigned long long before = s->launches;
+  cudaStream_t user = s->stream;
+  CUDA_TRY(s, cudaStreamBeginCapture(s->cap, cudaStreamCaptureModeThreadLocal));
+  s->stream = s->cur = s->cap;
+  body();
+  s->stream = s->cur = user;
+  cudaError_t e = cudaStreamEndCapture(s->cap, &graph);
+  if (e != cudaSuccess || !graph) return fail(s, FDTD_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+  const unsigned long long per = s->launches - before;
+  e = cudaGraphInstantiate(&exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+  for (int r = 0; r < times; ++r) {
+    e = cudaGraphLaunch(exec, s->stream);
+    if (e != cudaSuccess) break;
   }
-  launch_inject(s, m_base, step_dev, 0, interp);
-  launch_split(s, 3, pb);
+  s->launches = before + per * (unsigned long long)times;
+  s->dead_graphs.push_back(exec);   // destroyed at the next sync point (the launches above are still in flight)
+  if (e != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "graph launch failed: %s", cudaGetErrorString(e));
+  return FDTD_OK;
+}
+void reap_graphs(fdtd_sim* s) {
+  for (cudaGraphExec_t g : s->dead_graphs) cudaGraphExecDestroy(g);
+  s->dead_graphs.clear();
 }
 
 fdtd_status zero_state(fdtd_sim* s) {
@@ -472,8 +560,31 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
   s->st.nslots = slots; s->st.nsteps = nsteps; s->st.k = k; s->st.dtype = (int)dt;
   s->st.slot_bytes = (size_t)slot_values(s) * elem_bytes_host(dt);
   if (dt == FDTD_F8E4M3_SCALED) CUDA_TRY(s, cudaMemsetAsync(s->st.amax, 0, (size_t)slots * 36 * 4, s->stream));
-  launch_record(s, 0, nullptr);                       // state 0 (R10)
-  for (int m = 1; m <= nsteps; ++m) forward_step(s, m, nullptr, m % k == 0 || m == nsteps);
+  s->cur = s->stream;
+  if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
+  // state 0 (R10): its E half now, its H half during the first E phase (H is untouched until then)
+  launch_record(s, 0, nullptr, 0);
+  bool pend = true;
+  int done = 0;
+  // steady-state period of L = k*r steps as one CUDA graph: every period starts and ends with a pending H half
+  const int L = k * std::max(1, (16 + k - 1) / k);
+  const int periods = (s->use_graphs && s->aux[0]) ? nsteps / L : 0;
+  if (periods > 0) {
+    int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
+    LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
+    s->parallel = true;
+    fdtd_status g = run_graph(s, periods, [&]() {
+      bool p = true;
+      for (int t = 1; t <= L; ++t) forward_step(s, t, step_dev, t % k == 0, &p);
+      LAUNCH(s, k_tick, 1, 1, step_dev, L);
+    });
+    s->parallel = false;
+    s->cur = s->stream;
+    if (g != FDTD_OK) return g;
+    done = periods * L;
+  }
+  for (int m = done + 1; m <= nsteps; ++m) forward_step(s, m, nullptr, m % k == 0 || m == nsteps, &pend);
+  if (pend) launch_record(s, nsteps, nullptr, 1);
   CUDA_TRY(s, cudaGetLastError());
   s->forward_done = s->state_final = true;
   return FDTD_OK;
@@ -486,6 +597,8 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   if ((int)interp < 0 || (int)interp > 1) return fail(s, FDTD_ERR_INVALID_ARG, "unknown interpolation %d", (int)interp);
   if (dmon && !s->has_mon) return fail(s, FDTD_ERR_INVALID_ARG, "dL_dmon given but no monitor is set");
   const size_t N = (size_t)s->d.N;
+  s->cur = s->stream;
+  if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
   for (int c = 0; c < 3; ++c) {
     CUDA_TRY(s, cudaMemsetAsync(s->d.lE[c], 0, N * 4, s->stream));
     CUDA_TRY(s, cudaMemsetAsync(s->d.lH[c], 0, N * 4, s->stream));
@@ -509,7 +622,25 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   }
   s->state_final = false;
   int pb = 0;
-  for (int m = s->nsteps; m >= 1; --m, pb ^= 1) reverse_step(s, m, nullptr, dmon, (int)interp, pb);
+  int top = s->nsteps;
+  {
+    const int L = 16;   // even, so the psi ping-pong parity is the same at the start of every period
+    const int periods = (s->use_graphs && s->aux[0]) ? s->nsteps / L : 0;
+    if (periods > 0) {
+      int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
+      LAUNCH(s, k_set_int, 1, 1, step_dev, s->nsteps);
+      s->parallel = true;
+      fdtd_status g = run_graph(s, periods, [&]() {
+        for (int t = 0; t < L; ++t) reverse_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+        LAUNCH(s, k_tick, 1, 1, step_dev, -L);
+      });
+      s->parallel = false;
+      s->cur = s->stream;
+      if (g != FDTD_OK) return g;
+      top -= periods * L;
+    }
+  }
+  for (int m = top; m >= 1; --m, pb ^= 1) reverse_step(s, m, nullptr, dmon, (int)interp, pb);
   if (grad_dev && s->has_design)
     LAUNCH(s, k_grad_finalize, (unsigned)((design_cells(s) + 255) / 256), 256, s->d, s->eps_dev, grad_dev);
   CUDA_TRY(s, cudaGetLastError());
@@ -534,6 +665,13 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   s->n[0] = nx; s->n[1] = ny; s->n[2] = nz; s->P = pml_width; s->dx = dx; s->dt = dt; s->Sd = S;
   s->eps_dev = eps_dev;
   s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  s->cur = s->stream;
+  bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+  for (int b = 0; b < 3 && ok; ++b)
+    ok = cudaStreamCreateWithFlags(&s->aux[b], cudaStreamNonBlocking) == cudaSuccess &&
+         cudaEventCreateWithFlags(&s->ev_join[b], cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaStreamCreateWithFlags(&s->cap, cudaStreamNonBlocking) == cudaSuccess;
+  if (!ok) { for (int b = 0; b < 3; ++b) s->aux[b] = nullptr; cudaGetLastError(); }   // graphs off, serial launches
   *out = s;
   return FDTD_OK;
 }
@@ -812,19 +950,17 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
   if (id >= 6 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
-  const dim3 b(32, TY);
-  dim3 gi;
-  const bool inner = grid_inner(s, &gi);
+  s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
   auto once = [&]() {
     switch (id) {
       case 0: launch_fwd_e(s); break;
       case 1: launch_fwd_h(s); break;
-      case 2: if (inner) { if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d); else LAUNCH(s, k_inv_h<1>, gi, b, s->d); } break;
+      case 2: launch_inv_h(s); break;
       case 3: launch_split(s, 2, 0); break;
-      case 4: if (inner) { if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d); else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d); } break;
+      case 4: launch_grad_inv_e(s); break;
       case 5: launch_split(s, 3, 0); break;
-      case 6: launch_record(s, s->nsteps, nullptr); break;
+      case 6: launch_record(s, s->nsteps, nullptr, 2); break;
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
       default: launch_inject(s, mrev, nullptr, 0, 0); break;
     }
@@ -878,12 +1014,24 @@ fdtd_status fdtd_sync(fdtd_sim* s) {
   if (!s) return FDTD_ERR_INVALID_ARG;
   CUDA_TRY(s, cudaStreamSynchronize(s->stream));
   CUDA_TRY(s, cudaGetLastError());
+  reap_graphs(s);
   return FDTD_OK;
 }
 
 const char* fdtd_last_error(const fdtd_sim* s) { return s ? s->err.c_str() : "null handle"; }
 
-void fdtd_destroy(fdtd_sim* s) { delete s; }
+void fdtd_destroy(fdtd_sim* s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  reap_graphs(s);
+  for (int b = 0; b < 3; ++b) {
+    if (s->aux[b]) cudaStreamDestroy(s->aux[b]);
+    if (s->ev_join[b]) cudaEventDestroy(s->ev_join[b]);
+  }
+  if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->cap) cudaStreamDestroy(s->cap);
+  delete s;
+}
 
 unsigned long long fdtd_launch_count(const fdtd_sim* s) { return s ? s->launches : 0; }
 

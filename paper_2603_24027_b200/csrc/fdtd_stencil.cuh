@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d
 
 // ---------------------------------------------------------------------------------------------------------
 // Reverse run, primal reconstruction on the inner interior (row R2).  One thread = one (i, j, z-group);
-// elements outside the inner interior keep their value.  Grid: x = z groups, y = rows from P+1, z = planes
+// elements outside the inner interior are neither computed nor written.  Grid: x = z groups, y = rows from P+1, z = planes
 // from P+1.
 // ---------------------------------------------------------------------------------------------------------
 // inverse of the H half-step:  H^{m-1/2} = H^{m+1/2} + S * curl^+(E^m)
@@ -274,9 +274,20 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
     hy.v[v] = fmaf(S, (ex_zq - ex.v[v]) - (ez_xp.v[v] - ez.v[v]), hy.v[v]);
     hz.v[v] = fmaf(S, (ey_xp.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
   }
-  stv<V>(d.H[0] + q, hx);
-  stv<V>(d.H[1] + q, hy);
-  stv<V>(d.H[2] + q, hz);
+  // a group that straddles the shell must not touch the shell cells: inject H runs concurrently with this kernel
+  if (k0 >= klo && k0 + V <= khi) {
+    stv<V>(d.H[0] + q, hx);
+    stv<V>(d.H[1] + q, hy);
+    stv<V>(d.H[2] + q, hz);
+  } else {
+#pragma unroll
+    for (int v = 0; v < V; ++v)
+      if (k0 + v >= klo && k0 + v < khi) {
+        d.H[0][q + v] = hx.v[v];
+        d.H[1][q + v] = hy.v[v];
+        d.H[2][q + v] = hz.v[v];
+      }
+  }
 }
 
 // gradient term (row R3) + inverse of the E half-step (row R2), fused since both need curl^-(H^{m-1/2}):
@@ -331,9 +342,19 @@ __global__ void __launch_bounds__(32 * TY) k_grad_inv_e(const __grid_constant__ 
     ey.v[v] = fmaf(-ce.v[v], cy, ey.v[v]);
     ez.v[v] = fmaf(-ce.v[v], cz, ez.v[v]);
   }
-  stv<V>(d.E[0] + q, ex);
-  stv<V>(d.E[1] + q, ey);
-  stv<V>(d.E[2] + q, ez);
+  if (k0 >= klo && k0 + V <= khi) {   // see k_inv_h: inject E runs concurrently on the shell cells
+    stv<V>(d.E[0] + q, ex);
+    stv<V>(d.E[1] + q, ey);
+    stv<V>(d.E[2] + q, ez);
+  } else {
+#pragma unroll
+    for (int v = 0; v < V; ++v)
+      if (k0 + v >= klo && k0 + v < khi) {
+        d.E[0][q + v] = ex.v[v];
+        d.E[1][q + v] = ey.v[v];
+        d.E[2][q + v] = ez.v[v];
+      }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -146,17 +146,34 @@ __device__ __forceinline__ int record_slot(const StoreDev& s, int m) {
 // Record (row A5).  Phase 1 (fp8 only): per-slice absmax, warp-reduced, one atomicMax per (warp, slice).
 // Phase 2: gather the 36 slices from the field arrays, cast, write the slot.
 // ---------------------------------------------------------------------------------------------------------
+// half = 0: the three E components, 1: the three H components, 2: all six.  The two halves of a slot can be written
+// by different launches: E^m is final after the E half-step, H^{m+1/2} after the H half-step.
+struct RecItem { int f, comp; long long e, vidx; };
+__device__ __forceinline__ bool record_item(const StoreDev& s, long long t, int half, RecItem& it) {
+  const int nc = half == 2 ? 6 : 3;
+  if (t >= s.cell_off[6] * nc) return false;
+  // t enumerates [face][comp in half][element]; cell_off = prefix sums of face sizes
+  int f = 0;
+#pragma unroll
+  for (int g = 1; g < 6; ++g) f += (t >= s.cell_off[g] * nc);
+  const long long fs = s.cell_off[f + 1] - s.cell_off[f];
+  const long long r = t - s.cell_off[f] * nc;
+  it.f = f;
+  it.comp = (int)(r / fs) + (half == 1 ? 3 : 0);
+  it.e = r % fs;
+  it.vidx = s.val_off[f] + it.comp * fs + it.e;
+  return true;
+}
+
 __global__ void __launch_bounds__(256) k_record_amax(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
-                                                      int m_base, const int* step_dev) {
+                                                      int m_base, const int* step_dev, int half) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= s.slot_values) return;
+  RecItem it;
+  if (!record_item(s, t, half, it)) return;
   const int slot = record_slot(s, cur_step(m_base, step_dev));
-  const int f = find_face(s.val_off, t);
-  const long long fs = (long long)s.du[f] * s.dv[f];
-  const long long r = t - s.val_off[f];
-  const int comp = (int)(r / fs);
+  const int f = it.f, comp = it.comp;
   int c[3];
-  face_cell(d, s, f, r % fs, c);
+  face_cell(d, s, f, it.e, c);
   const float x = field_ptr(d, comp)[((long long)c[0] * d.n[1] + c[1]) * d.n[2] + c[2]];
   const unsigned bits = __float_as_uint(fabsf(x));
   const unsigned key = f * 6 + comp;
@@ -168,16 +185,14 @@ __global__ void __launch_bounds__(256) k_record_amax(const __grid_constant__ Dev
 
 template <int DT>
 __global__ void __launch_bounds__(256) k_record(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
-                                                int m_base, const int* step_dev) {
+                                                int m_base, const int* step_dev, int half) {
   typedef typename Codec<DT>::code_t code_t;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= s.slot_values) return;
+  RecItem it;
+  if (!record_item(s, t, half, it)) return;
   const int slot = record_slot(s, cur_step(m_base, step_dev));
-  const int f = find_face(s.val_off, t);
-  const long long fs = (long long)s.du[f] * s.dv[f];
-  const long long r = t - s.val_off[f];
-  const int comp = (int)(r / fs);
-  const long long e = r % fs;
+  const int f = it.f, comp = it.comp;
+  const long long e = it.e;
   int c[3];
   face_cell(d, s, f, e, c);
   const float x = field_ptr(d, comp)[((long long)c[0] * d.n[1] + c[1]) * d.n[2] + c[2]];
@@ -187,7 +202,7 @@ __global__ void __launch_bounds__(256) k_record(const __grid_constant__ Dev d, c
     inv = amax > 0.0f ? 448.0f / amax : 0.0f;
     if (e == 0) s.scales[(size_t)slot * 36 + f * 6 + comp] = amax > 0.0f ? amax / 448.0f : 0.0f;
   }
-  reinterpret_cast<code_t*>(s.base + (size_t)slot * s.slot_bytes)[t] = Codec<DT>::enc(x, inv);
+  reinterpret_cast<code_t*>(s.base + (size_t)slot * s.slot_bytes)[it.vidx] = Codec<DT>::enc(x, inv);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -299,6 +314,7 @@ __global__ void k_box(const __grid_constant__ Dev d, const __grid_constant__ Box
 }
 
 __global__ void k_tick(int* step_dev, int delta) { *step_dev += delta; }
+__global__ void k_set_int(int* p, int v) { *p = v; }
 
 // ce = fl(S * fl(1/eps)) (R3); also the minimum of eps for validation
 __global__ void k_make_ce(const float* __restrict__ eps, float* __restrict__ ce, long long N, float S) {
