@@ -66,7 +66,7 @@ typedef struct {
 
 /* Create a simulation (eq. 1): grid nx*ny*nz cells of size dx [m], time step dt [s] (must satisfy
  * dt <= dx/(c*sqrt(3)); the Courant number used by the kernels is S = c*dt/dx), CPML of pml_width cells on all six
- * faces backed by a PEC wall (R3,R5), relative permittivity eps_dev[nx][ny][nz] (all >= 1; read during
+ * faces backed by a PEC wall (R4,R5), relative permittivity eps_dev[nx][ny][nz] (all >= 1; read during
  * fdtd_set_workspace / fdtd_set_eps, and again by fdtd_reverse, so it must stay valid and unchanged).
  * cuda_stream is a cudaStream_t (NULL = default stream).  Requires n_a - 2*pml_width >= 2 on every axis.
  * Synchronises once (eps validation). */

@@ -172,7 +172,7 @@ BY_NAME = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "tiny": tiny}
 # ----------------------------------------------------------------------------------------------------
 # Objectives (harness level: SURVEY.md layer L4; PAPER.md:45,51 measure Poynting flux through detectors).
 # Each returns (L, dmon) with dmon = dL/d(monitor record), same shape as the record, float64.
-# E and H are taken as stored (co-indexed, half a step apart): synthetic objectives (R8).
+# E and H are taken as stored (co-indexed, half a step apart): synthetic objectives (R19).
 # ----------------------------------------------------------------------------------------------------
 def loss_and_cotangent(w: Workload, mon: np.ndarray, extra: Optional[dict] = None):
     mon = np.asarray(mon, dtype=np.float64)
