@@ -217,6 +217,22 @@ bool in_grid(const fdtd_sim* s, const int lo[3], const int hi[3]) {
   return box_ok(lo, hi, ilo, s->n);
 }
 
+// x / d == __umulhi(x, mul) for all x <= xmax (checked here; d == 1 is handled in fast_div)
+FastDiv make_fastdiv(unsigned d, unsigned xmax) {
+  FastDiv f{0u, d};
+  if (d <= 1) { f.d = 1; return f; }
+  f.mul = (unsigned)((1ull << 32) / d) + 1u;
+  for (unsigned x = 0; x <= xmax; ++x)
+    if ((unsigned)(((unsigned long long)x * f.mul) >> 32) != x / d) { std::fprintf(stderr, "fdtd: fastdiv(%u) fails at %u\n", d, x); std::abort(); }
+  return f;
+}
+unsigned make_ginv(int G) {
+  const unsigned m = (65536u + (unsigned)G - 1u) / (unsigned)G;
+  for (unsigned lane = 0; lane < 32; ++lane)
+    if (((lane * m) >> 16) != lane / (unsigned)G) { std::fprintf(stderr, "fdtd: ginv(%d) fails\n", G); std::abort(); }
+  return m;
+}
+
 // Lean region [lo, hi) of split half-step `which` and the disjoint boxes covering the rest of the grid.
 void make_split(fdtd_sim* s, int which) {
   const int P = s->P, V = s->V, VG = s->VG;
@@ -236,27 +252,31 @@ void make_split(fdtd_sim* s, int which) {
   s->has_lean[which] = r.hi[0] > r.lo[0] && r.hi[1] > r.lo[1] && r.hi[2] > r.lo[2];
   BoxList& B = s->boxes[which];
   B = BoxList{};
-  auto add = [&](int x0, int x1, int y0, int y1, int z0, int z1) {
+  auto add = [&](int cls, int x0, int x1, int y0, int y1, int z0, int z1) {
     if (x1 <= x0 || y1 <= y0 || z1 <= z0) return;
     const int b = B.nb++;
     B.lo[b][0] = x0; B.hi[b][0] = x1; B.lo[b][1] = y0; B.hi[b][1] = y1; B.lo[b][2] = z0; B.hi[b][2] = z1;
+    B.cls[b] = cls;
     const int groups = (z1 - z0 + VG - 1) / VG;
-    int lzs = 0;
-    while ((1 << lzs) < groups && lzs < 5) ++lzs;
-    B.lzs[b] = lzs;
-    B.nbx[b] = (groups + (1 << lzs) - 1) >> lzs;
-    const int rows_per_block = TY << (5 - lzs);
-    B.nby[b] = (y1 - y0 + rows_per_block - 1) / rows_per_block;
+    const int G = std::min(groups, 32), RW = 32 / G;
+    B.G[b] = G; B.RW[b] = RW;
+    B.ginv[b] = make_ginv(G);
+    B.nbx[b] = (groups + G - 1) / G;
+    B.nby[b] = (y1 - y0 + TY * RW - 1) / (TY * RW);
+    B.dnbx[b] = make_fastdiv((unsigned)B.nbx[b], (unsigned)B.nbx[b] * B.nby[b] * (unsigned)(x1 - x0));
+    B.dnby[b] = make_fastdiv((unsigned)B.nby[b], (unsigned)B.nby[b] * (unsigned)(x1 - x0));
     B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b] * (x1 - x0);
   };
   const int nx = s->n[0], ny = s->n[1], nz = s->n[2];
-  if (!s->has_lean[which]) { add(0, nx, 0, ny, 0, nz); return; }
-  add(0, r.lo[0], 0, ny, 0, nz);
-  add(r.hi[0], nx, 0, ny, 0, nz);
-  add(r.lo[0], r.hi[0], 0, r.lo[1], 0, nz);
-  add(r.lo[0], r.hi[0], r.hi[1], ny, 0, nz);
-  add(r.lo[0], r.hi[0], r.lo[1], r.hi[1], 0, r.lo[2]);
-  add(r.lo[0], r.hi[0], r.lo[1], r.hi[1], r.hi[2], nz);
+  // classes: the x range of the lean region holds no x-slab cell, no wall plane and (adjoint) no cell whose x
+  // neighbour is a slab cell, so boxes confined to it need no x terms (CLS_Y); likewise y for CLS_Z
+  if (!s->has_lean[which]) { add(CLS_X, 0, nx, 0, ny, 0, nz); return; }
+  add(CLS_X, 0, r.lo[0], 0, ny, 0, nz);
+  add(CLS_X, r.hi[0], nx, 0, ny, 0, nz);
+  add(CLS_Y, r.lo[0], r.hi[0], 0, r.lo[1], 0, nz);
+  add(CLS_Y, r.lo[0], r.hi[0], r.hi[1], ny, 0, nz);
+  add(CLS_Z, r.lo[0], r.hi[0], r.lo[1], r.hi[1], 0, r.lo[2]);
+  add(CLS_Z, r.lo[0], r.hi[0], r.lo[1], r.hi[1], r.hi[2], nz);
 }
 dim3 grid_lean(const fdtd_sim* s, int which) {
   const Region& r = s->reg[which];
@@ -323,7 +343,14 @@ void launch_gen(fdtd_sim* s, int which, int pb) {
   const BoxList& B = s->boxes[which];
   const unsigned g = (unsigned)B.off[B.nb];
   if (g == 0) return;
-  if (s->VG == 2) {
+  if (s->VG == 4) {
+    switch (which) {
+      case 0: LAUNCH(s, k_gen_e<4>, g, b, s->d, B); break;
+      case 1: LAUNCH(s, k_gen_h<4>, g, b, s->d, B); break;
+      case 2: LAUNCH(s, k_gen_adj_h<4>, g, b, s->d, B, pb); break;
+      default: LAUNCH(s, k_gen_adj_e<4>, g, b, s->d, B, pb);
+    }
+  } else if (s->VG == 2) {
     switch (which) {
       case 0: LAUNCH(s, k_gen_e<2>, g, b, s->d, B); break;
       case 1: LAUNCH(s, k_gen_h<2>, g, b, s->d, B); break;
@@ -353,12 +380,27 @@ void launch_inv_h(fdtd_sim* s) {
   if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
   else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
 }
-void launch_grad_inv_e(fdtd_sim* s) {
+void launch_inv_e(fdtd_sim* s) {
   dim3 gi;
   if (!grid_inner(s, &gi)) return;
   const dim3 b(32, TY);
-  if (s->V == 4) LAUNCH(s, k_grad_inv_e<4>, gi, b, s->d);
-  else LAUNCH(s, k_grad_inv_e<1>, gi, b, s->d);
+  if (s->V == 4) LAUNCH(s, k_inv_e<4>, gi, b, s->d);
+  else LAUNCH(s, k_inv_e<1>, gi, b, s->d);
+}
+// design ∩ inner interior extents; false if empty
+bool grad_extents(const fdtd_sim* s, int ext[3]) {
+  if (!s->has_design) return false;
+  for (int a = 0; a < 3; ++a) {
+    ext[a] = std::min(s->dhi[a], s->n[a] - s->P - 1) - std::max(s->dlo[a], s->P + 1);
+    if (ext[a] <= 0) return false;
+  }
+  return true;
+}
+void launch_grad(fdtd_sim* s) {
+  int ext[3];
+  if (!grad_extents(s, ext)) return;
+  const long long cells = (long long)ext[0] * ext[1] * ext[2];
+  LAUNCH(s, k_grad, (unsigned)((cells + 255) / 256), 256, s->d);
 }
 void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
   if (s->nsrc == 0) return;
@@ -435,7 +477,7 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
   fork(s, 4);
   on(s, 0); launch_lean(s, 3);
   on(s, 1); launch_gen(s, 3, pb);
-  on(s, 2); launch_grad_inv_e(s);
+  on(s, 2); launch_inv_e(s); launch_grad(s);
   on(s, 3); launch_inject(s, m_base, step_dev, 0, interp);
   join(s, 4);
 }
@@ -657,7 +699,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   *out = nullptr;
   if (nx < 3 || ny < 3 || nz < 3 || pml_width < 0 || !eps_dev || !(dx > 0) || !(dt > 0)) return FDTD_ERR_INVALID_ARG;
   if (nx - 2 * pml_width < 2 || ny - 2 * pml_width < 2 || nz - 2 * pml_width < 2) return FDTD_ERR_INVALID_ARG;
-  if ((long long)nx * ny * nz > (1LL << 40)) return FDTD_ERR_INVALID_ARG;
+  if ((long long)nx * ny * nz >= (1LL << 32)) return FDTD_ERR_INVALID_ARG;   // 32-bit element offsets in the kernels
   const double S = kC0 * dt / dx;
   if (S > (1.0 / std::sqrt(3.0)) * (1.0 + 1e-9)) return FDTD_ERR_INVALID_ARG;   // PAPER.md:37-39 CFL limit
   fdtd_sim* s = new (std::nothrow) fdtd_sim();
@@ -729,7 +771,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   for (int a = 0; a < 3; ++a) d.n[a] = s->n[a];
   d.P = s->P;
   d.sy = s->n[2];
-  d.sx = (long long)s->n[1] * s->n[2];
+  d.sx = (idx_t)s->n[1] * (idx_t)s->n[2];
   d.N = (long long)s->n[0] * s->n[1] * s->n[2];
   d.S = (float)s->Sd;
   char* w = s->ws;
@@ -778,8 +820,8 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
   }
   s->V = (s->n[2] % 4 == 0 && s->P % 4 == 0) ? 4 : 1;
-  s->VG = s->V == 4 ? 2 : 1;
-  if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2) && s->V == 4) s->VG = v; }
+  s->VG = s->V == 4 ? 4 : 1;
+  if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2 || v == 4) && s->V == 4) s->VG = v; }
   for (int which = 0; which < 4; ++which) make_split(s, which);
   build_tables(s);
   CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
@@ -958,7 +1000,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 1: launch_fwd_h(s); break;
       case 2: launch_inv_h(s); break;
       case 3: launch_split(s, 2, 0); break;
-      case 4: launch_grad_inv_e(s); break;
+      case 4: launch_inv_e(s); launch_grad(s); break;
       case 5: launch_split(s, 3, 0); break;
       case 6: launch_record(s, s->nsteps, nullptr, 2); break;
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;

@@ -6,6 +6,9 @@
 
 namespace fdtd {
 
+// Element offsets are 32-bit: fdtd_create rejects grids of 2^32 cells or more.
+typedef unsigned idx_t;
+
 // Everything a kernel needs to find its data.  Passed by value (__grid_constant__).
 // Layout in HBM: six component-planar f32 arrays [nx][ny][nz], z fastest; ce = S/eps;
 // CPML psi arrays stored compactly (slab cells only): psi?[c][t] belongs to component c and derivative axis
@@ -13,7 +16,7 @@ namespace fdtd {
 struct Dev {
   int n[3];
   int P;
-  long long sx, sy;  // strides of i and j (k stride = 1)
+  idx_t sx, sy;      // strides of i and j (k stride = 1)
   long long N;
   float S;           // Courant number c*dt/dx (eq. 1)
   float* E[3];
@@ -33,23 +36,30 @@ struct Dev {
 };
 
 // A lean kernel's region (plain Yee cells) and the list of boxes that make up its complement (slab cells and the
-// layers that touch them), each with its own lane shape: LZ = 1 << lzs lanes along z, 32/LZ rows per warp.
+// layers that touch them).  Each box has a class that says which CPML axes can occur in it (so the others compile
+// out) and its own lane shape: G lanes along z (groups of V cells) x RW rows per warp, G*RW <= 32.
 struct Region { int lo[3], hi[3]; };
+struct FastDiv { unsigned mul, d; };   // x / d == __umulhi(x, mul) for the x range checked on the host (d == 1: x)
+enum { CLS_X = 0, CLS_Y = 1, CLS_Z = 2 };   // X: any axis; Y: no x terms; Z: z terms only
 struct BoxList {
   int nb;
   int lo[6][3], hi[6][3];
-  int lzs[6];
-  int nbx[6], nby[6];
+  int cls[6];
+  int G[6], RW[6];
+  unsigned ginv[6];        // (lane * ginv) >> 16 == lane / G for lane < 32
+  int nbx[6], nby[6];      // blocks along z and along y per x plane
+  FastDiv dnbx[6], dnby[6];
   int off[7];
 };
+__device__ __forceinline__ unsigned fast_div(unsigned x, const FastDiv f) { return f.d == 1u ? x : __umulhi(x, f.mul); }
 
 __device__ __forceinline__ bool in_slab(int i, int n, int P) { return i < P || i >= n - P; }
 __device__ __forceinline__ int slab_s(int i, int n, int P) { return i < P ? i : i - (n - 2 * P); }
-__device__ __forceinline__ long long psi_index(const Dev& d, int a, int i, int j, int k) {
+__device__ __forceinline__ idx_t psi_index(const Dev& d, int a, int i, int j, int k) {
   const int P2 = 2 * d.P;
-  if (a == 0) return ((long long)slab_s(i, d.n[0], d.P) * d.n[1] + j) * d.n[2] + k;
-  if (a == 1) return ((long long)i * P2 + slab_s(j, d.n[1], d.P)) * d.n[2] + k;
-  return ((long long)i * d.n[1] + j) * P2 + slab_s(k, d.n[2], d.P);
+  if (a == 0) return ((idx_t)slab_s(i, d.n[0], d.P) * d.n[1] + j) * d.n[2] + k;
+  if (a == 1) return ((idx_t)i * P2 + slab_s(j, d.n[1], d.P)) * d.n[2] + k;
+  return ((idx_t)i * d.n[1] + j) * P2 + slab_s(k, d.n[2], d.P);
 }
 
 // V consecutive z cells held by one thread (V = 4: one 16-byte access; V = 1: scalar path for odd shapes).

@@ -15,35 +15,44 @@ namespace fdtd {
 
 constexpr int TY = 8;
 
-// block / thread -> (i, j, first k) inside the box list of a GENERAL kernel
+// block / thread -> box b and (i, j, first k) inside the box list of a GENERAL kernel.  One x plane per block;
+// a warp covers G z-groups x RW rows of its box (thin z slabs pack several rows into one warp).
 template <int V>
-__device__ __forceinline__ bool box_decode(const BoxList& B, int& i, int& j, int& k0) {
-  const int blk = blockIdx.x;
-  int b = 0;
+__device__ __forceinline__ bool box_decode(const BoxList& B, int& b, int& i, int& j, int& k0) {
+  const unsigned blk = blockIdx.x;
+  b = 0;
 #pragma unroll
-  for (int g = 1; g < 6; ++g) b += (g < B.nb && blk >= B.off[g]);
-  const int local = blk - B.off[b];
-  const int bx = local % B.nbx[b];
-  const int t = local / B.nbx[b];
-  const int by = t % B.nby[b], bz = t / B.nby[b];
-  const int lzs = B.lzs[b];
-  const int zl = threadIdx.x & ((1 << lzs) - 1), yl = threadIdx.x >> lzs;
-  j = B.lo[b][1] + ((by * TY + threadIdx.y) << (5 - lzs)) + yl;
-  k0 = B.lo[b][2] + ((bx << lzs) + zl) * V;
-  i = B.lo[b][0] + bz;
-  return j < B.hi[b][1] && k0 < B.hi[b][2];
+  for (int g = 1; g < 6; ++g) b += (g < B.nb && blk >= (unsigned)B.off[g]);
+  const unsigned local = blk - B.off[b];
+  const unsigned t = fast_div(local, B.dnbx[b]);
+  const unsigned bx = local - t * B.nbx[b];
+  const unsigned bz = fast_div(t, B.dnby[b]);
+  const unsigned by = t - bz * B.nby[b];
+  const int G = B.G[b], RW = B.RW[b];
+  const int yl = (int)((threadIdx.x * B.ginv[b]) >> 16), zl = (int)threadIdx.x - yl * G;
+  j = B.lo[b][1] + ((int)by * TY + (int)threadIdx.y) * RW + yl;
+  k0 = B.lo[b][2] + ((int)bx * G + zl) * V;
+  i = B.lo[b][0] + (int)bz;
+  return yl < RW && j < B.hi[b][1] && k0 < B.hi[b][2];
 }
+
+// A general kernel body is instantiated per box class: HX / HY say whether CPML terms of the x / y axis (and, for
+// the adjoint, neighbour terms across that axis) can occur in the box; z terms are always compiled in.
+#define FDTD_CLASS_DISPATCH(BODY, ...)                                    \
+  switch (B.cls[b]) {                                                     \
+    case CLS_X: BODY<V, true, true>(__VA_ARGS__); break;                  \
+    case CLS_Y: BODY<V, false, true>(__VA_ARGS__); break;                 \
+    default: BODY<V, false, false>(__VA_ARGS__); break;                   \
+  }
 
 // ---------------------------------------------------------------------------------------------------------
 // Forward E half-step (SURVEY 8(a) rows A1 + A3):  E_c += ce * (d_a1^- H_b1 - d_a2^- H_b2) + CPML terms,
 // tangential E on the three low PEC walls held at zero.  DESIGN.md R1-R5.
 // ---------------------------------------------------------------------------------------------------------
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+template <int V, bool HX, bool HY>
+__device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int j, const int k0) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  int i, j, k0;
-  if (!box_decode<V>(B, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
+  const idx_t sx = d.sx, sy = d.sy;
 
   bool zs[V];
   float bz[V], cz[V], kz[V];
@@ -55,11 +64,11 @@ __global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d
     cz[v] = zs[v] ? __ldg(d.tab[2][1] + k) : 0.0f;
     kz[v] = zs[v] ? __ldg(d.tab[2][2] + k) : 0.0f;
   }
-  const bool ys = P > 0 && in_slab(j, ny, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P);
   const float by = ys ? __ldg(d.tab[1][0] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][1] + j) : 0.0f,
               ky = ys ? __ldg(d.tab[1][2] + j) : 0.0f;
 
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   VF<V> pHy = zerov<V>(), pHz = zerov<V>();
   if (i > 0) {
     pHy = ldv<V>(d.H[1] + q - sx);
@@ -80,13 +89,13 @@ __global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d
     VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
     const VF<V> ce = ldv<V>(d.ce + q);
 
-    const bool xs = P > 0 && in_slab(i, nx, P);
+    const bool xs = HX && P > 0 && in_slab(i, nx, P);
     const float bx = xs ? __ldg(d.tab[0][0] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][1] + i) : 0.0f,
                 kx = xs ? __ldg(d.tab[0][2] + i) : 0.0f;
     // psi_E[c][t]: (0,0)=Ex/y (0,1)=Ex/z (1,0)=Ey/z (1,1)=Ey/x (2,0)=Ez/x (2,1)=Ez/y
     VF<V> p_ey_x = zerov<V>(), p_ez_x = zerov<V>(), p_ex_y = zerov<V>(), p_ez_y = zerov<V>(),
           p_ex_z = zerov<V>(), p_ey_z = zerov<V>();
-    long long qx = 0, qy = 0, qz = 0;
+    idx_t qx = 0, qy = 0, qz = 0;
     if (xs) {
       qx = psi_index(d, 0, i, j, k0);
       p_ey_x = ldv<V>(d.psiE[1][1] + qx);
@@ -141,12 +150,10 @@ __global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d
 // ---------------------------------------------------------------------------------------------------------
 // Forward H half-step (rows A2 + A4):  H_c -= S * (d_a1^+ E_b1 - d_a2^+ E_b2) + CPML terms; ghost E[n] = 0.
 // ---------------------------------------------------------------------------------------------------------
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+template <int V, bool HX, bool HY>
+__device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int j, const int k0) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  int i, j, k0;
-  if (!box_decode<V>(B, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
+  const idx_t sx = d.sx, sy = d.sy;
   const float mS = -d.S;
 
   bool zs[V];
@@ -159,11 +166,11 @@ __global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d
     cz[v] = zs[v] ? __ldg(d.tab[2][4] + k) : 0.0f;
     kz[v] = zs[v] ? __ldg(d.tab[2][5] + k) : 0.0f;
   }
-  const bool ys = P > 0 && in_slab(j, ny, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P);
   const float by = ys ? __ldg(d.tab[1][3] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][4] + j) : 0.0f,
               ky = ys ? __ldg(d.tab[1][5] + j) : 0.0f;
 
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const VF<V> ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   {
     const VF<V> ex = ldv<V>(d.E[0] + q);
@@ -184,13 +191,13 @@ __global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d
     }
     VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
 
-    const bool xs = P > 0 && in_slab(i, nx, P);
+    const bool xs = HX && P > 0 && in_slab(i, nx, P);
     const float bx = xs ? __ldg(d.tab[0][3] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][4] + i) : 0.0f,
                 kx = xs ? __ldg(d.tab[0][5] + i) : 0.0f;
     // psi_H[c][t]: (0,0)=Hx/y (0,1)=Hx/z (1,0)=Hy/z (1,1)=Hy/x (2,0)=Hz/x (2,1)=Hz/y
     VF<V> p_hy_x = zerov<V>(), p_hz_x = zerov<V>(), p_hx_y = zerov<V>(), p_hz_y = zerov<V>(),
           p_hx_z = zerov<V>(), p_hy_z = zerov<V>();
-    long long qx = 0, qy = 0, qz = 0;
+    idx_t qx = 0, qy = 0, qz = 0;
     if (xs) {
       qx = psi_index(d, 0, i, j, k0);
       p_hy_x = ldv<V>(d.psiH[1][1] + qx);
@@ -252,8 +259,8 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
   const int j = P + 1 + blockIdx.y * TY + threadIdx.y;
   const int i = P + 1 + blockIdx.z;
   if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const float S = d.S;
   const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   const VF<V> ey_xp = ldv<V>(d.E[1] + q + sx), ez_xp = ldv<V>(d.E[2] + q + sx);
@@ -290,54 +297,30 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
   }
 }
 
-// gradient term (row R3) + inverse of the E half-step (row R2), fused since both need curl^-(H^{m-1/2}):
-//   acc += sum_c lE_c * curl_c  on design ∩ inner interior;   E^{m-1} = E^m - ce * curl
+// inverse of the E half-step (row R2):  E^{m-1} = E^m - ce * curl^-(H^{m-1/2})   on the inner interior
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_grad_inv_e(const __grid_constant__ Dev d) {
+__global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const int klo = P + 1, khi = nz - P - 1;
   const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
   const int j = P + 1 + blockIdx.y * TY + threadIdx.y;
   const int i = P + 1 + blockIdx.z;
   if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
   const VF<V> hy_xm = ldv<V>(d.H[1] + q - sx), hz_xm = ldv<V>(d.H[2] + q - sx);
   const VF<V> hx_ym = ldv<V>(d.H[0] + q - sy), hz_ym = ldv<V>(d.H[2] + q - sy);
-  float hx_z0 = 0.0f, hy_z0 = 0.0f;
-  if (k0 > 0) {
-    hx_z0 = d.H[0][q - 1];
-    hy_z0 = d.H[1][q - 1];
-  }
+  const float hx_z0 = d.H[0][q - 1], hy_z0 = d.H[1][q - 1];   // k0 >= 1: the inner interior starts at P + 1
   VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   const VF<V> ce = ldv<V>(d.ce + q);
-  const bool des_ij = d.has_design && i >= d.dlo[0] && i < d.dhi[0] && j >= d.dlo[1] && j < d.dhi[1] &&
-                      k0 + V > d.dlo[2] && k0 < d.dhi[2];
-  VF<V> lx = zerov<V>(), ly = zerov<V>(), lz = zerov<V>();
-  if (des_ij) {
-    lx = ldv<V>(d.lE[0] + q);
-    ly = ldv<V>(d.lE[1] + q);
-    lz = ldv<V>(d.lE[2] + q);
-  }
 #pragma unroll
   for (int v = 0; v < V; ++v) {
-    const int k = k0 + v;
-    if (k < klo || k >= khi) continue;
     const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
     const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
     const float cx = (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm);
     const float cy = (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]);
     const float cz = (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]);
-    if (des_ij && k >= d.dlo[2] && k < d.dhi[2]) {
-      double s = 0.0;
-      s += (double)lx.v[v] * (double)cx;
-      s += (double)ly.v[v] * (double)cy;
-      s += (double)lz.v[v] * (double)cz;
-      const long long e = ((long long)(i - d.dlo[0]) * (d.dhi[1] - d.dlo[1]) + (j - d.dlo[1])) * (d.dhi[2] - d.dlo[2]) +
-                          (k - d.dlo[2]);
-      d.acc[e] += s;
-    }
     ex.v[v] = fmaf(-ce.v[v], cx, ex.v[v]);
     ey.v[v] = fmaf(-ce.v[v], cy, ey.v[v]);
     ez.v[v] = fmaf(-ce.v[v], cz, ez.v[v]);
@@ -357,24 +340,54 @@ __global__ void __launch_bounds__(32 * TY) k_grad_inv_e(const __grid_constant__ 
   }
 }
 
+// gradient term (row R3) on design ∩ inner interior:  acc += sum_c lE_c * curl^-(H^{m-1/2})_c  (f64 accumulator).
+// Its own kernel so that the inverse-E sweep above stays a lean f32 kernel; it reads H^{m-1/2} and lE, both
+// read-only in this phase (it runs beside k_inv_e and the adjoint-E kernels).  One thread per design cell.
+__global__ void __launch_bounds__(256) k_grad(const __grid_constant__ Dev d) {
+  const int P = d.P;
+  int lo[3], ext[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    lo[a] = max(d.dlo[a], P + 1);
+    ext[a] = min(d.dhi[a], d.n[a] - P - 1) - lo[a];
+  }
+  const idx_t t = blockIdx.x * 256u + threadIdx.x;   // flat index over the clipped design box, z fastest
+  if (t >= (idx_t)ext[0] * ext[1] * ext[2]) return;
+  const idx_t row = t / (idx_t)ext[2];
+  const int k = lo[2] + (int)(t - row * ext[2]);
+  const int i = lo[0] + (int)(row / (idx_t)ext[1]), j = lo[1] + (int)(row % (idx_t)ext[1]);
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k;
+  const float hx = d.H[0][q], hy = d.H[1][q], hz = d.H[2][q];
+  const float cx = (hz - d.H[2][q - sy]) - (hy - d.H[1][q - 1]);
+  const float cy = (hx - d.H[0][q - 1]) - (hz - d.H[2][q - sx]);
+  const float cz = (hy - d.H[1][q - sx]) - (hx - d.H[0][q - sy]);
+  double s = 0.0;
+  s += (double)d.lE[0][q] * (double)cx;
+  s += (double)d.lE[1][q] * (double)cy;
+  s += (double)d.lE[2][q] * (double)cz;
+  const idx_t e = ((idx_t)(i - d.dlo[0]) * (d.dhi[1] - d.dlo[1]) + (j - d.dlo[1])) * (d.dhi[2] - d.dlo[2]) + (k - d.dlo[2]);
+  d.acc[e] += s;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Adjoint of the H half-step (row R4): lE_e += -S * curl^-(lH)_e on all cells (PEC-masked nodes -> 0), plus the
 // transposed CPML: for the H term (c,t) with axis a and field b:  g = -S*s*lH_c, W = cH*(lpsiH + g) + kH*g,
 // lpsiH <- bH*(lpsiH + g), lE_b -= d_a^-(W).   lpsiH is ping-ponged (pb = buffer read, pb^1 = written), because
 // W at the low-side neighbour needs that neighbour's OLD lpsiH.
+// Layout of the body: plain update of the three components, then one correction block per CPML axis in the
+// order z, y, x — the canonical subtraction order of every component (lE_x: z,y; lE_y: z,x; lE_z: y,x).  A block is
+// entered when this cell or its low-side neighbour along that axis is a slab cell (x, y: uniform over the warp's
+// row).  Inside a block the arithmetic is unconditional: the coefficient tables are zero outside the slabs and a
+// missing lpsi reads as zero, so absent terms evaluate to W = 0 exactly.
 // ---------------------------------------------------------------------------------------------------------
-struct WTerm {  // W(q) - W(q - stride_a) of one transposed H term, evaluated by the thread that owns q
-  float wq, wm;
-};
-
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+template <int V, bool HX, bool HY>
+__device__ __forceinline__ void gen_adj_h_body(const Dev& d, const int i, const int j, const int k0, int pb) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  int i, j, k0;
-  if (!box_decode<V>(B, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const float S = d.S;
+  const int nb = pb ^ 1;
   const VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
   VF<V> lhy_xm = zerov<V>(), lhz_xm = zerov<V>(), lhx_ym = zerov<V>(), lhz_ym = zerov<V>();
   if (i > 0) {
@@ -392,28 +405,25 @@ __global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ D
   }
   VF<V> lex = ldv<V>(d.lE[0] + q), ley = ldv<V>(d.lE[1] + q), lez = ldv<V>(d.lE[2] + q);
 
-  // --- slab state at this cell and at its low-side neighbours ---
-  const bool xs = P > 0 && in_slab(i, nx, P), xsm = P > 0 && i > 0 && in_slab(i - 1, nx, P);
-  const bool ys = P > 0 && in_slab(j, ny, P), ysm = P > 0 && j > 0 && in_slab(j - 1, ny, P);
-  float bx = 0, cx = 0, kx = 0, cxm = 0, kxm = 0, by = 0, cy = 0, ky = 0, cym = 0, kym = 0;
-  if (xs) { bx = __ldg(d.tab[0][3] + i); cx = __ldg(d.tab[0][4] + i); kx = __ldg(d.tab[0][5] + i); }
-  if (xsm) { cxm = __ldg(d.tab[0][4] + i - 1); kxm = __ldg(d.tab[0][5] + i - 1); }
-  if (ys) { by = __ldg(d.tab[1][3] + j); cy = __ldg(d.tab[1][4] + j); ky = __ldg(d.tab[1][5] + j); }
-  if (ysm) { cym = __ldg(d.tab[1][4] + j - 1); kym = __ldg(d.tab[1][5] + j - 1); }
-  // old lambda_psi_H at q and at the neighbour, per term
-  VF<V> o11 = zerov<V>(), o20 = zerov<V>(), o11m = zerov<V>(), o20m = zerov<V>();   // axis x: (c=1,t=1), (c=2,t=0)
-  VF<V> o00 = zerov<V>(), o21 = zerov<V>(), o00m = zerov<V>(), o21m = zerov<V>();   // axis y: (c=0,t=0), (c=2,t=1)
-  VF<V> o01 = zerov<V>(), o10 = zerov<V>();                                         // axis z: (c=0,t=1), (c=1,t=0)
-  long long qx = 0, qy = 0, qz = 0;
-  if (xs) {
-    qx = psi_index(d, 0, i, j, k0);
-    o11 = ldv<V>(d.lpsiH[pb][1][1] + qx);
-    o20 = ldv<V>(d.lpsiH[pb][2][0] + qx);
+  const bool xs = HX && P > 0 && in_slab(i, nx, P), xsm = HX && P > 0 && i > 0 && in_slab(i - 1, nx, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P), ysm = HY && P > 0 && j > 0 && in_slab(j - 1, ny, P);
+  const bool zs0 = P > 0 && in_slab(k0, nz, P);                 // V = 4: a group never straddles a slab edge
+  const bool zsm0 = P > 0 && k0 > 0 && in_slab(k0 - 1, nz, P);
+  const bool zany = zs0 || zsm0;                                // (P % V == 0, so only element 0 can have a slab neighbour alone)
+  // issue the lpsi loads of every active block before any arithmetic
+  VF<V> o01 = zerov<V>(), o10 = zerov<V>(), o00 = zerov<V>(), o21 = zerov<V>(), o11 = zerov<V>(), o20 = zerov<V>();
+  VF<V> o00m = zerov<V>(), o21m = zerov<V>(), o11m = zerov<V>(), o20m = zerov<V>();
+  float o01_z0 = 0.0f, o10_z0 = 0.0f;
+  idx_t qx = 0, qy = 0, qz = 0;
+  if (zs0) {
+    qz = psi_index(d, 2, i, j, k0);
+    o01 = ldv<V>(d.lpsiH[pb][0][1] + qz);
+    o10 = ldv<V>(d.lpsiH[pb][1][0] + qz);
   }
-  if (xsm) {
-    const long long qm = psi_index(d, 0, i - 1, j, k0);
-    o11m = ldv<V>(d.lpsiH[pb][1][1] + qm);
-    o20m = ldv<V>(d.lpsiH[pb][2][0] + qm);
+  if (zsm0) {
+    const idx_t qm = psi_index(d, 2, i, j, k0 - 1);
+    o01_z0 = d.lpsiH[pb][0][1][qm];
+    o10_z0 = d.lpsiH[pb][1][0][qm];
   }
   if (ys) {
     qy = psi_index(d, 1, i, j, k0);
@@ -421,168 +431,161 @@ __global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ D
     o21 = ldv<V>(d.lpsiH[pb][2][1] + qy);
   }
   if (ysm) {
-    const long long qm = psi_index(d, 1, i, j - 1, k0);
+    const idx_t qm = psi_index(d, 1, i, j - 1, k0);
     o00m = ldv<V>(d.lpsiH[pb][0][0] + qm);
     o21m = ldv<V>(d.lpsiH[pb][2][1] + qm);
   }
-  const bool zs0 = P > 0 && in_slab(k0, nz, P);           // V = 4: groups never straddle a slab edge (P % 4 == 0)
-  const bool zsm0 = P > 0 && k0 > 0 && in_slab(k0 - 1, nz, P);
-  float o01_z0 = 0.0f, o10_z0 = 0.0f;
-  if (zs0) {
-    qz = psi_index(d, 2, i, j, k0);
-    o01 = ldv<V>(d.lpsiH[pb][0][1] + qz);
-    o10 = ldv<V>(d.lpsiH[pb][1][0] + qz);
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    o11 = ldv<V>(d.lpsiH[pb][1][1] + qx);
+    o20 = ldv<V>(d.lpsiH[pb][2][0] + qx);
   }
-  if (zsm0) {
-    const long long qm = psi_index(d, 2, i, j, k0 - 1);
-    o01_z0 = d.lpsiH[pb][0][1][qm];
-    o10_z0 = d.lpsiH[pb][1][0][qm];
+  if (xsm) {
+    const idx_t qm = psi_index(d, 0, i - 1, j, k0);
+    o11m = ldv<V>(d.lpsiH[pb][1][1] + qm);
+    o20m = ldv<V>(d.lpsiH[pb][2][0] + qm);
   }
-  VF<V> n11 = o11, n20 = o20, n00 = o00, n21 = o21, n01 = o01, n10 = o10;
-  float dummy;
+
+  // --- plain part ---
 #pragma unroll
   for (int v = 0; v < V; ++v) {
-    const int k = k0 + v;
     const float lhy_zm = v == 0 ? lhy_z0 : lhy.v[v > 0 ? v - 1 : 0];
     const float lhx_zm = v == 0 ? lhx_z0 : lhx.v[v > 0 ? v - 1 : 0];
-    // --- W terms (coef: t = 0 -> -S, t = 1 -> +S) ---
-    float w11 = 0, w11m = 0, w20 = 0, w20m = 0, w00 = 0, w00m = 0, w21 = 0, w21m = 0, w01 = 0, w01m = 0, w10 = 0, w10m = 0;
-    if (xs) {
-      w11 = cpml_adjoint_term(S * lhy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);
-      w20 = cpml_adjoint_term(-S * lhz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);
-    }
-    if (xsm) {
-      w11m = cpml_adjoint_term(S * lhy_xm.v[v], o11m.v[v], 0.0f, cxm, kxm, dummy);
-      w20m = cpml_adjoint_term(-S * lhz_xm.v[v], o20m.v[v], 0.0f, cxm, kxm, dummy);
-    }
-    if (ys) {
-      w00 = cpml_adjoint_term(-S * lhx.v[v], o00.v[v], by, cy, ky, n00.v[v]);
-      w21 = cpml_adjoint_term(S * lhz.v[v], o21.v[v], by, cy, ky, n21.v[v]);
-    }
-    if (ysm) {
-      w00m = cpml_adjoint_term(-S * lhx_ym.v[v], o00m.v[v], 0.0f, cym, kym, dummy);
-      w21m = cpml_adjoint_term(S * lhz_ym.v[v], o21m.v[v], 0.0f, cym, kym, dummy);
-    }
-    const bool zs = P > 0 && in_slab(k, nz, P);
-    if (zs) {
+    lex.v[v] = fmaf(-S, (lhz.v[v] - lhz_ym.v[v]) - (lhy.v[v] - lhy_zm), lex.v[v]);
+    ley.v[v] = fmaf(-S, (lhx.v[v] - lhx_zm) - (lhz.v[v] - lhz_xm.v[v]), ley.v[v]);
+    lez.v[v] = fmaf(-S, (lhy.v[v] - lhy_xm.v[v]) - (lhx.v[v] - lhx_ym.v[v]), lez.v[v]);
+  }
+  float dummy;
+  // --- z block: terms (c=0,t=1: g = +S*lH_x -> lE_y) and (c=1,t=0: g = -S*lH_y -> lE_x) ---
+  if (zany) {
+    VF<V> n01, n10;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
       const float bz = __ldg(d.tab[2][3] + k), cz = __ldg(d.tab[2][4] + k), kz = __ldg(d.tab[2][5] + k);
-      w01 = cpml_adjoint_term(S * lhx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);
-      w10 = cpml_adjoint_term(-S * lhy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);
-    }
-    if (P > 0 && k > 0 && in_slab(k - 1, nz, P)) {
-      const float czm = __ldg(d.tab[2][4] + k - 1), kzm = __ldg(d.tab[2][5] + k - 1);
+      const float czm = k > 0 ? __ldg(d.tab[2][4] + k - 1) : 0.0f, kzm = k > 0 ? __ldg(d.tab[2][5] + k - 1) : 0.0f;
+      const float lhy_zm = v == 0 ? lhy_z0 : lhy.v[v > 0 ? v - 1 : 0];
+      const float lhx_zm = v == 0 ? lhx_z0 : lhx.v[v > 0 ? v - 1 : 0];
       const float p01 = v == 0 ? o01_z0 : o01.v[v > 0 ? v - 1 : 0];
       const float p10 = v == 0 ? o10_z0 : o10.v[v > 0 ? v - 1 : 0];
-      w01m = cpml_adjoint_term(S * lhx_zm, p01, 0.0f, czm, kzm, dummy);
-      w10m = cpml_adjoint_term(-S * lhy_zm, p10, 0.0f, czm, kzm, dummy);
+      const float w01 = cpml_adjoint_term(S * lhx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);
+      const float w10 = cpml_adjoint_term(-S * lhy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);
+      const float w01m = cpml_adjoint_term(S * lhx_zm, p01, 0.0f, czm, kzm, dummy);
+      const float w10m = cpml_adjoint_term(-S * lhy_zm, p10, 0.0f, czm, kzm, dummy);
+      lex.v[v] -= (w10 - w10m);
+      ley.v[v] -= (w01 - w01m);
     }
-    // --- lE_x: plain, then (c=1,t=0,a=z), then (c=2,t=1,a=y) ---
-    if (j == 0 || k == 0) lex.v[v] = 0.0f;
-    else {
-      float x = fmaf(-S, (lhz.v[v] - lhz_ym.v[v]) - (lhy.v[v] - lhy_zm), lex.v[v]);
-      x -= (w10 - w10m);
-      x -= (w21 - w21m);
-      lex.v[v] = x;
+    if (zs0) {
+      stv<V>(d.lpsiH[nb][0][1] + qz, n01);
+      stv<V>(d.lpsiH[nb][1][0] + qz, n10);
     }
-    // --- lE_y: plain, then (c=0,t=1,a=z), then (c=2,t=0,a=x) ---
-    if (k == 0 || i == 0) ley.v[v] = 0.0f;
-    else {
-      float x = fmaf(-S, (lhx.v[v] - lhx_zm) - (lhz.v[v] - lhz_xm.v[v]), ley.v[v]);
-      x -= (w01 - w01m);
-      x -= (w20 - w20m);
-      ley.v[v] = x;
+  }
+  // --- y block: terms (c=0,t=0: g = -S*lH_x -> lE_z) and (c=2,t=1: g = +S*lH_z -> lE_x) ---
+  if (HY && (ys || ysm)) {
+    const float by = __ldg(d.tab[1][3] + j), cy = __ldg(d.tab[1][4] + j), ky = __ldg(d.tab[1][5] + j);
+    const float cym = j > 0 ? __ldg(d.tab[1][4] + j - 1) : 0.0f, kym = j > 0 ? __ldg(d.tab[1][5] + j - 1) : 0.0f;
+    VF<V> n00, n21;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const float w00 = cpml_adjoint_term(-S * lhx.v[v], o00.v[v], by, cy, ky, n00.v[v]);
+      const float w21 = cpml_adjoint_term(S * lhz.v[v], o21.v[v], by, cy, ky, n21.v[v]);
+      const float w00m = cpml_adjoint_term(-S * lhx_ym.v[v], o00m.v[v], 0.0f, cym, kym, dummy);
+      const float w21m = cpml_adjoint_term(S * lhz_ym.v[v], o21m.v[v], 0.0f, cym, kym, dummy);
+      lex.v[v] -= (w21 - w21m);
+      lez.v[v] -= (w00 - w00m);
     }
-    // --- lE_z: plain, then (c=0,t=0,a=y), then (c=1,t=1,a=x) ---
-    if (i == 0 || j == 0) lez.v[v] = 0.0f;
-    else {
-      float x = fmaf(-S, (lhy.v[v] - lhy_xm.v[v]) - (lhx.v[v] - lhx_ym.v[v]), lez.v[v]);
-      x -= (w00 - w00m);
-      x -= (w11 - w11m);
-      lez.v[v] = x;
+    if (ys) {
+      stv<V>(d.lpsiH[nb][0][0] + qy, n00);
+      stv<V>(d.lpsiH[nb][2][1] + qy, n21);
+    }
+  }
+  // --- x block: terms (c=1,t=1: g = +S*lH_y -> lE_z) and (c=2,t=0: g = -S*lH_z -> lE_y) ---
+  if (HX && (xs || xsm)) {
+    const float bx = __ldg(d.tab[0][3] + i), cx = __ldg(d.tab[0][4] + i), kx = __ldg(d.tab[0][5] + i);
+    const float cxm = i > 0 ? __ldg(d.tab[0][4] + i - 1) : 0.0f, kxm = i > 0 ? __ldg(d.tab[0][5] + i - 1) : 0.0f;
+    VF<V> n11, n20;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const float w11 = cpml_adjoint_term(S * lhy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);
+      const float w20 = cpml_adjoint_term(-S * lhz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);
+      const float w11m = cpml_adjoint_term(S * lhy_xm.v[v], o11m.v[v], 0.0f, cxm, kxm, dummy);
+      const float w20m = cpml_adjoint_term(-S * lhz_xm.v[v], o20m.v[v], 0.0f, cxm, kxm, dummy);
+      ley.v[v] -= (w20 - w20m);
+      lez.v[v] -= (w11 - w11m);
+    }
+    if (xs) {
+      stv<V>(d.lpsiH[nb][1][1] + qx, n11);
+      stv<V>(d.lpsiH[nb][2][0] + qx, n20);
+    }
+  }
+  // --- PEC-masked nodes (low walls) ---
+  if (i == 0 || j == 0 || k0 == 0) {
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
+      if (j == 0 || k == 0) lex.v[v] = 0.0f;
+      if (k == 0 || i == 0) ley.v[v] = 0.0f;
+      if (i == 0 || j == 0) lez.v[v] = 0.0f;
     }
   }
   stv<V>(d.lE[0] + q, lex);
   stv<V>(d.lE[1] + q, ley);
   stv<V>(d.lE[2] + q, lez);
-  const int nb = pb ^ 1;
-  if (xs) {
-    stv<V>(d.lpsiH[nb][1][1] + qx, n11);
-    stv<V>(d.lpsiH[nb][2][0] + qx, n20);
-  }
-  if (ys) {
-    stv<V>(d.lpsiH[nb][0][0] + qy, n00);
-    stv<V>(d.lpsiH[nb][2][1] + qy, n21);
-  }
-  if (zs0) {
-    stv<V>(d.lpsiH[nb][0][1] + qz, n01);
-    stv<V>(d.lpsiH[nb][1][0] + qz, n10);
-  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // Adjoint of the E half-step (row R4): with G_c = ce*lE_c,  lH_h += curl^+(G)_h on all cells, plus the transposed
 // CPML: for the E term (c,t) with axis a and field b: g = s*G_c, W = cE*(lpsiE + g) + kE*g, lpsiE <- bE*(lpsiE+g)
-// (skipped on PEC-masked E_c nodes), lH_b -= d_a^+(W).
+// (skipped on PEC-masked E_c nodes: W = 0, lpsiE kept), lH_b -= d_a^+(W).
+// Same layout as gen_adj_h_body: plain part, then the z, y, x correction blocks (lH_x: z,y; lH_y: z,x; lH_z: y,x).
 // ---------------------------------------------------------------------------------------------------------
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+template <int V, bool HX, bool HY>
+__device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const int j, const int k0, int pb) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
-  int i, j, k0;
-  if (!box_decode<V>(B, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * ny + j) * nz + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
+  const int nb = pb ^ 1;
   const VF<V> ce = ldv<V>(d.ce + q);
   VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
   VF<V> gy_xp = zerov<V>(), gz_xp = zerov<V>(), gx_yp = zerov<V>(), gz_yp = zerov<V>();
-  float gx_zp = 0.0f, gy_zp = 0.0f;
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    gx.v[v] = ce.v[v] * gx.v[v];
-    gy.v[v] = ce.v[v] * gy.v[v];
-    gz.v[v] = ce.v[v] * gz.v[v];
-  }
+  VF<V> ce_xp = zerov<V>(), ce_yp = zerov<V>();
+  float gx_zp = 0.0f, gy_zp = 0.0f, ce_zp = 0.0f;
   if (i + 1 < nx) {
-    const VF<V> c2 = ldv<V>(d.ce + q + sx);
+    ce_xp = ldv<V>(d.ce + q + sx);
     gy_xp = ldv<V>(d.lE[1] + q + sx);
     gz_xp = ldv<V>(d.lE[2] + q + sx);
-#pragma unroll
-    for (int v = 0; v < V; ++v) { gy_xp.v[v] = c2.v[v] * gy_xp.v[v]; gz_xp.v[v] = c2.v[v] * gz_xp.v[v]; }
   }
   if (j + 1 < ny) {
-    const VF<V> c2 = ldv<V>(d.ce + q + sy);
+    ce_yp = ldv<V>(d.ce + q + sy);
     gx_yp = ldv<V>(d.lE[0] + q + sy);
     gz_yp = ldv<V>(d.lE[2] + q + sy);
-#pragma unroll
-    for (int v = 0; v < V; ++v) { gx_yp.v[v] = c2.v[v] * gx_yp.v[v]; gz_yp.v[v] = c2.v[v] * gz_yp.v[v]; }
   }
   if (k0 + V < nz) {
-    const float c2 = d.ce[q + V];
-    gx_zp = c2 * d.lE[0][q + V];
-    gy_zp = c2 * d.lE[1][q + V];
+    ce_zp = d.ce[q + V];
+    gx_zp = d.lE[0][q + V];
+    gy_zp = d.lE[1][q + V];
   }
   VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
 
-  const bool xs = P > 0 && in_slab(i, nx, P), xsp = P > 0 && i + 1 < nx && in_slab(i + 1, nx, P);
-  const bool ys = P > 0 && in_slab(j, ny, P), ysp = P > 0 && j + 1 < ny && in_slab(j + 1, ny, P);
-  float bx = 0, cx = 0, kx = 0, cxp = 0, kxp = 0, by = 0, cy = 0, ky = 0, cyp = 0, kyp = 0;
-  if (xs) { bx = __ldg(d.tab[0][0] + i); cx = __ldg(d.tab[0][1] + i); kx = __ldg(d.tab[0][2] + i); }
-  if (xsp) { cxp = __ldg(d.tab[0][1] + i + 1); kxp = __ldg(d.tab[0][2] + i + 1); }
-  if (ys) { by = __ldg(d.tab[1][0] + j); cy = __ldg(d.tab[1][1] + j); ky = __ldg(d.tab[1][2] + j); }
-  if (ysp) { cyp = __ldg(d.tab[1][1] + j + 1); kyp = __ldg(d.tab[1][2] + j + 1); }
+  const bool xs = HX && P > 0 && in_slab(i, nx, P), xsp = HX && P > 0 && i + 1 < nx && in_slab(i + 1, nx, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P), ysp = HY && P > 0 && j + 1 < ny && in_slab(j + 1, ny, P);
+  const bool zs0 = P > 0 && in_slab(k0, nz, P);
+  const bool zsp0 = P > 0 && k0 + V < nz && in_slab(k0 + V, nz, P);
+  const bool zany = zs0 || zsp0;
   // old lambda_psi_E: axis x terms (c=1,t=1: Ey) (c=2,t=0: Ez); axis y (c=0,t=0: Ex) (c=2,t=1: Ez); axis z (c=0,t=1: Ex) (c=1,t=0: Ey)
-  VF<V> o11 = zerov<V>(), o20 = zerov<V>(), o11p = zerov<V>(), o20p = zerov<V>();
-  VF<V> o00 = zerov<V>(), o21 = zerov<V>(), o00p = zerov<V>(), o21p = zerov<V>();
-  VF<V> o01 = zerov<V>(), o10 = zerov<V>();
-  long long qx = 0, qy = 0, qz = 0;
-  if (xs) {
-    qx = psi_index(d, 0, i, j, k0);
-    o11 = ldv<V>(d.lpsiE[pb][1][1] + qx);
-    o20 = ldv<V>(d.lpsiE[pb][2][0] + qx);
+  VF<V> o01 = zerov<V>(), o10 = zerov<V>(), o00 = zerov<V>(), o21 = zerov<V>(), o11 = zerov<V>(), o20 = zerov<V>();
+  VF<V> o00p = zerov<V>(), o21p = zerov<V>(), o11p = zerov<V>(), o20p = zerov<V>();
+  float o01_zp = 0.0f, o10_zp = 0.0f;
+  idx_t qx = 0, qy = 0, qz = 0;
+  if (zs0) {
+    qz = psi_index(d, 2, i, j, k0);
+    o01 = ldv<V>(d.lpsiE[pb][0][1] + qz);
+    o10 = ldv<V>(d.lpsiE[pb][1][0] + qz);
   }
-  if (xsp) {
-    const long long qp = psi_index(d, 0, i + 1, j, k0);
-    o11p = ldv<V>(d.lpsiE[pb][1][1] + qp);
-    o20p = ldv<V>(d.lpsiE[pb][2][0] + qp);
+  if (zsp0) {
+    const idx_t qp = psi_index(d, 2, i, j, k0 + V);
+    o01_zp = d.lpsiE[pb][0][1][qp];
+    o10_zp = d.lpsiE[pb][1][0][qp];
   }
   if (ys) {
     qy = psi_index(d, 1, i, j, k0);
@@ -590,98 +593,142 @@ __global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ D
     o21 = ldv<V>(d.lpsiE[pb][2][1] + qy);
   }
   if (ysp) {
-    const long long qp = psi_index(d, 1, i, j + 1, k0);
+    const idx_t qp = psi_index(d, 1, i, j + 1, k0);
     o00p = ldv<V>(d.lpsiE[pb][0][0] + qp);
     o21p = ldv<V>(d.lpsiE[pb][2][1] + qp);
   }
-  const bool zs0 = P > 0 && in_slab(k0, nz, P);
-  const bool zsp0 = P > 0 && k0 + V < nz && in_slab(k0 + V, nz, P);
-  float o01_zp = 0.0f, o10_zp = 0.0f;
-  if (zs0) {
-    qz = psi_index(d, 2, i, j, k0);
-    o01 = ldv<V>(d.lpsiE[pb][0][1] + qz);
-    o10 = ldv<V>(d.lpsiE[pb][1][0] + qz);
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    o11 = ldv<V>(d.lpsiE[pb][1][1] + qx);
+    o20 = ldv<V>(d.lpsiE[pb][2][0] + qx);
   }
-  if (zsp0) {
-    const long long qp = psi_index(d, 2, i, j, k0 + V);
-    o01_zp = d.lpsiE[pb][0][1][qp];
-    o10_zp = d.lpsiE[pb][1][0][qp];
+  if (xsp) {
+    const idx_t qp = psi_index(d, 0, i + 1, j, k0);
+    o11p = ldv<V>(d.lpsiE[pb][1][1] + qp);
+    o20p = ldv<V>(d.lpsiE[pb][2][0] + qp);
   }
-  VF<V> n11 = o11, n20 = o20, n00 = o00, n21 = o21, n01 = o01, n10 = o10;   // masked nodes keep lambda_psi
-  float dummy;
+
+  // --- G = ce * lE at the cell and its high-side neighbours; plain part ---
+  gx_zp = ce_zp * gx_zp;
+  gy_zp = ce_zp * gy_zp;
 #pragma unroll
   for (int v = 0; v < V; ++v) {
-    const int k = k0 + v;
+    gx.v[v] = ce.v[v] * gx.v[v];
+    gy.v[v] = ce.v[v] * gy.v[v];
+    gz.v[v] = ce.v[v] * gz.v[v];
+    gy_xp.v[v] = ce_xp.v[v] * gy_xp.v[v];
+    gz_xp.v[v] = ce_xp.v[v] * gz_xp.v[v];
+    gx_yp.v[v] = ce_yp.v[v] * gx_yp.v[v];
+    gz_yp.v[v] = ce_yp.v[v] * gz_yp.v[v];
+  }
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
     const float gx_zq = v == V - 1 ? gx_zp : gx.v[v < V - 1 ? v + 1 : v];
     const float gy_zq = v == V - 1 ? gy_zp : gy.v[v < V - 1 ? v + 1 : v];
-    // PEC masks of E_c at q: Ex: j==0||k==0, Ey: k==0||i==0, Ez: i==0||j==0 ; at the +a neighbour only the other axis counts
-    float w11 = 0, w11p = 0, w20 = 0, w20p = 0, w00 = 0, w00p = 0, w21 = 0, w21p = 0, w01 = 0, w01p = 0, w10 = 0, w10p = 0;
-    if (xs) {
-      if (!(k == 0 || i == 0)) w11 = cpml_adjoint_term(-gy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);   // (c=1,t=1): g = -G_y
-      if (!(i == 0 || j == 0)) w20 = cpml_adjoint_term(gz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);    // (c=2,t=0): g = +G_z
-    }
-    if (xsp) {
-      if (k != 0) w11p = cpml_adjoint_term(-gy_xp.v[v], o11p.v[v], 0.0f, cxp, kxp, dummy);
-      if (j != 0) w20p = cpml_adjoint_term(gz_xp.v[v], o20p.v[v], 0.0f, cxp, kxp, dummy);
-    }
-    if (ys) {
-      if (!(j == 0 || k == 0)) w00 = cpml_adjoint_term(gx.v[v], o00.v[v], by, cy, ky, n00.v[v]);    // (c=0,t=0): g = +G_x
-      if (!(i == 0 || j == 0)) w21 = cpml_adjoint_term(-gz.v[v], o21.v[v], by, cy, ky, n21.v[v]);   // (c=2,t=1): g = -G_z
-    }
-    if (ysp) {
-      if (k != 0) w00p = cpml_adjoint_term(gx_yp.v[v], o00p.v[v], 0.0f, cyp, kyp, dummy);
-      if (i != 0) w21p = cpml_adjoint_term(-gz_yp.v[v], o21p.v[v], 0.0f, cyp, kyp, dummy);
-    }
-    if (P > 0 && in_slab(k, nz, P)) {
+    lhx.v[v] = lhx.v[v] + ((gz_yp.v[v] - gz.v[v]) - (gy_zq - gy.v[v]));
+    lhy.v[v] = lhy.v[v] + ((gx_zq - gx.v[v]) - (gz_xp.v[v] - gz.v[v]));
+    lhz.v[v] = lhz.v[v] + ((gy_xp.v[v] - gy.v[v]) - (gx_yp.v[v] - gx.v[v]));
+  }
+  float dummy;
+  // PEC masks of E_c at q: Ex: j==0||k==0, Ey: k==0||i==0, Ez: i==0||j==0; at the +a neighbour only the other axis counts
+  // --- z block: terms (c=0,t=1: g = -G_x -> lH_y) and (c=1,t=0: g = +G_y -> lH_x) ---
+  if (zany) {
+    VF<V> n01 = o01, n10 = o10;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
       const float bz = __ldg(d.tab[2][0] + k), cz = __ldg(d.tab[2][1] + k), kz = __ldg(d.tab[2][2] + k);
-      if (!(j == 0 || k == 0)) w01 = cpml_adjoint_term(-gx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);   // (c=0,t=1): g = -G_x
-      if (!(k == 0 || i == 0)) w10 = cpml_adjoint_term(gy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);    // (c=1,t=0): g = +G_y
-    }
-    if (P > 0 && k + 1 < nz && in_slab(k + 1, nz, P)) {
-      const float czp = __ldg(d.tab[2][1] + k + 1), kzp = __ldg(d.tab[2][2] + k + 1);
+      const float czp = k + 1 < nz ? __ldg(d.tab[2][1] + k + 1) : 0.0f, kzp = k + 1 < nz ? __ldg(d.tab[2][2] + k + 1) : 0.0f;
+      const float gx_zq = v == V - 1 ? gx_zp : gx.v[v < V - 1 ? v + 1 : v];
+      const float gy_zq = v == V - 1 ? gy_zp : gy.v[v < V - 1 ? v + 1 : v];
       const float p01 = v == V - 1 ? o01_zp : o01.v[v < V - 1 ? v + 1 : v];
       const float p10 = v == V - 1 ? o10_zp : o10.v[v < V - 1 ? v + 1 : v];
+      float w01 = 0.0f, w10 = 0.0f, w01p = 0.0f, w10p = 0.0f;
+      if (!(j == 0 || k == 0)) w01 = cpml_adjoint_term(-gx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);
+      if (!(k == 0 || i == 0)) w10 = cpml_adjoint_term(gy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);
       if (j != 0) w01p = cpml_adjoint_term(-gx_zq, p01, 0.0f, czp, kzp, dummy);
       if (i != 0) w10p = cpml_adjoint_term(gy_zq, p10, 0.0f, czp, kzp, dummy);
+      lhx.v[v] -= (w10p - w10);
+      lhy.v[v] -= (w01p - w01);
     }
-    // lH_x: d1 = d_y^+ G_z, d2 = d_z^+ G_y ; then (c=1,t=0,a=z), then (c=2,t=1,a=y)
-    {
-      float x = lhx.v[v] + ((gz_yp.v[v] - gz.v[v]) - (gy_zq - gy.v[v]));
-      x -= (w10p - w10);
-      x -= (w21p - w21);
-      lhx.v[v] = x;
+    if (zs0) {
+      stv<V>(d.lpsiE[nb][0][1] + qz, n01);
+      stv<V>(d.lpsiE[nb][1][0] + qz, n10);
     }
-    // lH_y: d1 = d_z^+ G_x, d2 = d_x^+ G_z ; then (c=0,t=1,a=z), then (c=2,t=0,a=x)
-    {
-      float x = lhy.v[v] + ((gx_zq - gx.v[v]) - (gz_xp.v[v] - gz.v[v]));
-      x -= (w01p - w01);
-      x -= (w20p - w20);
-      lhy.v[v] = x;
+  }
+  // --- y block: terms (c=0,t=0: g = +G_x -> lH_z) and (c=2,t=1: g = -G_z -> lH_x) ---
+  if (HY && (ys || ysp)) {
+    const float by = __ldg(d.tab[1][0] + j), cy = __ldg(d.tab[1][1] + j), ky = __ldg(d.tab[1][2] + j);
+    const float cyp = j + 1 < ny ? __ldg(d.tab[1][1] + j + 1) : 0.0f, kyp = j + 1 < ny ? __ldg(d.tab[1][2] + j + 1) : 0.0f;
+    VF<V> n00 = o00, n21 = o21;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
+      float w00 = 0.0f, w21 = 0.0f, w00p = 0.0f, w21p = 0.0f;
+      if (!(j == 0 || k == 0)) w00 = cpml_adjoint_term(gx.v[v], o00.v[v], by, cy, ky, n00.v[v]);
+      if (!(i == 0 || j == 0)) w21 = cpml_adjoint_term(-gz.v[v], o21.v[v], by, cy, ky, n21.v[v]);
+      if (k != 0) w00p = cpml_adjoint_term(gx_yp.v[v], o00p.v[v], 0.0f, cyp, kyp, dummy);
+      if (i != 0) w21p = cpml_adjoint_term(-gz_yp.v[v], o21p.v[v], 0.0f, cyp, kyp, dummy);
+      lhx.v[v] -= (w21p - w21);
+      lhz.v[v] -= (w00p - w00);
     }
-    // lH_z: d1 = d_x^+ G_y, d2 = d_y^+ G_x ; then (c=0,t=0,a=y), then (c=1,t=1,a=x)
-    {
-      float x = lhz.v[v] + ((gy_xp.v[v] - gy.v[v]) - (gx_yp.v[v] - gx.v[v]));
-      x -= (w00p - w00);
-      x -= (w11p - w11);
-      lhz.v[v] = x;
+    if (ys) {
+      stv<V>(d.lpsiE[nb][0][0] + qy, n00);
+      stv<V>(d.lpsiE[nb][2][1] + qy, n21);
+    }
+  }
+  // --- x block: terms (c=1,t=1: g = -G_y -> lH_z) and (c=2,t=0: g = +G_z -> lH_y) ---
+  if (HX && (xs || xsp)) {
+    const float bx = __ldg(d.tab[0][0] + i), cx = __ldg(d.tab[0][1] + i), kx = __ldg(d.tab[0][2] + i);
+    const float cxp = i + 1 < nx ? __ldg(d.tab[0][1] + i + 1) : 0.0f, kxp = i + 1 < nx ? __ldg(d.tab[0][2] + i + 1) : 0.0f;
+    VF<V> n11 = o11, n20 = o20;
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      const int k = k0 + v;
+      float w11 = 0.0f, w20 = 0.0f, w11p = 0.0f, w20p = 0.0f;
+      if (!(k == 0 || i == 0)) w11 = cpml_adjoint_term(-gy.v[v], o11.v[v], bx, cx, kx, n11.v[v]);
+      if (!(i == 0 || j == 0)) w20 = cpml_adjoint_term(gz.v[v], o20.v[v], bx, cx, kx, n20.v[v]);
+      if (k != 0) w11p = cpml_adjoint_term(-gy_xp.v[v], o11p.v[v], 0.0f, cxp, kxp, dummy);
+      if (j != 0) w20p = cpml_adjoint_term(gz_xp.v[v], o20p.v[v], 0.0f, cxp, kxp, dummy);
+      lhy.v[v] -= (w20p - w20);
+      lhz.v[v] -= (w11p - w11);
+    }
+    if (xs) {
+      stv<V>(d.lpsiE[nb][1][1] + qx, n11);
+      stv<V>(d.lpsiE[nb][2][0] + qx, n20);
     }
   }
   stv<V>(d.lH[0] + q, lhx);
   stv<V>(d.lH[1] + q, lhy);
   stv<V>(d.lH[2] + q, lhz);
-  const int nb = pb ^ 1;
-  if (xs) {
-    stv<V>(d.lpsiE[nb][1][1] + qx, n11);
-    stv<V>(d.lpsiE[nb][2][0] + qx, n20);
-  }
-  if (ys) {
-    stv<V>(d.lpsiE[nb][0][0] + qy, n00);
-    stv<V>(d.lpsiE[nb][2][1] + qy, n21);
-  }
-  if (zs0) {
-    stv<V>(d.lpsiE[nb][0][1] + qz, n01);
-    stv<V>(d.lpsiE[nb][1][0] + qz, n10);
-  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// GENERAL kernels: one launch per half-step over the box list; each block runs the body of its box's class.
+// ---------------------------------------------------------------------------------------------------------
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+  int b, i, j, k0;
+  if (!box_decode<V>(B, b, i, j, k0)) return;
+  FDTD_CLASS_DISPATCH(gen_e_body, d, i, j, k0)
+}
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+  int b, i, j, k0;
+  if (!box_decode<V>(B, b, i, j, k0)) return;
+  FDTD_CLASS_DISPATCH(gen_h_body, d, i, j, k0)
+}
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+  int b, i, j, k0;
+  if (!box_decode<V>(B, b, i, j, k0)) return;
+  FDTD_CLASS_DISPATCH(gen_adj_h_body, d, i, j, k0, pb)
+}
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+  int b, i, j, k0;
+  if (!box_decode<V>(B, b, i, j, k0)) return;
+  FDTD_CLASS_DISPATCH(gen_adj_e_body, d, i, j, k0, pb)
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -703,8 +750,8 @@ template <int V, bool ADJ>
 __global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
   int i, j, k0;
   if (!lean_decode<V>(r, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const float* const* in = ADJ ? d.lH : d.H;
   float* const* out = ADJ ? d.lE : d.E;
   const VF<V> hx = ldv<V>(in[0] + q), hy = ldv<V>(in[1] + q), hz = ldv<V>(in[2] + q);
@@ -734,8 +781,8 @@ template <int V>
 __global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
   int i, j, k0;
   if (!lean_decode<V>(r, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   const VF<V> ey_xp = ldv<V>(d.E[1] + q + sx), ez_xp = ldv<V>(d.E[2] + q + sx);
   const VF<V> ex_yp = ldv<V>(d.E[0] + q + sy), ez_yp = ldv<V>(d.E[2] + q + sy);
@@ -760,8 +807,8 @@ template <int V>
 __global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
   int i, j, k0;
   if (!lean_decode<V>(r, i, j, k0)) return;
-  const long long sx = d.sx, sy = d.sy;
-  const long long q = ((long long)i * d.n[1] + j) * d.n[2] + k0;
+  const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ce = ldv<V>(d.ce + q), ce_xp = ldv<V>(d.ce + q + sx), ce_yp = ldv<V>(d.ce + q + sy);
   const float ce_zp = d.ce[q + V];
   VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
