@@ -50,6 +50,27 @@ def make_workload(name, nsteps, seed_offset=0):
     return f(**kw)
 
 
+def replica_seed_offset(rank):
+    """Replica r of an N-GPU run gets its own seeded design (the paper's batch of independent gradients)."""
+    return int(rank)
+
+
+def reduce_max(values, world, device=None):
+    """Max over ranks of a list of floats (device timings): the slowest replica sets the job's time."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.tolist()]
+
+
+def whole_job_value(cells, nsteps, steps, world, total_ms):
+    """Mcell-updates/s of the whole job: every replica's cell updates over the slowest replica's time."""
+    return float(cells) * nsteps * steps * world / (total_ms * 1e-3) / 1e6
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -104,7 +125,7 @@ def run_gpu(args, rank, world):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-    w = make_workload(args.workload, args.nsteps, seed_offset=rank)
+    w = make_workload(args.workload, args.nsteps, seed_offset=replica_seed_offset(rank))
     flags = fdtd.WS_REVERSE | fdtd.WS_HOST_IO
     eps_dev = torch.from_numpy(w.eps).to(dev)
     sim = fdtd.Sim(eps_dev, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor)
@@ -165,12 +186,8 @@ def run_gpu(args, rank, world):
     launches = sim.launch_count() - l0
     clocks = sampler.stop(t0, t1) if sampler else None
     tot_ms = float(np.sum(tf) + np.sum(tr))
-    t = torch.tensor([tot_ms, float(np.sum(tf)), float(np.sum(tr))], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    tot_ms, f_ms, r_ms = [float(x) for x in t.tolist()]
-    cell_updates = float(w.cells) * w.nsteps * args.steps * world
-    value = cell_updates / (tot_ms * 1e-3) / 1e6
+    tot_ms, f_ms, r_ms = reduce_max([tot_ms, float(np.sum(tf)), float(np.sum(tr))], world, dev)
+    value = whole_job_value(w.cells, w.nsteps, args.steps, world, tot_ms)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     eps_host = torch.from_numpy(w.eps).pin_memory()
@@ -199,11 +216,9 @@ def run_gpu(args, rank, world):
     e2e_ms = max(ev0.elapsed_time(ev1), 0.0)
     e2e_wall = (time.perf_counter() - te) * 1e3
     e2e_ms = max(e2e_ms, e2e_wall)                      # host work sits between GPU segments: take the longer clock
-    te_t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(te_t, op=dist.ReduceOp.MAX)
+    e2e_ms = reduce_max([e2e_ms], world, dev)[0]
     amp_bytes = sum(int(np.prod([s.hi[a] - s.lo[a] for a in range(3)])) * 4 for s in w.sources if s.amp is not None)
-    e2e = {"value": float(w.cells) * w.nsteps * ne2e * world / (float(te_t.item()) * 1e-3) / 1e6, "unit": UNIT,
+    e2e = {"value": whole_job_value(w.cells, w.nsteps, ne2e, world, e2e_ms), "unit": UNIT,
            "h2d_bytes_per_step": int(w.eps.nbytes + dmon_host.numel() * 4 + amp_bytes + sum(s.wave.nbytes for s in w.sources)),
            "d2h_bytes_per_step": int(mon_host.numel() * 4 + grad_host.numel() * 4), "steps": ne2e}
     if world > 1:
@@ -257,8 +272,8 @@ def run_gpu(args, rank, world):
                    "l2": "256 MB write between timed steps flushes L2; inside a step the working set "
                          f"({13 * w.cells * 4 / 1e6:.0f} MB of fields) is what the workload itself keeps resident",
                    "replicas": world, "parallelism": "replicas only (the path runs on one GPU)"},
-        "forward_mcells_per_s": float(w.cells) * w.nsteps * args.steps * world / (f_ms * 1e-3) / 1e6,
-        "reverse_mcells_per_s": float(w.cells) * w.nsteps * args.steps * world / (r_ms * 1e-3) / 1e6,
+        "forward_mcells_per_s": whole_job_value(w.cells, w.nsteps, args.steps, world, f_ms),
+        "reverse_mcells_per_s": whole_job_value(w.cells, w.nsteps, args.steps, world, r_ms),
         "forward_ms": f_ms / args.steps, "reverse_ms": r_ms / args.steps,
         "store_bytes": sim_store_bytes(sim, w, flags), "store_bytes_per_step": sim_store_bytes(sim, w, flags) / w.nsteps,
         "store_bytes_f32_k1": (w.nsteps + 1) * sim.slot_values() * 4,

@@ -37,6 +37,15 @@ struct Layout {
 
 }  // namespace
 
+namespace {
+struct Split {          // one half-step over an x range: lean region + complement boxes
+  Region reg{};
+  bool has_lean = false;
+  BoxList boxes{};
+  int x0 = 0, x1 = 0;
+};
+}  // namespace
+
 struct fdtd_sim {
   int n[3] = {0, 0, 0};
   int P = 0;
@@ -71,9 +80,8 @@ struct fdtd_sim {
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
   // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
-  Region reg[4]{};
-  bool has_lean[4] = {false, false, false, false};
-  BoxList boxes[4]{};
+  Split split[4]{};
+
   // run state
   int nsteps = 0, k = 1, dtype = 0;
   bool forward_done = false, state_final = false;
@@ -234,9 +242,11 @@ unsigned make_ginv(int G) {
 }
 
 // Lean region [lo, hi) of split half-step `which` and the disjoint boxes covering the rest of the grid.
-void make_split(fdtd_sim* s, int which) {
+Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
   const int P = s->P, V = s->V, VG = s->VG;
-  Region& r = s->reg[which];
+  Split sp;
+  sp.x0 = x0; sp.x1 = x1;
+  Region full;
   for (int a = 0; a < 3; ++a) {
     const int n = s->n[a];
     int lo, hi;
@@ -247,15 +257,20 @@ void make_split(fdtd_sim* s, int which) {
       default: lo = P; hi = std::min(n - P - 1, n - 1); break;        // adj E: the +1 neighbour must not be a slab cell
     }
     if (a == 2) { lo = (lo + V - 1) / V * V; hi = hi / V * V; }
-    r.lo[a] = lo; r.hi[a] = hi;
+    full.lo[a] = lo; full.hi[a] = hi;
   }
-  s->has_lean[which] = r.hi[0] > r.lo[0] && r.hi[1] > r.lo[1] && r.hi[2] > r.lo[2];
-  BoxList& B = s->boxes[which];
+  const bool full_lean = full.hi[0] > full.lo[0] && full.hi[1] > full.lo[1] && full.hi[2] > full.lo[2];
+  Region& r = sp.reg;
+  r = full;
+  r.lo[0] = std::max(full.lo[0], x0); r.hi[0] = std::min(full.hi[0], x1);
+  sp.has_lean = full_lean && r.hi[0] > r.lo[0];
+  BoxList& B = sp.boxes;
   B = BoxList{};
-  auto add = [&](int cls, int x0, int x1, int y0, int y1, int z0, int z1) {
-    if (x1 <= x0 || y1 <= y0 || z1 <= z0) return;
+  auto add = [&](int cls, int bx0, int bx1, int y0, int y1, int z0, int z1) {
+    bx0 = std::max(bx0, x0); bx1 = std::min(bx1, x1);
+    if (bx1 <= bx0 || y1 <= y0 || z1 <= z0) return;
     const int b = B.nb++;
-    B.lo[b][0] = x0; B.hi[b][0] = x1; B.lo[b][1] = y0; B.hi[b][1] = y1; B.lo[b][2] = z0; B.hi[b][2] = z1;
+    B.lo[b][0] = bx0; B.hi[b][0] = bx1; B.lo[b][1] = y0; B.hi[b][1] = y1; B.lo[b][2] = z0; B.hi[b][2] = z1;
     B.cls[b] = cls;
     const int groups = (z1 - z0 + VG - 1) / VG;
     const int G = std::min(groups, 32), RW = 32 / G;
@@ -263,23 +278,23 @@ void make_split(fdtd_sim* s, int which) {
     B.ginv[b] = make_ginv(G);
     B.nbx[b] = (groups + G - 1) / G;
     B.nby[b] = (y1 - y0 + TY * RW - 1) / (TY * RW);
-    B.dnbx[b] = make_fastdiv((unsigned)B.nbx[b], (unsigned)B.nbx[b] * B.nby[b] * (unsigned)(x1 - x0));
-    B.dnby[b] = make_fastdiv((unsigned)B.nby[b], (unsigned)B.nby[b] * (unsigned)(x1 - x0));
-    B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b] * (x1 - x0);
+    B.dnbx[b] = make_fastdiv((unsigned)B.nbx[b], (unsigned)B.nbx[b] * B.nby[b] * (unsigned)(bx1 - bx0));
+    B.dnby[b] = make_fastdiv((unsigned)B.nby[b], (unsigned)B.nby[b] * (unsigned)(bx1 - bx0));
+    B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b] * (bx1 - bx0);
   };
   const int nx = s->n[0], ny = s->n[1], nz = s->n[2];
   // classes: the x range of the lean region holds no x-slab cell, no wall plane and (adjoint) no cell whose x
   // neighbour is a slab cell, so boxes confined to it need no x terms (CLS_Y); likewise y for CLS_Z
-  if (!s->has_lean[which]) { add(CLS_X, 0, nx, 0, ny, 0, nz); return; }
-  add(CLS_X, 0, r.lo[0], 0, ny, 0, nz);
-  add(CLS_X, r.hi[0], nx, 0, ny, 0, nz);
-  add(CLS_Y, r.lo[0], r.hi[0], 0, r.lo[1], 0, nz);
-  add(CLS_Y, r.lo[0], r.hi[0], r.hi[1], ny, 0, nz);
-  add(CLS_Z, r.lo[0], r.hi[0], r.lo[1], r.hi[1], 0, r.lo[2]);
-  add(CLS_Z, r.lo[0], r.hi[0], r.lo[1], r.hi[1], r.hi[2], nz);
+  if (!full_lean) { add(CLS_X, 0, nx, 0, ny, 0, nz); return sp; }
+  add(CLS_X, 0, full.lo[0], 0, ny, 0, nz);
+  add(CLS_X, full.hi[0], nx, 0, ny, 0, nz);
+  add(CLS_Y, full.lo[0], full.hi[0], 0, full.lo[1], 0, nz);
+  add(CLS_Y, full.lo[0], full.hi[0], full.hi[1], ny, 0, nz);
+  add(CLS_Z, full.lo[0], full.hi[0], full.lo[1], full.hi[1], 0, full.lo[2]);
+  add(CLS_Z, full.lo[0], full.hi[0], full.lo[1], full.hi[1], full.hi[2], nz);
+  return sp;
 }
-dim3 grid_lean(const fdtd_sim* s, int which) {
-  const Region& r = s->reg[which];
+dim3 grid_lean(const fdtd_sim* s, const Region& r) {
   return dim3((unsigned)((r.hi[2] - r.lo[2] + 32 * s->V - 1) / (32 * s->V)), (unsigned)((r.hi[1] - r.lo[1] + TY - 1) / TY),
               (unsigned)(r.hi[0] - r.lo[0]));
 }
@@ -317,11 +332,11 @@ void join(fdtd_sim* s, int branches) {
   }
 }
 
-void launch_lean(fdtd_sim* s, int which) {
-  if (!s->has_lean[which]) return;
+void launch_lean(fdtd_sim* s, int which, const Split& sp) {
+  if (!sp.has_lean) return;
   const dim3 b(32, TY);
-  const dim3 g = grid_lean(s, which);
-  const Region& r = s->reg[which];
+  const dim3 g = grid_lean(s, sp.reg);
+  const Region& r = sp.reg;
   if (s->V == 4) {
     switch (which) {
       case 0: LAUNCH(s, (k_lean_curlm<4, false>), g, b, s->d, r); break;
@@ -338,9 +353,9 @@ void launch_lean(fdtd_sim* s, int which) {
     }
   }
 }
-void launch_gen(fdtd_sim* s, int which, int pb) {
+void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp) {
   const dim3 b(32, TY);
-  const BoxList& B = s->boxes[which];
+  const BoxList& B = sp.boxes;
   const unsigned g = (unsigned)B.off[B.nb];
   if (g == 0) return;
   if (s->VG == 4) {
@@ -367,6 +382,8 @@ void launch_gen(fdtd_sim* s, int which, int pb) {
   }
 }
 // The four split half-steps: lean kernel on the plain cells + general kernel on the rest (disjoint writes).
+void launch_lean(fdtd_sim* s, int which) { launch_lean(s, which, s->split[which]); }
+void launch_gen(fdtd_sim* s, int which, int pb) { launch_gen(s, which, pb, s->split[which]); }
 void launch_split(fdtd_sim* s, int which, int pb) {
   launch_lean(s, which);
   launch_gen(s, which, pb);
@@ -402,8 +419,11 @@ void launch_grad(fdtd_sim* s) {
   const long long cells = (long long)ext[0] * ext[1] * ext[2];
   LAUNCH(s, k_grad, (unsigned)((cells + 255) / 256), 256, s->d);
 }
-void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
+void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, int x0 = 0, int x1 = 1 << 30) {
   if (s->nsrc == 0) return;
+  bool any = false;
+  for (int i = 0; i < s->nsrc; ++i) any = any || (s->src_host[i].lo[0] < x1 && s->src_host[i].hi[0] > x0);
+  if (!any) return;
   long long maxc = 1;
   for (int i = 0; i < s->nsrc; ++i) {
     const SrcDev& q = s->src_host[i];
@@ -412,7 +432,7 @@ void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign) {
   const int threads = maxc >= 128 ? 128 : 32;
   const dim3 g((unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024), (unsigned)s->nsrc);
   LAUNCH(s, k_sources, g, threads, s->d, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
-         reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign);
+         reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign, x0, x1);
 }
 void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode) {
   const long long tot = (long long)b.ncomp * (b.hi[0] - b.lo[0]) * (b.hi[1] - b.lo[1]) * (b.hi[2] - b.lo[2]);
@@ -822,7 +842,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   s->V = (s->n[2] % 4 == 0 && s->P % 4 == 0) ? 4 : 1;
   s->VG = s->V == 4 ? 4 : 1;
   if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2 || v == 4) && s->V == 4) s->VG = v; }
-  for (int which = 0; which < 4; ++which) make_split(s, which);
+  for (int which = 0; which < 4; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
   build_tables(s);
   CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
   CUDA_TRY(s, cudaMemsetAsync(w + L.step, 0, 16, s->stream));

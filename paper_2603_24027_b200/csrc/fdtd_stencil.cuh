@@ -46,202 +46,240 @@ __device__ __forceinline__ bool box_decode(const BoxList& B, int& b, int& i, int
   }
 
 // ---------------------------------------------------------------------------------------------------------
+// Forward half-steps on the slab boxes.  Layout of both bodies: all loads first; per component the plain update
+// x = fma(coef, d1 - d2, x), then its CPML term of axis a1, then of axis a2 (canonical order, R3), each term
+// one block under a thread-level condition (x: block-uniform, y: row-uniform, z: uniform over the thread's group,
+// since P % V == 0); PEC-masked nodes are zeroed once at the end.
+// ---------------------------------------------------------------------------------------------------------
+// one CPML term over the thread's V cells: psi = fma(b, psi, c*d); x = fma(sgn*coef, fma(k, d, psi), x)
+template <int V, bool ZAXIS>
+__device__ __forceinline__ void cpml_term(VF<V>& x, VF<V>& psi, const VF<V>& coef, const float sgn, const float* dv,
+                                          const float* b, const float* c, const float* k) {
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const int t = ZAXIS ? v : 0;                 // coefficients vary along z only
+    const float ps = fmaf(b[t], psi.v[v], c[t] * dv[v]);
+    psi.v[v] = ps;
+    x.v[v] = fmaf(sgn * coef.v[v], fmaf(k[t], dv[v], ps), x.v[v]);
+  }
+}
+
 // Forward E half-step (SURVEY 8(a) rows A1 + A3):  E_c += ce * (d_a1^- H_b1 - d_a2^- H_b2) + CPML terms,
 // tangential E on the three low PEC walls held at zero.  DESIGN.md R1-R5.
-// ---------------------------------------------------------------------------------------------------------
 template <int V, bool HX, bool HY>
 __device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int j, const int k0) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
+  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
+  const bool xs = HX && P > 0 && in_slab(i, nx, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P);
+  const bool zs = P > 0 && in_slab(k0, nz, P);
 
-  bool zs[V];
-  float bz[V], cz[V], kz[V];
+  const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  VF<V> hy_xm = zerov<V>(), hz_xm = zerov<V>(), hx_ym = zerov<V>(), hz_ym = zerov<V>();
+  if (i > 0) {
+    hy_xm = ldv<V>(d.H[1] + q - sx);
+    hz_xm = ldv<V>(d.H[2] + q - sx);
+  }
+  if (j > 0) {
+    hx_ym = ldv<V>(d.H[0] + q - sy);
+    hz_ym = ldv<V>(d.H[2] + q - sy);
+  }
+  float hx_z0 = 0.0f, hy_z0 = 0.0f;
+  if (k0 > 0) {
+    hx_z0 = d.H[0][q - 1];
+    hy_z0 = d.H[1][q - 1];
+  }
+  VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  const VF<V> ce = ldv<V>(d.ce + q);
+  // psi_E[c][t]: (0,0)=Ex/y (0,1)=Ex/z (1,0)=Ey/z (1,1)=Ey/x (2,0)=Ez/x (2,1)=Ez/y
+  VF<V> p_ey_x, p_ez_x, p_ex_y, p_ez_y, p_ex_z, p_ey_z;
+  idx_t qx = 0, qy = 0, qz = 0;
+  float bx = 0, cx = 0, kx = 0, by = 0, cy = 0, ky = 0, bz[V], cz[V], kz[V];
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    p_ey_x = ldv<V>(d.psiE[1][1] + qx);
+    p_ez_x = ldv<V>(d.psiE[2][0] + qx);
+    bx = __ldg(d.tab[0][0] + i); cx = __ldg(d.tab[0][1] + i); kx = __ldg(d.tab[0][2] + i);
+  }
+  if (ys) {
+    qy = psi_index(d, 1, i, j, k0);
+    p_ex_y = ldv<V>(d.psiE[0][0] + qy);
+    p_ez_y = ldv<V>(d.psiE[2][1] + qy);
+    by = __ldg(d.tab[1][0] + j); cy = __ldg(d.tab[1][1] + j); ky = __ldg(d.tab[1][2] + j);
+  }
+  if (zs) {
+    qz = psi_index(d, 2, i, j, k0);
+    p_ex_z = ldv<V>(d.psiE[0][1] + qz);
+    p_ey_z = ldv<V>(d.psiE[1][0] + qz);
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+      bz[v] = __ldg(d.tab[2][0] + k0 + v); cz[v] = __ldg(d.tab[2][1] + k0 + v); kz[v] = __ldg(d.tab[2][2] + k0 + v);
+    }
+  }
+  // the six one-sided differences
+  float dy_hz[V], dz_hy[V], dz_hx[V], dx_hz[V], dx_hy[V], dy_hx[V];
 #pragma unroll
   for (int v = 0; v < V; ++v) {
-    const int k = k0 + v;
-    zs[v] = P > 0 && in_slab(k, nz, P);
-    bz[v] = zs[v] ? __ldg(d.tab[2][0] + k) : 0.0f;
-    cz[v] = zs[v] ? __ldg(d.tab[2][1] + k) : 0.0f;
-    kz[v] = zs[v] ? __ldg(d.tab[2][2] + k) : 0.0f;
+    const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+    const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+    dy_hz[v] = hz.v[v] - hz_ym.v[v];
+    dz_hy[v] = hy.v[v] - hy_zm;
+    dz_hx[v] = hx.v[v] - hx_zm;
+    dx_hz[v] = hz.v[v] - hz_xm.v[v];
+    dx_hy[v] = hy.v[v] - hy_xm.v[v];
+    dy_hx[v] = hx.v[v] - hx_ym.v[v];
   }
-  const bool ys = HY && P > 0 && in_slab(j, ny, P);
-  const float by = ys ? __ldg(d.tab[1][0] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][1] + j) : 0.0f,
-              ky = ys ? __ldg(d.tab[1][2] + j) : 0.0f;
-
-  const idx_t q = ((idx_t)i * ny + j) * nz + k0;
-  VF<V> pHy = zerov<V>(), pHz = zerov<V>();
-  if (i > 0) {
-    pHy = ldv<V>(d.H[1] + q - sx);
-    pHz = ldv<V>(d.H[2] + q - sx);
-  }
-  {
-    const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
-    VF<V> hx_ym = zerov<V>(), hz_ym = zerov<V>();
-    if (j > 0) {
-      hx_ym = ldv<V>(d.H[0] + q - sy);
-      hz_ym = ldv<V>(d.H[2] + q - sy);
-    }
-    float hx_z0 = 0.0f, hy_z0 = 0.0f;
-    if (k0 > 0) {
-      hx_z0 = d.H[0][q - 1];
-      hy_z0 = d.H[1][q - 1];
-    }
-    VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
-    const VF<V> ce = ldv<V>(d.ce + q);
-
-    const bool xs = HX && P > 0 && in_slab(i, nx, P);
-    const float bx = xs ? __ldg(d.tab[0][0] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][1] + i) : 0.0f,
-                kx = xs ? __ldg(d.tab[0][2] + i) : 0.0f;
-    // psi_E[c][t]: (0,0)=Ex/y (0,1)=Ex/z (1,0)=Ey/z (1,1)=Ey/x (2,0)=Ez/x (2,1)=Ez/y
-    VF<V> p_ey_x = zerov<V>(), p_ez_x = zerov<V>(), p_ex_y = zerov<V>(), p_ez_y = zerov<V>(),
-          p_ex_z = zerov<V>(), p_ey_z = zerov<V>();
-    idx_t qx = 0, qy = 0, qz = 0;
-    if (xs) {
-      qx = psi_index(d, 0, i, j, k0);
-      p_ey_x = ldv<V>(d.psiE[1][1] + qx);
-      p_ez_x = ldv<V>(d.psiE[2][0] + qx);
-    }
-    if (ys) {
-      qy = psi_index(d, 1, i, j, k0);
-      p_ex_y = ldv<V>(d.psiE[0][0] + qy);
-      p_ez_y = ldv<V>(d.psiE[2][1] + qy);
-    }
-    if (zs[0]) {
-      qz = psi_index(d, 2, i, j, k0);
-      p_ex_z = ldv<V>(d.psiE[0][1] + qz);
-      p_ey_z = ldv<V>(d.psiE[1][0] + qz);
-    }
+  // Ex: a1 = y (d_y^- Hz), a2 = z (d_z^- Hy)
+#pragma unroll
+  for (int v = 0; v < V; ++v) ex.v[v] = fmaf(ce.v[v], dy_hz[v] - dz_hy[v], ex.v[v]);
+  if (ys) cpml_term<V, false>(ex, p_ex_y, ce, 1.0f, dy_hz, &by, &cy, &ky);
+  if (zs) cpml_term<V, true>(ex, p_ex_z, ce, -1.0f, dz_hy, bz, cz, kz);
+  // Ey: a1 = z (d_z^- Hx), a2 = x (d_x^- Hz)
+#pragma unroll
+  for (int v = 0; v < V; ++v) ey.v[v] = fmaf(ce.v[v], dz_hx[v] - dx_hz[v], ey.v[v]);
+  if (zs) cpml_term<V, true>(ey, p_ey_z, ce, 1.0f, dz_hx, bz, cz, kz);
+  if (xs) cpml_term<V, false>(ey, p_ey_x, ce, -1.0f, dx_hz, &bx, &cx, &kx);
+  // Ez: a1 = x (d_x^- Hy), a2 = y (d_y^- Hx)
+#pragma unroll
+  for (int v = 0; v < V; ++v) ez.v[v] = fmaf(ce.v[v], dx_hy[v] - dy_hx[v], ez.v[v]);
+  if (xs) cpml_term<V, false>(ez, p_ez_x, ce, 1.0f, dx_hy, &bx, &cx, &kx);
+  if (ys) cpml_term<V, false>(ez, p_ez_y, ce, -1.0f, dy_hx, &by, &cy, &ky);
+  // PEC walls (rare): a masked node keeps E = 0 and its psi untouched, as if the update had skipped it
+  if (i == 0 || j == 0 || k0 == 0) {
+    auto keep = [&](VF<V>& psi, const float* arr, idx_t qq, bool active, bool ij_masked, bool k_masks) {
+      if (!active) return;
+      const VF<V> old = ldv<V>(arr + qq);
+#pragma unroll
+      for (int v = 0; v < V; ++v)
+        if (ij_masked || (k_masks && k0 + v == 0)) psi.v[v] = old.v[v];
+    };
+    keep(p_ex_y, d.psiE[0][0], qy, ys, j == 0, true);
+    keep(p_ex_z, d.psiE[0][1], qz, zs, j == 0, true);
+    keep(p_ey_z, d.psiE[1][0], qz, zs, i == 0, true);
+    keep(p_ey_x, d.psiE[1][1], qx, xs, i == 0, true);
+    keep(p_ez_x, d.psiE[2][0], qx, xs, i == 0 || j == 0, false);
+    keep(p_ez_y, d.psiE[2][1], qy, ys, i == 0 || j == 0, false);
 #pragma unroll
     for (int v = 0; v < V; ++v) {
       const int k = k0 + v;
-      const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
-      const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
-      // Ex: a1 = y (d_y^- Hz), a2 = z (d_z^- Hy)
       if (j == 0 || k == 0) ex.v[v] = 0.0f;
-      else ex.v[v] = yee_update(ex.v[v], ce.v[v], hz.v[v] - hz_ym.v[v], hy.v[v] - hy_zm, ys, by, cy, ky, p_ex_y.v[v],
-                                zs[v], bz[v], cz[v], kz[v], p_ex_z.v[v]);
-      // Ey: a1 = z (d_z^- Hx), a2 = x (d_x^- Hz)
       if (k == 0 || i == 0) ey.v[v] = 0.0f;
-      else ey.v[v] = yee_update(ey.v[v], ce.v[v], hx.v[v] - hx_zm, hz.v[v] - pHz.v[v], zs[v], bz[v], cz[v], kz[v],
-                                p_ey_z.v[v], xs, bx, cx, kx, p_ey_x.v[v]);
-      // Ez: a1 = x (d_x^- Hy), a2 = y (d_y^- Hx)
       if (i == 0 || j == 0) ez.v[v] = 0.0f;
-      else ez.v[v] = yee_update(ez.v[v], ce.v[v], hy.v[v] - pHy.v[v], hx.v[v] - hx_ym.v[v], xs, bx, cx, kx,
-                                p_ez_x.v[v], ys, by, cy, ky, p_ez_y.v[v]);
     }
-    stv<V>(d.E[0] + q, ex);
-    stv<V>(d.E[1] + q, ey);
-    stv<V>(d.E[2] + q, ez);
-    if (xs) {
-      stv<V>(d.psiE[1][1] + qx, p_ey_x);
-      stv<V>(d.psiE[2][0] + qx, p_ez_x);
-    }
-    if (ys) {
-      stv<V>(d.psiE[0][0] + qy, p_ex_y);
-      stv<V>(d.psiE[2][1] + qy, p_ez_y);
-    }
-    if (zs[0]) {
-      stv<V>(d.psiE[0][1] + qz, p_ex_z);
-      stv<V>(d.psiE[1][0] + qz, p_ey_z);
-    }
+  }
+  stv<V>(d.E[0] + q, ex);
+  stv<V>(d.E[1] + q, ey);
+  stv<V>(d.E[2] + q, ez);
+  if (xs) {
+    stv<V>(d.psiE[1][1] + qx, p_ey_x);
+    stv<V>(d.psiE[2][0] + qx, p_ez_x);
+  }
+  if (ys) {
+    stv<V>(d.psiE[0][0] + qy, p_ex_y);
+    stv<V>(d.psiE[2][1] + qy, p_ez_y);
+  }
+  if (zs) {
+    stv<V>(d.psiE[0][1] + qz, p_ex_z);
+    stv<V>(d.psiE[1][0] + qz, p_ey_z);
   }
 }
 
-// ---------------------------------------------------------------------------------------------------------
 // Forward H half-step (rows A2 + A4):  H_c -= S * (d_a1^+ E_b1 - d_a2^+ E_b2) + CPML terms; ghost E[n] = 0.
-// ---------------------------------------------------------------------------------------------------------
 template <int V, bool HX, bool HY>
 __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int j, const int k0) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
-  const float mS = -d.S;
-
-  bool zs[V];
-  float bz[V], cz[V], kz[V];
-#pragma unroll
-  for (int v = 0; v < V; ++v) {
-    const int k = k0 + v;
-    zs[v] = P > 0 && in_slab(k, nz, P);
-    bz[v] = zs[v] ? __ldg(d.tab[2][3] + k) : 0.0f;
-    cz[v] = zs[v] ? __ldg(d.tab[2][4] + k) : 0.0f;
-    kz[v] = zs[v] ? __ldg(d.tab[2][5] + k) : 0.0f;
-  }
-  const bool ys = HY && P > 0 && in_slab(j, ny, P);
-  const float by = ys ? __ldg(d.tab[1][3] + j) : 0.0f, cy = ys ? __ldg(d.tab[1][4] + j) : 0.0f,
-              ky = ys ? __ldg(d.tab[1][5] + j) : 0.0f;
-
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
-  const VF<V> ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
-  {
-    const VF<V> ex = ldv<V>(d.E[0] + q);
-    VF<V> ey_xp = zerov<V>(), ez_xp = zerov<V>();
-    if (i + 1 < nx) {
-      ey_xp = ldv<V>(d.E[1] + q + sx);
-      ez_xp = ldv<V>(d.E[2] + q + sx);
-    }
-    VF<V> ex_yp = zerov<V>(), ez_yp = zerov<V>();
-    if (j + 1 < ny) {
-      ex_yp = ldv<V>(d.E[0] + q + sy);
-      ez_yp = ldv<V>(d.E[2] + q + sy);
-    }
-    float ex_zp = 0.0f, ey_zp = 0.0f;
-    if (k0 + V < nz) {
-      ex_zp = d.E[0][q + V];
-      ey_zp = d.E[1][q + V];
-    }
-    VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  const bool xs = HX && P > 0 && in_slab(i, nx, P);
+  const bool ys = HY && P > 0 && in_slab(j, ny, P);
+  const bool zs = P > 0 && in_slab(k0, nz, P);
 
-    const bool xs = HX && P > 0 && in_slab(i, nx, P);
-    const float bx = xs ? __ldg(d.tab[0][3] + i) : 0.0f, cx = xs ? __ldg(d.tab[0][4] + i) : 0.0f,
-                kx = xs ? __ldg(d.tab[0][5] + i) : 0.0f;
-    // psi_H[c][t]: (0,0)=Hx/y (0,1)=Hx/z (1,0)=Hy/z (1,1)=Hy/x (2,0)=Hz/x (2,1)=Hz/y
-    VF<V> p_hy_x = zerov<V>(), p_hz_x = zerov<V>(), p_hx_y = zerov<V>(), p_hz_y = zerov<V>(),
-          p_hx_z = zerov<V>(), p_hy_z = zerov<V>();
-    idx_t qx = 0, qy = 0, qz = 0;
-    if (xs) {
-      qx = psi_index(d, 0, i, j, k0);
-      p_hy_x = ldv<V>(d.psiH[1][1] + qx);
-      p_hz_x = ldv<V>(d.psiH[2][0] + qx);
-    }
-    if (ys) {
-      qy = psi_index(d, 1, i, j, k0);
-      p_hx_y = ldv<V>(d.psiH[0][0] + qy);
-      p_hz_y = ldv<V>(d.psiH[2][1] + qy);
-    }
-    if (zs[0]) {
-      qz = psi_index(d, 2, i, j, k0);
-      p_hx_z = ldv<V>(d.psiH[0][1] + qz);
-      p_hy_z = ldv<V>(d.psiH[1][0] + qz);
-    }
+  const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  VF<V> ey_xp = zerov<V>(), ez_xp = zerov<V>(), ex_yp = zerov<V>(), ez_yp = zerov<V>();
+  if (i + 1 < nx) {
+    ey_xp = ldv<V>(d.E[1] + q + sx);
+    ez_xp = ldv<V>(d.E[2] + q + sx);
+  }
+  if (j + 1 < ny) {
+    ex_yp = ldv<V>(d.E[0] + q + sy);
+    ez_yp = ldv<V>(d.E[2] + q + sy);
+  }
+  float ex_zp = 0.0f, ey_zp = 0.0f;
+  if (k0 + V < nz) {
+    ex_zp = d.E[0][q + V];
+    ey_zp = d.E[1][q + V];
+  }
+  VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  // psi_H[c][t]: (0,0)=Hx/y (0,1)=Hx/z (1,0)=Hy/z (1,1)=Hy/x (2,0)=Hz/x (2,1)=Hz/y
+  VF<V> p_hy_x, p_hz_x, p_hx_y, p_hz_y, p_hx_z, p_hy_z;
+  idx_t qx = 0, qy = 0, qz = 0;
+  float bx = 0, cx = 0, kx = 0, by = 0, cy = 0, ky = 0, bz[V], cz[V], kz[V];
+  if (xs) {
+    qx = psi_index(d, 0, i, j, k0);
+    p_hy_x = ldv<V>(d.psiH[1][1] + qx);
+    p_hz_x = ldv<V>(d.psiH[2][0] + qx);
+    bx = __ldg(d.tab[0][3] + i); cx = __ldg(d.tab[0][4] + i); kx = __ldg(d.tab[0][5] + i);
+  }
+  if (ys) {
+    qy = psi_index(d, 1, i, j, k0);
+    p_hx_y = ldv<V>(d.psiH[0][0] + qy);
+    p_hz_y = ldv<V>(d.psiH[2][1] + qy);
+    by = __ldg(d.tab[1][3] + j); cy = __ldg(d.tab[1][4] + j); ky = __ldg(d.tab[1][5] + j);
+  }
+  if (zs) {
+    qz = psi_index(d, 2, i, j, k0);
+    p_hx_z = ldv<V>(d.psiH[0][1] + qz);
+    p_hy_z = ldv<V>(d.psiH[1][0] + qz);
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-      const float ey_zq = v == V - 1 ? ey_zp : ey.v[v < V - 1 ? v + 1 : v];
-      const float ex_zq = v == V - 1 ? ex_zp : ex.v[v < V - 1 ? v + 1 : v];
-      // Hx: a1 = y (d_y^+ Ez), a2 = z (d_z^+ Ey)
-      hx.v[v] = yee_update(hx.v[v], mS, ez_yp.v[v] - ez.v[v], ey_zq - ey.v[v], ys, by, cy, ky, p_hx_y.v[v], zs[v],
-                           bz[v], cz[v], kz[v], p_hx_z.v[v]);
-      // Hy: a1 = z (d_z^+ Ex), a2 = x (d_x^+ Ez)
-      hy.v[v] = yee_update(hy.v[v], mS, ex_zq - ex.v[v], ez_xp.v[v] - ez.v[v], zs[v], bz[v], cz[v], kz[v],
-                           p_hy_z.v[v], xs, bx, cx, kx, p_hy_x.v[v]);
-      // Hz: a1 = x (d_x^+ Ey), a2 = y (d_y^+ Ex)
-      hz.v[v] = yee_update(hz.v[v], mS, ey_xp.v[v] - ey.v[v], ex_yp.v[v] - ex.v[v], xs, bx, cx, kx, p_hz_x.v[v], ys,
-                           by, cy, ky, p_hz_y.v[v]);
+      bz[v] = __ldg(d.tab[2][3] + k0 + v); cz[v] = __ldg(d.tab[2][4] + k0 + v); kz[v] = __ldg(d.tab[2][5] + k0 + v);
     }
-    stv<V>(d.H[0] + q, hx);
-    stv<V>(d.H[1] + q, hy);
-    stv<V>(d.H[2] + q, hz);
-    if (xs) {
-      stv<V>(d.psiH[1][1] + qx, p_hy_x);
-      stv<V>(d.psiH[2][0] + qx, p_hz_x);
-    }
-    if (ys) {
-      stv<V>(d.psiH[0][0] + qy, p_hx_y);
-      stv<V>(d.psiH[2][1] + qy, p_hz_y);
-    }
-    if (zs[0]) {
-      stv<V>(d.psiH[0][1] + qz, p_hx_z);
-      stv<V>(d.psiH[1][0] + qz, p_hy_z);
-    }
+  }
+  float dy_ez[V], dz_ey[V], dz_ex[V], dx_ez[V], dx_ey[V], dy_ex[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) {
+    const float ey_zq = v == V - 1 ? ey_zp : ey.v[v < V - 1 ? v + 1 : v];
+    const float ex_zq = v == V - 1 ? ex_zp : ex.v[v < V - 1 ? v + 1 : v];
+    dy_ez[v] = ez_yp.v[v] - ez.v[v];
+    dz_ey[v] = ey_zq - ey.v[v];
+    dz_ex[v] = ex_zq - ex.v[v];
+    dx_ez[v] = ez_xp.v[v] - ez.v[v];
+    dx_ey[v] = ey_xp.v[v] - ey.v[v];
+    dy_ex[v] = ex_yp.v[v] - ex.v[v];
+  }
+  VF<V> mS;
+#pragma unroll
+  for (int v = 0; v < V; ++v) mS.v[v] = -d.S;
+  // Hx: a1 = y (d_y^+ Ez), a2 = z (d_z^+ Ey)
+#pragma unroll
+  for (int v = 0; v < V; ++v) hx.v[v] = fmaf(mS.v[v], dy_ez[v] - dz_ey[v], hx.v[v]);
+  if (ys) cpml_term<V, false>(hx, p_hx_y, mS, 1.0f, dy_ez, &by, &cy, &ky);
+  if (zs) cpml_term<V, true>(hx, p_hx_z, mS, -1.0f, dz_ey, bz, cz, kz);
+  // Hy: a1 = z (d_z^+ Ex), a2 = x (d_x^+ Ez)
+#pragma unroll
+  for (int v = 0; v < V; ++v) hy.v[v] = fmaf(mS.v[v], dz_ex[v] - dx_ez[v], hy.v[v]);
+  if (zs) cpml_term<V, true>(hy, p_hy_z, mS, 1.0f, dz_ex, bz, cz, kz);
+  if (xs) cpml_term<V, false>(hy, p_hy_x, mS, -1.0f, dx_ez, &bx, &cx, &kx);
+  // Hz: a1 = x (d_x^+ Ey), a2 = y (d_y^+ Ex)
+#pragma unroll
+  for (int v = 0; v < V; ++v) hz.v[v] = fmaf(mS.v[v], dx_ey[v] - dy_ex[v], hz.v[v]);
+  if (xs) cpml_term<V, false>(hz, p_hz_x, mS, 1.0f, dx_ey, &bx, &cx, &kx);
+  if (ys) cpml_term<V, false>(hz, p_hz_y, mS, -1.0f, dy_ex, &by, &cy, &ky);
+  stv<V>(d.H[0] + q, hx);
+  stv<V>(d.H[1] + q, hy);
+  stv<V>(d.H[2] + q, hz);
+  if (xs) {
+    stv<V>(d.psiH[1][1] + qx, p_hy_x);
+    stv<V>(d.psiH[2][0] + qx, p_hz_x);
+  }
+  if (ys) {
+    stv<V>(d.psiH[0][0] + qy, p_hx_y);
+    stv<V>(d.psiH[2][1] + qy, p_hz_y);
+  }
+  if (zs) {
+    stv<V>(d.psiH[0][1] + qz, p_hx_z);
+    stv<V>(d.psiH[1][0] + qz, p_hy_z);
   }
 }
 

@@ -270,7 +270,7 @@ struct SrcDev {
 
 // E_comp += sign * (amp * wave[m-1]) on each source box; blockIdx.y = source (R8)
 __global__ void k_sources(const __grid_constant__ Dev d, const SrcDev* __restrict__ src, const float* __restrict__ waves,
-                          int m_base, const int* step_dev, float sign) {
+                          int m_base, const int* step_dev, float sign, int x0, int x1) {
   const SrcDev s = src[blockIdx.y];
   const int ey = s.hi[1] - s.lo[1], ez = s.hi[2] - s.lo[2];
   const long long cells = (long long)(s.hi[0] - s.lo[0]) * ey * ez;
@@ -278,6 +278,7 @@ __global__ void k_sources(const __grid_constant__ Dev d, const SrcDev* __restric
   const float w = waves[s.wave_off + m - 1];
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < cells; t += (long long)gridDim.x * blockDim.x) {
     const int kk = (int)(t % ez), jj = (int)((t / ez) % ey), ii = (int)(t / ((long long)ez * ey));
+    if (s.lo[0] + ii < x0 || s.lo[0] + ii >= x1) continue;   // x clip (chunked launches)
     const float amp = s.amp ? s.amp[t] : 1.0f;
     const float v = amp * w;
     atomicAdd(&d.E[s.comp][((long long)(s.lo[0] + ii) * d.n[1] + (s.lo[1] + jj)) * d.n[2] + (s.lo[2] + kk)], sign * v);
