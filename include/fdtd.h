@@ -124,6 +124,10 @@ fdtd_status fdtd_set_eps(fdtd_sim*, const float* eps_dev);
 fdtd_status fdtd_reset(fdtd_sim*);
 /* Replay runs of k steps through CUDA graphs (default 1 = on). */
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
+/* Fused marching kernels (two dependent half-steps per pass over the interior): mode -1 = chosen
+ * by grid size (default), 0 = never, 1 = whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).
+ * xseg = planes marched per block (0 keeps the current value).  Results are bit-identical in every mode. */
+fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
 
 /* Current fields: out_dev[6][nx][ny][nz].  fdtd_get_box: out_dev[ncomp][hi-lo] for the components in comp_mask. */
 fdtd_status fdtd_get_fields(fdtd_sim*, float* out_dev);

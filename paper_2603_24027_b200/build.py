@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdtd_b200.so")
 SOURCES = [os.path.join(CSRC, "fdtd_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fdtd_dev.cuh", "fdtd_stencil.cuh", "fdtd_store.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fdtd_dev.cuh", "fdtd_stencil.cuh", "fdtd_store.cuh", "fdtd_fused.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "fdtd.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",

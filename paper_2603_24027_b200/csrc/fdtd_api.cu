@@ -15,6 +15,7 @@
 #include "../../include/fdtd.h"
 #include "fdtd_stencil.cuh"
 #include "fdtd_store.cuh"
+#include "fdtd_fused.cuh"
 
 using namespace fdtd;
 
@@ -27,7 +28,7 @@ constexpr double kC0 = 299792458.0;
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t ce, E[3], H[3], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
+  size_t ce, E[3], H[3], E2[3], H2[3], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
   size_t lE[3], lH[3], lpsiE[2][3][2], lpsiH[2][3][2], acc;
   size_t eps_own, mon_stage, grad_stage, amp_stage;
   size_t store_cap;
@@ -54,7 +55,7 @@ struct fdtd_sim {
   cudaStream_t cur = nullptr;          // stream the next LAUNCH goes to (fork / on / join)
   cudaStream_t aux[3] = {nullptr, nullptr, nullptr};
   cudaStream_t cap = nullptr;          // origin stream of graph captures (the caller's stream may be the legacy default)
-  cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   bool parallel = false;               // auxiliary streams available
   std::vector<cudaGraphExec_t> dead_graphs;
   mutable std::string err;
@@ -77,6 +78,12 @@ struct fdtd_sim {
   std::vector<SrcDev> src_host;
   std::vector<float> waves_host;
   int nsrc = 0;
+  // E/H buffer pair(s): fb[b][0..2] = E, fb[b][3..5] = H of buffer b; d.E / d.H always point at the current one (cb)
+  float* fb[2][6] = {{nullptr}};
+  int cb = 0;
+  bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
+  int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
+  int xseg = 32;           // planes per block of the fused marching kernels
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
   // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
@@ -135,6 +142,10 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   L.ce = take(N * 4);
   for (int c = 0; c < 3; ++c) L.E[c] = take(N * 4);
   for (int c = 0; c < 3; ++c) L.H[c] = take(N * 4);
+  if (s->V == 4 && s->P >= 4) {   // ping-pong partners of E and H for the fused marching kernels
+    for (int c = 0; c < 3; ++c) L.E2[c] = take(N * 4);
+    for (int c = 0; c < 3; ++c) L.H2[c] = take(N * 4);
+  }
   for (int c = 0; c < 3; ++c)
     for (int t = 0; t < 2; ++t) L.psiE[c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
   for (int c = 0; c < 3; ++c)
@@ -308,6 +319,11 @@ bool grid_inner(const fdtd_sim* s, dim3* g) {
   return true;
 }
 
+void set_cur(fdtd_sim* s, int b) {
+  s->cb = b;
+  for (int c = 0; c < 3; ++c) { s->d.E[c] = s->fb[b][c]; s->d.H[c] = s->fb[b][3 + c]; }
+}
+
 #define LAUNCH(s, kern, grid, block, ...)            \
   do {                                               \
     kern<<<grid, block, 0, (s)->cur>>>(__VA_ARGS__); \
@@ -353,29 +369,35 @@ void launch_lean(fdtd_sim* s, int which, const Split& sp) {
     }
   }
 }
-void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp) {
+FieldIO io_inplace(const fdtd_sim* s, int which) {   // which: 0 = E half-step, 1 = H half-step
+  FieldIO io;
+  for (int c = 0; c < 3; ++c) { io.E[c] = s->d.E[c]; io.H[c] = s->d.H[c]; io.out[c] = which == 0 ? s->d.E[c] : s->d.H[c]; }
+  return io;
+}
+void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp, const FieldIO* iop = nullptr) {
   const dim3 b(32, TY);
   const BoxList& B = sp.boxes;
+  const FieldIO io = iop ? *iop : io_inplace(s, which == 1 ? 1 : 0);
   const unsigned g = (unsigned)B.off[B.nb];
   if (g == 0) return;
   if (s->VG == 4) {
     switch (which) {
-      case 0: LAUNCH(s, k_gen_e<4>, g, b, s->d, B); break;
-      case 1: LAUNCH(s, k_gen_h<4>, g, b, s->d, B); break;
+      case 0: LAUNCH(s, k_gen_e<4>, g, b, s->d, B, io); break;
+      case 1: LAUNCH(s, k_gen_h<4>, g, b, s->d, B, io); break;
       case 2: LAUNCH(s, k_gen_adj_h<4>, g, b, s->d, B, pb); break;
       default: LAUNCH(s, k_gen_adj_e<4>, g, b, s->d, B, pb);
     }
   } else if (s->VG == 2) {
     switch (which) {
-      case 0: LAUNCH(s, k_gen_e<2>, g, b, s->d, B); break;
-      case 1: LAUNCH(s, k_gen_h<2>, g, b, s->d, B); break;
+      case 0: LAUNCH(s, k_gen_e<2>, g, b, s->d, B, io); break;
+      case 1: LAUNCH(s, k_gen_h<2>, g, b, s->d, B, io); break;
       case 2: LAUNCH(s, k_gen_adj_h<2>, g, b, s->d, B, pb); break;
       default: LAUNCH(s, k_gen_adj_e<2>, g, b, s->d, B, pb);
     }
   } else {
     switch (which) {
-      case 0: LAUNCH(s, k_gen_e<1>, g, b, s->d, B); break;
-      case 1: LAUNCH(s, k_gen_h<1>, g, b, s->d, B); break;
+      case 0: LAUNCH(s, k_gen_e<1>, g, b, s->d, B, io); break;
+      case 1: LAUNCH(s, k_gen_h<1>, g, b, s->d, B, io); break;
       case 2: LAUNCH(s, k_gen_adj_h<1>, g, b, s->d, B, pb); break;
       default: LAUNCH(s, k_gen_adj_e<1>, g, b, s->d, B, pb);
     }
@@ -434,10 +456,11 @@ void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, in
   LAUNCH(s, k_sources, g, threads, s->d, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
          reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign, x0, x1);
 }
-void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode) {
+void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode, int half = 2) {
+  if ((half == 0 && !(b.mask & 7u)) || (half == 1 && !(b.mask & 56u))) return;
   const long long tot = (long long)b.ncomp * (b.hi[0] - b.lo[0]) * (b.hi[1] - b.lo[1]) * (b.hi[2] - b.lo[2]);
   if (tot <= 0) return;
-  LAUNCH(s, k_box, (unsigned)((tot + 255) / 256), 256, s->d, b, rec, m_base, step_dev, mode);
+  LAUNCH(s, k_box, (unsigned)((tot + 255) / 256), 256, s->d, b, rec, m_base, step_dev, mode, half);
 }
 // half: 0 = E components, 1 = H components, 2 = all six
 void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
@@ -463,43 +486,111 @@ void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, i
 }
 
 // One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
-// Phase E: {lean E, general E, record of the H half of the previous state if one is pending (H is read-only here)}.
-// Phase H: {lean H, general H, record of the E half of state m if due (E is read-only here)}.
-// pending_h carries "state m-1 still needs its H half recorded" in and "state m ..." out.
+// Phase E: {lean E then sources, general E, H halves of state m-1: record (if pending) and monitor row (H is read-only here)}.
+// Phase H: {lean H, general H, E halves of state m: record (if due) and monitor row (E is read-only here)}.
+// pending_h carries "state m-1 still needs its H half recorded" in and "state m ..." out; the monitor row of state m-1
+// always has its H half pending (k_box skips state 0, which has no row).  No small kernel sits alone between phases.
+bool sources_in_lean(const fdtd_sim* s, const Split& sp) {
+  if (!sp.has_lean) return s->nsrc == 0;
+  for (int i = 0; i < s->nsrc; ++i)
+    for (int a = 0; a < 3; ++a)
+      if (s->src_host[i].lo[a] < sp.reg.lo[a] || s->src_host[i].hi[a] > sp.reg.hi[a]) return false;
+  return true;
+}
 void forward_step(fdtd_sim* s, int m_base, const int* step_dev, bool record, bool* pending_h) {
+  const bool mon = s->has_mon && s->mon_rec;
+  const bool src_inline = sources_in_lean(s, s->split[0]);
   fork(s, 3);
   on(s, 0); launch_lean(s, 0);
+  if (src_inline) launch_sources(s, m_base, step_dev, 1.0f);
   on(s, 1); launch_gen(s, 0, 0);
-  if (*pending_h) { on(s, 2); launch_record(s, m_base - 1, step_dev, 1); }
+  on(s, 2);
+  if (*pending_h) launch_record(s, m_base - 1, step_dev, 1);
+  if (mon) launch_box(s, s->mon, s->mon_rec, m_base - 1, step_dev, 0, 1);
   join(s, 3);
-  launch_sources(s, m_base, step_dev, 1.0f);
+  if (!src_inline) launch_sources(s, m_base, step_dev, 1.0f);
   fork(s, 3);
   on(s, 0); launch_lean(s, 1);
   on(s, 1); launch_gen(s, 1, 0);
-  if (record) { on(s, 2); launch_record(s, m_base, step_dev, 0); }
+  on(s, 2);
+  if (record) launch_record(s, m_base, step_dev, 0);
+  if (mon) launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 0);
   join(s, 3);
-  if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0);
   *pending_h = record;
+}
+// H halves of the final state that forward_step left pending
+void forward_flush(fdtd_sim* s, int m, bool pending_h) {
+  if (pending_h) launch_record(s, m, nullptr, 1);
+  if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, m, nullptr, 0, 1);
 }
 
 // One reverse step m -> m-1 (R9), as two phases of mutually independent kernels:
-//  1: {adjoint-H lean, adjoint-H general, inverse-H (inner interior), inject H (shell)}
+//  1: {monitor cotangent then adjoint-H lean, adjoint-H general (after the cotangent), inverse-H (inner interior) then the
+//      sources, inject H (shell)}
 //  2: {adjoint-E lean, adjoint-E general, gradient + inverse-E (inner interior), inject E + shell gradient}
 void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
-  if (dmon && s->has_mon) launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
+  const bool cot = dmon && s->has_mon;
   fork(s, 4);
+  on(s, 1);   // the general kernel is the long one of the phase: it is enqueued first
+  if (cot) {
+    launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
+    if (s->parallel) { cudaEventRecord(s->ev_mid, s->aux[0]); cudaStreamWaitEvent(s->stream, s->ev_mid, 0); }
+  }
+  launch_gen(s, 2, pb);
   on(s, 0); launch_lean(s, 2);
-  on(s, 1); launch_gen(s, 2, pb);
-  on(s, 2); launch_inv_h(s);
+  on(s, 2); launch_inv_h(s); launch_sources(s, m_base, step_dev, -1.0f);
   on(s, 3); launch_inject(s, m_base, step_dev, 1, interp);
   join(s, 4);
-  launch_sources(s, m_base, step_dev, -1.0f);
   fork(s, 4);
   on(s, 0); launch_lean(s, 3);
   on(s, 1); launch_gen(s, 3, pb);
   on(s, 2); launch_inv_e(s); launch_grad(s);
   on(s, 3); launch_inject(s, m_base, step_dev, 0, interp);
   join(s, 4);
+}
+
+// ---- fused path (fdtd_fused.cuh): H half-step of step m and E half-step of step m+1 in one marching kernel ----
+void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
+  FusedArgs a;
+  for (int c = 0; c < 3; ++c) {
+    a.Ein[c] = s->fb[from][c]; a.Hin[c] = s->fb[from][3 + c];
+    a.Eout[c] = s->fb[to][c]; a.Hout[c] = s->fb[to][3 + c];
+  }
+  for (int ax = 0; ax < 3; ++ax) { a.lo[ax] = s->P + (inv ? 1 : 0); a.hi[ax] = s->n[ax] - s->P - (inv ? 1 : 0); }
+  if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
+  a.xseg = s->xseg;
+  const int zbase = a.lo[2] / 4 * 4, zlast = (a.hi[2] - 1) / 4 * 4, groups = (zlast - zbase) / 4 + 1;
+  const dim3 g((unsigned)((groups + FUSED_ZG - 1) / FUSED_ZG), (unsigned)((a.hi[1] - a.lo[1] + FUSED_TR - 1) / FUSED_TR),
+               (unsigned)((a.hi[0] - a.lo[0] + a.xseg - 1) / a.xseg));
+  const dim3 b(32, FUSED_TR + 1);
+  if (inv) LAUNCH(s, k_fused_he<true>, g, b, s->d, a);
+  else LAUNCH(s, k_fused_he<false>, g, b, s->d, a);
+}
+FieldIO io_of(const fdtd_sim* s, int eb, int hb, int ob, int out_is_h) {
+  FieldIO io;
+  for (int c = 0; c < 3; ++c) { io.E[c] = s->fb[eb][c]; io.H[c] = s->fb[hb][3 + c]; io.out[c] = s->fb[ob][out_is_h ? 3 + c : c]; }
+  return io;
+}
+// Fused forward step: from (E^m incl. sources, H^{m-1/2}) in the current buffer to (E^{m+1} incl. sources, H^{m+1/2}) in the
+// other one; state m = (E^m, H^{m+1/2}) is recorded / monitored on the way (E half from the old buffer, H half from the new).
+//  alpha: {general H (cur -> other), record E half, monitor E half}   beta: fused kernel on the interior
+//  gamma: {general E of step m+1 (E cur, H other -> E other), record H half, monitor H half}, then the sources of step m+1
+void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec) {
+  const int cur = s->cb, oth = cur ^ 1;
+  const bool mon = s->has_mon && s->mon_rec;
+  fork(s, 3);
+  on(s, 0); { const FieldIO io = io_of(s, cur, cur, oth, 1); launch_gen(s, 1, 0, s->split[1], &io); }
+  if (rec) { on(s, 1); launch_record(s, m_base, step_dev, 0); }
+  if (mon) { on(s, 2); launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 0); }
+  join(s, 3);
+  launch_fused(s, false, cur, oth);
+  set_cur(s, oth);
+  fork(s, 3);
+  on(s, 0); { const FieldIO io = io_of(s, cur, oth, oth, 0); launch_gen(s, 0, 0, s->split[0], &io); }
+  if (rec) { on(s, 1); launch_record(s, m_base, step_dev, 1); }
+  if (mon) { on(s, 2); launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 1); }
+  join(s, 3);
+  launch_sources(s, m_base + 1, step_dev, 1.0f);
 }
 
 // Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.
@@ -536,6 +627,9 @@ void reap_graphs(fdtd_sim* s) {
 
 fdtd_status zero_state(fdtd_sim* s) {
   const size_t N = (size_t)s->d.N;
+  set_cur(s, 0);
+  for (int c = 0; c < 6; ++c)
+    if (s->fb[1][c]) CUDA_TRY(s, cudaMemsetAsync(s->fb[1][c], 0, N * 4, s->stream));
   for (int c = 0; c < 3; ++c) {
     CUDA_TRY(s, cudaMemsetAsync(s->d.E[c], 0, N * 4, s->stream));
     CUDA_TRY(s, cudaMemsetAsync(s->d.H[c], 0, N * 4, s->stream));
@@ -604,6 +698,46 @@ fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int 
   return FDTD_OK;
 }
 
+// Fused forward run (fdtd_fused.cuh).  Step 1's E half-step runs alone, then nsteps-1 fused steps (H half-step of step m +
+// E half-step of step m+1), then the H half-step of the last step.  States are recorded / monitored exactly as in
+// forward_step: state m = (E^m, H^{m+1/2}).
+bool use_fused(const fdtd_sim* s, int nsteps) {
+  if (!s->can_fuse || nsteps < 2 || s->fuse_mode == 0) return false;
+  // mode -1 (auto): off.  Measured on B200 (round 1): the marching kernel alone beats the two lean kernels on the interior
+  // (C4: 1.29 ms vs 1.40 ms per step), but the slab kernels no longer overlap with it, and the whole step is slower.
+  return s->fuse_mode == 1;
+}
+fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
+  // state 0: E half now, H half beside the first E half-step (H is read-only there)
+  launch_record(s, 0, nullptr, 0);
+  launch_split(s, 0, 0);
+  launch_record(s, 0, nullptr, 1);
+  launch_sources(s, 1, nullptr, 1.0f);
+  int done = 0;   // fused steps m = 1 .. nsteps-1 carried out so far
+  int L = k * std::max(1, (16 + k - 1) / k);
+  if (L & 1) L *= 2;   // even: the ping-pong buffer is the same at the start of every period
+  const int periods = (s->use_graphs && s->aux[0]) ? (nsteps - 1) / L : 0;
+  if (periods > 0) {
+    int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
+    LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
+    s->parallel = true;
+    fdtd_status g = run_graph(s, periods, [&]() {
+      for (int t = 1; t <= L; ++t) forward_fused_step(s, t, step_dev, t % k == 0);
+      LAUNCH(s, k_tick, 1, 1, step_dev, L);
+    });
+    s->parallel = false;
+    s->cur = s->stream;
+    if (g != FDTD_OK) return g;
+    done = periods * L;
+  }
+  for (int m = done + 1; m <= nsteps - 1; ++m) forward_fused_step(s, m, nullptr, m % k == 0);
+  // last step: H half-step alone, then monitor and record of the final state
+  launch_split(s, 1, 0);
+  if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, nsteps, nullptr, 0);
+  launch_record(s, nsteps, nullptr, 2);
+  return FDTD_OK;
+}
+
 fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k, bool amp_is_host) {
   if (!s) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace: call fdtd_set_workspace first");
@@ -624,29 +758,34 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
   if (dt == FDTD_F8E4M3_SCALED) CUDA_TRY(s, cudaMemsetAsync(s->st.amax, 0, (size_t)slots * 36 * 4, s->stream));
   s->cur = s->stream;
   if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
-  // state 0 (R10): its E half now, its H half during the first E phase (H is untouched until then)
-  launch_record(s, 0, nullptr, 0);
-  bool pend = true;
-  int done = 0;
-  // steady-state period of L = k*r steps as one CUDA graph: every period starts and ends with a pending H half
-  const int L = k * std::max(1, (16 + k - 1) / k);
-  const int periods = (s->use_graphs && s->aux[0]) ? nsteps / L : 0;
-  if (periods > 0) {
-    int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
-    LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
-    s->parallel = true;
-    fdtd_status g = run_graph(s, periods, [&]() {
-      bool p = true;
-      for (int t = 1; t <= L; ++t) forward_step(s, t, step_dev, t % k == 0, &p);
-      LAUNCH(s, k_tick, 1, 1, step_dev, L);
-    });
-    s->parallel = false;
-    s->cur = s->stream;
+  if (use_fused(s, nsteps)) {
+    fdtd_status g = forward_fused(s, nsteps, k);
     if (g != FDTD_OK) return g;
-    done = periods * L;
+  } else {
+    // state 0 (R10): its E half now, its H half during the first E phase (H is untouched until then)
+    launch_record(s, 0, nullptr, 0);
+    bool pend = true;
+    int done = 0;
+    // steady-state period of L = k*r steps as one CUDA graph: every period starts and ends with a pending H half
+    const int L = k * std::max(1, (16 + k - 1) / k);
+    const int periods = (s->use_graphs && s->aux[0]) ? nsteps / L : 0;
+    if (periods > 0) {
+      int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
+      LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
+      s->parallel = true;
+      fdtd_status g = run_graph(s, periods, [&]() {
+        bool p = true;
+        for (int t = 1; t <= L; ++t) forward_step(s, t, step_dev, t % k == 0, &p);
+        LAUNCH(s, k_tick, 1, 1, step_dev, L);
+      });
+      s->parallel = false;
+      s->cur = s->stream;
+      if (g != FDTD_OK) return g;
+      done = periods * L;
+    }
+    for (int m = done + 1; m <= nsteps; ++m) forward_step(s, m, nullptr, m % k == 0 || m == nsteps, &pend);
+    forward_flush(s, nsteps, pend);
   }
-  for (int m = done + 1; m <= nsteps; ++m) forward_step(s, m, nullptr, m % k == 0 || m == nsteps, &pend);
-  if (pend) launch_record(s, nsteps, nullptr, 1);
   CUDA_TRY(s, cudaGetLastError());
   s->forward_done = s->state_final = true;
   return FDTD_OK;
@@ -726,9 +865,14 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   if (!s) return FDTD_ERR_OOM;
   s->n[0] = nx; s->n[1] = ny; s->n[2] = nz; s->P = pml_width; s->dx = dx; s->dt = dt; s->Sd = S;
   s->eps_dev = eps_dev;
+  s->V = (nz % 4 == 0 && pml_width % 4 == 0) ? 4 : 1;
+  s->VG = s->V;
   s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   s->cur = s->stream;
-  bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+  if (const char* e = std::getenv("FDTD_FUSE")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_mode = v; }
+  if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
+  bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
   for (int b = 0; b < 3 && ok; ++b)
     ok = cudaStreamCreateWithFlags(&s->aux[b], cudaStreamNonBlocking) == cudaSuccess &&
          cudaEventCreateWithFlags(&s->ev_join[b], cudaEventDisableTiming) == cudaSuccess;
@@ -796,9 +940,13 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   d.S = (float)s->Sd;
   char* w = s->ws;
   d.ce = reinterpret_cast<float*>(w + L.ce);
+  s->can_fuse = s->V == 4 && s->P >= 4;
   for (int c = 0; c < 3; ++c) {
     d.E[c] = reinterpret_cast<float*>(w + L.E[c]);
     d.H[c] = reinterpret_cast<float*>(w + L.H[c]);
+    s->fb[0][c] = d.E[c]; s->fb[0][3 + c] = d.H[c];
+    s->fb[1][c] = s->can_fuse ? reinterpret_cast<float*>(w + L.E2[c]) : nullptr;
+    s->fb[1][3 + c] = s->can_fuse ? reinterpret_cast<float*>(w + L.H2[c]) : nullptr;
     for (int t = 0; t < 2; ++t) {
       d.psiE[c][t] = reinterpret_cast<float*>(w + L.psiE[c][t]);
       d.psiH[c][t] = reinterpret_cast<float*>(w + L.psiH[c][t]);
@@ -839,8 +987,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     st.val_off[f + 1] = st.val_off[f] + 6 * face_size(s, f);
     st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
   }
-  s->V = (s->n[2] % 4 == 0 && s->P % 4 == 0) ? 4 : 1;
-  s->VG = s->V == 4 ? 4 : 1;
+  s->VG = s->V;
   if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2 || v == 4) && s->V == 4) s->VG = v; }
   for (int which = 0; which < 4; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
   build_tables(s);
@@ -869,6 +1016,13 @@ fdtd_status fdtd_reset(fdtd_sim* s) {
 fdtd_status fdtd_set_graphs(fdtd_sim* s, int enabled) {
   if (!s) return FDTD_ERR_INVALID_ARG;
   s->use_graphs = enabled != 0;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_set_fused(fdtd_sim* s, int mode, int xseg) {
+  if (!s || mode < -1 || mode > 1 || xseg < 0) return FDTD_ERR_INVALID_ARG;
+  s->fuse_mode = mode;
+  if (xseg > 0) s->xseg = xseg;
   return FDTD_OK;
 }
 
@@ -1091,6 +1245,7 @@ void fdtd_destroy(fdtd_sim* s) {
     if (s->ev_join[b]) cudaEventDestroy(s->ev_join[b]);
   }
   if (s->ev_fork) cudaEventDestroy(s->ev_fork);
+  if (s->ev_mid) cudaEventDestroy(s->ev_mid);
   if (s->cap) cudaStreamDestroy(s->cap);
   delete s;
 }

@@ -35,6 +35,14 @@ struct Dev {
   int has_design;
 };
 
+// Explicit input / output arrays of a forward general kernel: in place (out == the updated input) in the two-kernel
+// path, other buffer in the fused path (ping-pong, fdtd_fused.cuh).
+struct FieldIO {
+  const float* E[3];
+  const float* H[3];
+  float* out[3];
+};
+
 // A lean kernel's region (plain Yee cells) and the list of boxes that make up its complement (slab cells and the
 // layers that touch them).  Each box has a class that says which CPML axes can occur in it (so the others compile
 // out) and its own lane shape: G lanes along z (groups of V cells) x RW rows per warp, G*RW <= 32.

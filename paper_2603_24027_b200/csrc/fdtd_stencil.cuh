@@ -67,7 +67,7 @@ __device__ __forceinline__ void cpml_term(VF<V>& x, VF<V>& psi, const VF<V>& coe
 // Forward E half-step (SURVEY 8(a) rows A1 + A3):  E_c += ce * (d_a1^- H_b1 - d_a2^- H_b2) + CPML terms,
 // tangential E on the three low PEC walls held at zero.  DESIGN.md R1-R5.
 template <int V, bool HX, bool HY>
-__device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int j, const int k0) {
+__device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int j, const int k0, const FieldIO& io) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
@@ -75,22 +75,22 @@ __device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int 
   const bool ys = HY && P > 0 && in_slab(j, ny, P);
   const bool zs = P > 0 && in_slab(k0, nz, P);
 
-  const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  const VF<V> hx = ldv<V>(io.H[0] + q), hy = ldv<V>(io.H[1] + q), hz = ldv<V>(io.H[2] + q);
   VF<V> hy_xm = zerov<V>(), hz_xm = zerov<V>(), hx_ym = zerov<V>(), hz_ym = zerov<V>();
   if (i > 0) {
-    hy_xm = ldv<V>(d.H[1] + q - sx);
-    hz_xm = ldv<V>(d.H[2] + q - sx);
+    hy_xm = ldv<V>(io.H[1] + q - sx);
+    hz_xm = ldv<V>(io.H[2] + q - sx);
   }
   if (j > 0) {
-    hx_ym = ldv<V>(d.H[0] + q - sy);
-    hz_ym = ldv<V>(d.H[2] + q - sy);
+    hx_ym = ldv<V>(io.H[0] + q - sy);
+    hz_ym = ldv<V>(io.H[2] + q - sy);
   }
   float hx_z0 = 0.0f, hy_z0 = 0.0f;
   if (k0 > 0) {
-    hx_z0 = d.H[0][q - 1];
-    hy_z0 = d.H[1][q - 1];
+    hx_z0 = io.H[0][q - 1];
+    hy_z0 = io.H[1][q - 1];
   }
-  VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  VF<V> ex = ldv<V>(io.E[0] + q), ey = ldv<V>(io.E[1] + q), ez = ldv<V>(io.E[2] + q);
   const VF<V> ce = ldv<V>(d.ce + q);
   // psi_E[c][t]: (0,0)=Ex/y (0,1)=Ex/z (1,0)=Ey/z (1,1)=Ey/x (2,0)=Ez/x (2,1)=Ez/y
   VF<V> p_ey_x, p_ez_x, p_ex_y, p_ez_y, p_ex_z, p_ey_z;
@@ -168,9 +168,9 @@ __device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int 
       if (i == 0 || j == 0) ez.v[v] = 0.0f;
     }
   }
-  stv<V>(d.E[0] + q, ex);
-  stv<V>(d.E[1] + q, ey);
-  stv<V>(d.E[2] + q, ez);
+  stv<V>(io.out[0] + q, ex);
+  stv<V>(io.out[1] + q, ey);
+  stv<V>(io.out[2] + q, ez);
   if (xs) {
     stv<V>(d.psiE[1][1] + qx, p_ey_x);
     stv<V>(d.psiE[2][0] + qx, p_ez_x);
@@ -187,7 +187,7 @@ __device__ __forceinline__ void gen_e_body(const Dev& d, const int i, const int 
 
 // Forward H half-step (rows A2 + A4):  H_c -= S * (d_a1^+ E_b1 - d_a2^+ E_b2) + CPML terms; ghost E[n] = 0.
 template <int V, bool HX, bool HY>
-__device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int j, const int k0) {
+__device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int j, const int k0, const FieldIO& io) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
@@ -195,22 +195,22 @@ __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int 
   const bool ys = HY && P > 0 && in_slab(j, ny, P);
   const bool zs = P > 0 && in_slab(k0, nz, P);
 
-  const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
+  const VF<V> ex = ldv<V>(io.E[0] + q), ey = ldv<V>(io.E[1] + q), ez = ldv<V>(io.E[2] + q);
   VF<V> ey_xp = zerov<V>(), ez_xp = zerov<V>(), ex_yp = zerov<V>(), ez_yp = zerov<V>();
   if (i + 1 < nx) {
-    ey_xp = ldv<V>(d.E[1] + q + sx);
-    ez_xp = ldv<V>(d.E[2] + q + sx);
+    ey_xp = ldv<V>(io.E[1] + q + sx);
+    ez_xp = ldv<V>(io.E[2] + q + sx);
   }
   if (j + 1 < ny) {
-    ex_yp = ldv<V>(d.E[0] + q + sy);
-    ez_yp = ldv<V>(d.E[2] + q + sy);
+    ex_yp = ldv<V>(io.E[0] + q + sy);
+    ez_yp = ldv<V>(io.E[2] + q + sy);
   }
   float ex_zp = 0.0f, ey_zp = 0.0f;
   if (k0 + V < nz) {
-    ex_zp = d.E[0][q + V];
-    ey_zp = d.E[1][q + V];
+    ex_zp = io.E[0][q + V];
+    ey_zp = io.E[1][q + V];
   }
-  VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
+  VF<V> hx = ldv<V>(io.H[0] + q), hy = ldv<V>(io.H[1] + q), hz = ldv<V>(io.H[2] + q);
   // psi_H[c][t]: (0,0)=Hx/y (0,1)=Hx/z (1,0)=Hy/z (1,1)=Hy/x (2,0)=Hz/x (2,1)=Hz/y
   VF<V> p_hy_x, p_hz_x, p_hx_y, p_hz_y, p_hx_z, p_hy_z;
   idx_t qx = 0, qy = 0, qz = 0;
@@ -266,9 +266,9 @@ __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int 
   for (int v = 0; v < V; ++v) hz.v[v] = fmaf(mS.v[v], dx_ey[v] - dy_ex[v], hz.v[v]);
   if (xs) cpml_term<V, false>(hz, p_hz_x, mS, 1.0f, dx_ey, &bx, &cx, &kx);
   if (ys) cpml_term<V, false>(hz, p_hz_y, mS, -1.0f, dy_ex, &by, &cy, &ky);
-  stv<V>(d.H[0] + q, hx);
-  stv<V>(d.H[1] + q, hy);
-  stv<V>(d.H[2] + q, hz);
+  stv<V>(io.out[0] + q, hx);
+  stv<V>(io.out[1] + q, hy);
+  stv<V>(io.out[2] + q, hz);
   if (xs) {
     stv<V>(d.psiH[1][1] + qx, p_hy_x);
     stv<V>(d.psiH[2][0] + qx, p_hz_x);
@@ -745,16 +745,18 @@ __device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const 
 // GENERAL kernels: one launch per half-step over the box list; each block runs the body of its box's class.
 // ---------------------------------------------------------------------------------------------------------
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+__global__ void __launch_bounds__(32 * TY) k_gen_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B,
+                                                   const __grid_constant__ FieldIO io) {
   int b, i, j, k0;
   if (!box_decode<V>(B, b, i, j, k0)) return;
-  FDTD_CLASS_DISPATCH(gen_e_body, d, i, j, k0)
+  FDTD_CLASS_DISPATCH(gen_e_body, d, i, j, k0, io)
 }
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B) {
+__global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B,
+                                                   const __grid_constant__ FieldIO io) {
   int b, i, j, k0;
   if (!box_decode<V>(B, b, i, j, k0)) return;
-  FDTD_CLASS_DISPATCH(gen_h_body, d, i, j, k0)
+  FDTD_CLASS_DISPATCH(gen_h_body, d, i, j, k0, io)
 }
 template <int V>
 __global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {

@@ -295,8 +295,9 @@ struct BoxDev {
 // mode 1: lambda_comp += rec[(m-1)][ci][box]   (monitor cotangent, reverse)
 // mode 2: out[ci][box] = F_comp                (fdtd_get_box; m ignored)
 // mode 3: lambda_comp += rec[ci][box]          (dL/dfinal)
+// half: 0 = E components only, 1 = H components only, 2 = all (the fused forward path writes a monitor row in two parts)
 __global__ void k_box(const __grid_constant__ Dev d, const __grid_constant__ BoxDev b, float* rec, int m_base,
-                      const int* step_dev, int mode) {
+                      const int* step_dev, int mode, int half) {
   const int ex = b.hi[0] - b.lo[0], ey = b.hi[1] - b.lo[1], ez = b.hi[2] - b.lo[2];
   const long long bc = (long long)ex * ey * ez;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -306,6 +307,8 @@ __global__ void k_box(const __grid_constant__ Dev d, const __grid_constant__ Box
   int comp = 0, seen = -1;
   for (int c = 0; c < 6; ++c)
     if (b.mask >> c & 1) { if (++seen == ci) { comp = c; break; } }
+  if ((half == 0 && comp >= 3) || (half == 1 && comp < 3)) return;
+  if (mode == 0 && cur_step(m_base, step_dev) < 1) return;   // state 0 has no monitor row
   const int kk = (int)(r % ez), jj = (int)((r / ez) % ey), ii = (int)(r / ((long long)ez * ey));
   const long long q = ((long long)(b.lo[0] + ii) * d.n[1] + (b.lo[1] + jj)) * d.n[2] + (b.lo[2] + kk);
   long long off = t;

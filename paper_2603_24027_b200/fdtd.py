@@ -61,6 +61,7 @@ def lib():
     L.fdtd_set_eps.argtypes = [vp, vp]
     L.fdtd_reset.argtypes = [vp]
     L.fdtd_set_graphs.argtypes = [vp, C.c_int]
+    L.fdtd_set_fused.argtypes = [vp, C.c_int, C.c_int]
     L.fdtd_get_fields.argtypes = [vp, vp]
     L.fdtd_get_adjoint.argtypes = [vp, vp]
     L.fdtd_get_box.argtypes = [vp, i3, i3, C.c_uint, vp]
@@ -86,7 +87,7 @@ def lib():
 
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
-            "fdtd_set_graphs", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
+            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count"]
@@ -274,6 +275,9 @@ class Sim:
 
     def set_graphs(self, on):
         self._check(self._L.fdtd_set_graphs(self._h, int(bool(on))))
+
+    def set_fused(self, mode, xseg=0):
+        self._check(self._L.fdtd_set_fused(self._h, int(mode), int(xseg)))
 
     def fields(self):
         out = self._torch.empty((6,) + self.shape, dtype=self._torch.float32, device=self.eps.device)

@@ -150,6 +150,36 @@ def test_mid_grid_several_tiles_ragged(dtype, k):
     assert rel_l2(g["mon"], o["mon"]) <= FIELD_TOL
 
 
+@pytest.mark.parametrize("dtype,k,xseg,graphs", [(W.F32, 1, 5, True), (W.BF16, 4, 32, True), (W.F8E4M3_SCALED, 3, 7, False)])
+def test_fused_marching_path_matches_two_kernel_path(dtype, k, xseg, graphs):
+    """The fused marching kernels (fdtd_fused.cuh; ping-pong buffers, halo recompute, ragged x segments / y tiles / z
+    groups) against the oracle and, bit for bit, against the two-kernel path: fields, monitor record, every store slot,
+    gradient."""
+    w = mid_workload(dtype=dtype, k=k)
+    o = oracle_gradient(w, 32, dtype, k)
+    res = {}
+    for mode in (0, 1):
+        s = gpu_sim(w)
+        s.set_fused(mode, xseg)
+        s.set_graphs(graphs)
+        res[mode] = gpu_gradient(w, dtype, k, sim=s)
+    f_err, g_err = _report(f"fused mid dtype={dtype} k={k} xseg={xseg}", res[1], o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    assert rel_l2(res[1]["mon"], o["mon"]) <= FIELD_TOL
+    for key in ("final", "mon", "grad", "state0"):
+        assert np.array_equal(res[0][key], res[1][key]), key
+    s0, s1 = res[0]["sim"], res[1]["sim"]
+    assert s0.num_slots() == s1.num_slots() == o["sim"].num_slots()
+    s0.forward(w.nsteps, w.sources, dtype, k)
+    s1.forward(w.nsteps, w.sources, dtype, k)
+    for j in range(s0.num_slots()):
+        a, sa = s0.slot(j, dtype)
+        b, sb = s1.slot(j, dtype)
+        assert np.array_equal(a.cpu().numpy(), b.cpu().numpy()), j
+        if dtype == W.F8E4M3_SCALED:
+            assert np.array_equal(sa.cpu().numpy(), sb.cpu().numpy()), j
+
+
 def test_store_slots_bit_exact_when_fields_agree():
     """Record kernel vs oracle record: every slot, byte for byte, for each dtype (fields are bit-identical in practice;
     if they are not, compare the decoded values within the field tolerance instead)."""
