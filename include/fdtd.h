@@ -40,7 +40,17 @@ typedef enum {
 
 /* Storage type of the interface store.  F8E4M3_SCALED = OCP E4M3 ("e4m3fn", max 448) with one
  * float32 absmax scale per (slot, face, component) slice — DESIGN.md R13/R14. */
-typedef enum { FDTD_F32 = 0, FDTD_F16 = 1, FDTD_BF16 = 2, FDTD_F8E4M3_SCALED = 3 } fdtd_dtype;
+typedef enum {
+  FDTD_F32 = 0, FDTD_F16 = 1, FDTD_BF16 = 2, FDTD_F8E4M3_SCALED = 3,
+  /* The paper's own float8 flavours, cast WITHOUT a scale, exactly like an array astype: round to
+   * nearest even, subnormals kept; a value above the largest finite one becomes NaN ("fn"/"fnuz": no infinities) or
+   * inf (e4m3, e3m4).  e4m3b11fnuz with k = 16 is the paper's 64x configuration.  Software casts (no hardware cvt). */
+  FDTD_F8E4M3B11FNUZ = 10, /* bias 11, max 30,    min subnormal 2^-13 */
+  FDTD_F8E5M2FNUZ = 11,    /* bias 16, max 57344, min subnormal 2^-17 */
+  FDTD_F8E4M3FNUZ = 12,    /* bias 8,  max 240,   min subnormal 2^-10 */
+  FDTD_F8E4M3 = 13,        /* IEEE-like, bias 7, max 240,  min subnormal 2^-9 */
+  FDTD_F8E3M4 = 14         /* IEEE-like, bias 3, max 15.5, min subnormal 2^-6 */
+} fdtd_dtype;
 /* Temporal interpolation between stored steps: linear is the paper's; cubic = 4-point Lagrange. */
 typedef enum { FDTD_LINEAR = 0, FDTD_CUBIC = 1 } fdtd_interp;
 

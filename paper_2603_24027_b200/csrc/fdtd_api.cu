@@ -122,7 +122,21 @@ long long slot_values(const fdtd_sim* s) {
   for (int f = 0; f < 6; ++f) v += 6 * face_size(s, f);
   return v;
 }
-int elem_bytes_host(int dt) { return dt == DT_F32 ? 4 : (dt == DT_E4M3S ? 1 : 2); }
+int elem_bytes_host(int dt) { return dt == DT_F32 ? 4 : ((dt == DT_F16 || dt == DT_BF16) ? 2 : 1); }
+bool dtype_ok(int dt) { return (dt >= 0 && dt <= 3) || (dt >= DT_E4M3B11FNUZ && dt <= DT_E3M4); }
+// run STMT with DT bound to the compile-time store dtype
+#define FDTD_DT_SWITCH(dt, STMT)                                                   \
+  switch (dt) {                                                                    \
+    case DT_F32: { constexpr int DT = DT_F32; STMT; } break;                       \
+    case DT_F16: { constexpr int DT = DT_F16; STMT; } break;                       \
+    case DT_BF16: { constexpr int DT = DT_BF16; STMT; } break;                     \
+    case DT_E4M3S: { constexpr int DT = DT_E4M3S; STMT; } break;                   \
+    case DT_E4M3B11FNUZ: { constexpr int DT = DT_E4M3B11FNUZ; STMT; } break;       \
+    case DT_E5M2FNUZ: { constexpr int DT = DT_E5M2FNUZ; STMT; } break;             \
+    case DT_E4M3FNUZ: { constexpr int DT = DT_E4M3FNUZ; STMT; } break;             \
+    case DT_E4M3: { constexpr int DT = DT_E4M3; STMT; } break;                     \
+    default: { constexpr int DT = DT_E3M4; STMT; } break;                          \
+  }
 int num_slots(int nsteps, int k) { return nsteps / k + 1 + (nsteps % k ? 1 : 0); }
 long long psi_elems(const fdtd_sim* s, int a) { return 2LL * s->P * s->n[(a + 1) % 3] * s->n[(a + 2) % 3]; }
 long long design_cells(const fdtd_sim* s) {
@@ -466,23 +480,12 @@ void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int*
 void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
   const long long items = s->st.cell_off[6] * (half == 2 ? 6 : 3);
   const unsigned g = (unsigned)((items + 255) / 256);
-  switch (s->dtype) {
-    case DT_F32: LAUNCH(s, k_record<DT_F32>, g, 256, s->d, s->st, m_base, step_dev, half); break;
-    case DT_F16: LAUNCH(s, k_record<DT_F16>, g, 256, s->d, s->st, m_base, step_dev, half); break;
-    case DT_BF16: LAUNCH(s, k_record<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev, half); break;
-    default:
-      LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
-      LAUNCH(s, k_record<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev, half);
-  }
+  if (s->dtype == DT_E4M3S) LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
+  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_record<DT>, g, 256, s->d, s->st, m_base, step_dev, half))
 }
 void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp) {
   const unsigned g = (unsigned)((s->st.cell_off[6] + 255) / 256);
-  switch (s->dtype) {
-    case DT_F32: LAUNCH(s, k_inject<DT_F32>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
-    case DT_F16: LAUNCH(s, k_inject<DT_F16>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
-    case DT_BF16: LAUNCH(s, k_inject<DT_BF16>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp); break;
-    default: LAUNCH(s, k_inject<DT_E4M3S>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp);
-  }
+  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_inject<DT>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp))
 }
 
 // One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
@@ -743,7 +746,7 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace: call fdtd_set_workspace first");
   if (nsteps < 1) return fail(s, FDTD_ERR_INVALID_ARG, "nsteps must be >= 1");
   if (k < 1) return fail(s, FDTD_ERR_INVALID_ARG, "k must be >= 1");
-  if ((int)dt < 0 || (int)dt > 3) return fail(s, FDTD_ERR_INVALID_ARG, "unknown store dtype %d", (int)dt);
+  if (!dtype_ok((int)dt)) return fail(s, FDTD_ERR_INVALID_ARG, "unknown store dtype %d", (int)dt);
   const int slots = num_slots(nsteps, k);
   const size_t need = (size_t)slots * slot_values(s) * elem_bytes_host(dt);
   if (nsteps > s->max_nsteps || slots > s->L.slots_cap || need > s->L.store_cap)
@@ -917,13 +920,13 @@ fdtd_status fdtd_set_monitor(fdtd_sim* s, const int lo[3], const int hi[3], unsi
 }
 
 size_t fdtd_workspace_bytes(const fdtd_sim* s, int nsteps, fdtd_dtype dt, int k, unsigned flags) {
-  if (!s || nsteps < 1 || k < 1 || (int)dt < 0 || (int)dt > 3) return 0;
+  if (!s || nsteps < 1 || k < 1 || !dtype_ok((int)dt)) return 0;
   return make_layout(s, nsteps, (int)dt, k, flags).total;
 }
 
 fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nsteps, fdtd_dtype dt, int k, unsigned flags) {
   if (!s) return FDTD_ERR_INVALID_ARG;
-  if (!ws_dev || nsteps < 1 || k < 1 || (int)dt < 0 || (int)dt > 3) return fail(s, FDTD_ERR_INVALID_ARG, "bad workspace arguments");
+  if (!ws_dev || nsteps < 1 || k < 1 || !dtype_ok((int)dt)) return fail(s, FDTD_ERR_INVALID_ARG, "bad workspace arguments");
   if (reinterpret_cast<uintptr_t>(ws_dev) % 256) return fail(s, FDTD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   const Layout L = make_layout(s, nsteps, (int)dt, k, flags);
   if (bytes < L.total) return fail(s, FDTD_ERR_OOM, "workspace too small: need %zu bytes, got %zu", L.total, bytes);
@@ -1127,37 +1130,28 @@ fdtd_status fdtd_reverse_host(fdtd_sim* s, const float* dmon_host, fdtd_interp i
 // ---- stand-alone codec ----
 fdtd_status fdtd_codec_encode(fdtd_dtype dt, const float* x_dev, size_t n, void* codes_dev, float* scale_dev,
                               unsigned* scratch_dev, void* cuda_stream) {
-  if (!x_dev || !codes_dev || !scale_dev || (int)dt < 0 || (int)dt > 3) return FDTD_ERR_INVALID_ARG;
+  if (!x_dev || !codes_dev || !scale_dev || !dtype_ok((int)dt)) return FDTD_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
-  switch ((int)dt) {
-    case DT_F32: k_codec_encode<DT_F32><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
-    case DT_F16: k_codec_encode<DT_F16><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
-    case DT_BF16: k_codec_encode<DT_BF16><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, nullptr); break;
-    default:
-      if (!scratch_dev) return FDTD_ERR_INVALID_ARG;
-      if (cudaMemsetAsync(scratch_dev, 0, 4, st) != cudaSuccess) return FDTD_ERR_CUDA;
-      k_codec_amax<<<g, 256, 0, st>>>(x_dev, n, scratch_dev);
-      k_codec_encode<DT_E4M3S><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, scratch_dev);
+  if ((int)dt == DT_E4M3S) {
+    if (!scratch_dev) return FDTD_ERR_INVALID_ARG;
+    if (cudaMemsetAsync(scratch_dev, 0, 4, st) != cudaSuccess) return FDTD_ERR_CUDA;
+    k_codec_amax<<<g, 256, 0, st>>>(x_dev, n, scratch_dev);
   }
+  FDTD_DT_SWITCH((int)dt, (k_codec_encode<DT><<<g, 256, 0, st>>>(x_dev, n, codes_dev, scale_dev, (int)dt == DT_E4M3S ? scratch_dev : nullptr)))
   return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
 }
 
 fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* const codes_dev[4], const float scales[4],
                              int num, int den, size_t n, float* out_dev, void* cuda_stream) {
-  if (!codes_dev || !scales || !out_dev || den < 1 || num < 0 || num >= den || (int)dt < 0 || (int)dt > 3) return FDTD_ERR_INVALID_ARG;
+  if (!codes_dev || !scales || !out_dev || den < 1 || num < 0 || num >= den || !dtype_ok((int)dt)) return FDTD_ERR_INVALID_ARG;
   const int mode = num == 0 ? 0 : ((int)interp == 1 ? 2 : 1);
   if (!codes_dev[1] || (mode >= 1 && !codes_dev[2]) || (mode == 2 && (!codes_dev[0] || !codes_dev[3]))) return FDTD_ERR_INVALID_ARG;
   FetchArgs a;
   for (int j = 0; j < 4; ++j) { a.codes[j] = codes_dev[j]; a.scales[j] = scales[j]; }
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
-  switch ((int)dt) {
-    case DT_F32: k_codec_fetch<DT_F32><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
-    case DT_F16: k_codec_fetch<DT_F16><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
-    case DT_BF16: k_codec_fetch<DT_BF16><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev); break;
-    default: k_codec_fetch<DT_E4M3S><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev);
-  }
+  FDTD_DT_SWITCH((int)dt, (k_codec_fetch<DT><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev)))
   return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
 }
 

@@ -11,7 +11,9 @@
 
 namespace fdtd {
 
-enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3S = 3 };
+// 0..3: BASELINE.json's store types.  10..14: the paper's five unscaled float8 flavours (ids as in fdtd.h).
+enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3S = 3,
+       DT_E4M3B11FNUZ = 10, DT_E5M2FNUZ = 11, DT_E4M3FNUZ = 12, DT_E4M3 = 13, DT_E3M4 = 14 };
 
 // Interface store: slot j = state min(j*k, nsteps); inside a slot
 // [face 0..5][comp 0..5][u][v] in the store dtype; face = 2*axis + side, plane index P (low) / n-P-1 (high),
@@ -28,7 +30,7 @@ struct StoreDev {
   int du[6], dv[6];
 };
 
-__device__ __forceinline__ int elem_bytes(int dt) { return dt == DT_F32 ? 4 : (dt == DT_E4M3S ? 1 : 2); }
+__device__ __forceinline__ int elem_bytes(int dt) { return dt == DT_F32 ? 4 : ((dt == DT_F16 || dt == DT_BF16) ? 2 : 1); }
 
 // ---- value codecs (round-to-nearest-even, subnormals kept) ----
 template <int DT> struct Codec;
@@ -59,6 +61,53 @@ template <> struct Codec<DT_E4M3S> {   // OCP E4M3 (max 448) after a per-slice s
     return __half2float(__half(h)) * scale;
   }
 };
+
+// Software minifloat cast for the paper's unscaled float8 flavours (e4m3b11fnuz, e5m2fnuz, e4m3fnuz, e4m3,
+// e3m4; "f" = finite only, "n" = a NaN code exists, "uz" = no negative zero).  EB exponent bits, MB mantissa bits.
+// Value-level rule (R12): e = max(floor(log2|x|), 1-BIAS), q = 2^(e-MB), result = sign * q * RNE(|x|/q); above the
+// largest finite value IEEE flavours give inf, fn / fnuz flavours NaN (what an XLA / ml_dtypes astype does); fnuz has a
+// single zero (0x00) and a single NaN (0x80).  The hardware has no conversion for these types, so this is integer code.
+enum { FL_IEEE = 0, FL_FN = 1, FL_FNUZ = 2 };
+template <int EB, int MB, int BIAS, int FL>
+struct MiniFloat {
+  typedef unsigned char code_t;
+  static constexpr unsigned EALL = (1u << EB) - 1u, MALL = (1u << MB) - 1u, SIGN = 1u << (EB + MB);
+  static __device__ __forceinline__ float pow2(int k) { return __uint_as_float((unsigned)(127 + k) << 23); }   // k in [-126, 127]
+  static __device__ __forceinline__ code_t enc(float x, float) {
+    const unsigned u = __float_as_uint(x);
+    const unsigned sbit = (u >> 31) ? SIGN : 0u;
+    const unsigned nan_code = FL == FL_FNUZ ? SIGN : (FL == FL_FN ? (sbit | (EALL << MB) | MALL) : (sbit | (EALL << MB) | (1u << (MB - 1))));
+    const unsigned inf_code = FL == FL_IEEE ? (sbit | (EALL << MB)) : nan_code;
+    const unsigned zero_code = FL == FL_FNUZ ? 0u : sbit;
+    const unsigned au = u & 0x7fffffffu;
+    if (au > 0x7f800000u) return (code_t)nan_code;
+    if (au == 0x7f800000u) return (code_t)inf_code;
+    const float a = __uint_as_float(au);
+    int e = (int)(au >> 23) - 127;                 // floor(log2 a) for normal a; f32 subnormals fall below every 1-BIAS
+    e = max(e, 1 - BIAS);
+    int r = (int)rintf(a * pow2(MB - e));          // exact product (power of two), round-to-nearest-even; r <= 2^(MB+1)
+    if (r == (2 << MB)) { r = 1 << MB; ++e; }
+    const int emax = FL == FL_IEEE ? (int)EALL - 1 - BIAS : (int)EALL - BIAS;
+    const int rmax = FL == FL_FN ? (2 << MB) - 2 : (2 << MB) - 1;
+    if (e > emax || (e == emax && r > rmax)) return (code_t)inf_code;
+    if (r == 0) return (code_t)zero_code;
+    if (r < (1 << MB)) return (code_t)(sbit | (unsigned)r);                       // subnormal: exponent field 0
+    return (code_t)(sbit | ((unsigned)(e + BIAS) << MB) | ((unsigned)r - (1u << MB)));
+  }
+  static __device__ __forceinline__ float dec(code_t c, float) {
+    const unsigned sign = (c >> (EB + MB)) & 1u, ef = (c >> MB) & EALL, mf = c & MALL;
+    if (FL == FL_FNUZ && c == SIGN) return __uint_as_float(0x7fc00000u);
+    if (FL == FL_FN && ef == EALL && mf == MALL) return __uint_as_float(0x7fc00000u);
+    if (FL == FL_IEEE && ef == EALL) return mf ? __uint_as_float(0x7fc00000u) : __uint_as_float(sign ? 0xff800000u : 0x7f800000u);
+    const float v = ef == 0 ? (float)mf * pow2(1 - BIAS - MB) : (float)((1u << MB) + mf) * pow2((int)ef - BIAS - MB);
+    return sign ? -v : v;
+  }
+};
+template <> struct Codec<DT_E4M3B11FNUZ> : MiniFloat<4, 3, 11, FL_FNUZ> {};
+template <> struct Codec<DT_E5M2FNUZ> : MiniFloat<5, 2, 16, FL_FNUZ> {};
+template <> struct Codec<DT_E4M3FNUZ> : MiniFloat<4, 3, 8, FL_FNUZ> {};
+template <> struct Codec<DT_E4M3> : MiniFloat<4, 3, 7, FL_IEEE> {};
+template <> struct Codec<DT_E3M4> : MiniFloat<3, 4, 3, FL_IEEE> {};
 
 // ---- temporal interpolation, all in f32 (R11) ----
 __device__ __forceinline__ float lerp_value(float a, float b, int num, int den) {

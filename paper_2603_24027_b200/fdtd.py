@@ -10,11 +10,14 @@ import os
 import numpy as np
 
 F32, F16, BF16, F8E4M3_SCALED = 0, 1, 2, 3
+# the paper's unscaled float8 flavours
+F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14
 LINEAR, CUBIC = 0, 1
 WS_REVERSE, WS_HOST_IO = 1, 2
 STATUS = {0: "FDTD_OK", 1: "FDTD_ERR_INVALID_ARG", 2: "FDTD_ERR_OOM", 3: "FDTD_ERR_CUDA", 4: "FDTD_ERR_STATE",
           5: "FDTD_ERR_UNSUPPORTED"}
-ELEM_BYTES = {F32: 4, F16: 2, BF16: 2, F8E4M3_SCALED: 1}
+ELEM_BYTES = {F32: 4, F16: 2, BF16: 2, F8E4M3_SCALED: 1, F8E4M3B11FNUZ: 1, F8E5M2FNUZ: 1, F8E4M3FNUZ: 1, F8E4M3: 1,
+              F8E3M4: 1}
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libfdtd_b200.so")

@@ -1,7 +1,8 @@
 """Accuracy / memory sweep of the interface store (BASELINE.json configs[4]; the shape of the paper's Fig. 3).
 
 For one workload (default C3, 256x256x128) and a few seeded designs: store dtype in {float32, float16, bfloat16,
-float8_e4m3+scale} x k in {1,2,4,8,16,32} x {linear, cubic}.  Reports, per setting, the store bytes
+float8_e4m3+scale} x k in {1,2,4,8,16,32} x {linear, cubic}; --paper-fp8 adds the paper's five unscaled float8
+flavours (e4m3b11fnuz, e5m2fnuz, e4m3fnuz, e4m3, e3m4).  Reports, per setting, the store bytes
 (fdtd_store_bytes), the paper's compression factor (32/bits)*k, the gradient throughput and the
 cosine similarity (eq. 2) of grad_eps against the (float32, k = 1, linear) gradient of the same design,
 averaged over the designs (PAPER.md:59 averages over 10 gradients).
@@ -11,6 +12,7 @@ averaged over the designs (PAPER.md:59 averages over 10 gradients).
 Everything numerical runs in the CUDA library; this file only loops over settings and forms the cosine.
 """
 import argparse
+import dataclasses
 import json
 import sys
 import time
@@ -24,7 +26,7 @@ def run(args):
     import torch
     from . import fdtd
     base_seed = {"C1": 1001, "C2": 1002, "C3": 1003, "C4": 1004}[args.workload]
-    dtypes = [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED]
+    dtypes = [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED] + (list(W.PAPER_FP8) if args.paper_fp8 else [])
     ks = [int(x) for x in args.k.split(",")]
     interps = [W.LINEAR, W.CUBIC] if args.cubic else [W.LINEAR]
     acc = {}
@@ -33,6 +35,9 @@ def run(args):
         if args.nsteps:
             kw["nsteps"] = args.nsteps
         w = W.BY_NAME[args.workload](**kw)
+        if args.field_scale != 1.0:
+            w = dataclasses.replace(w, sources=[dataclasses.replace(q, wave=(q.wave * args.field_scale).astype(np.float32))
+                                                for q in w.sources])
         eps = torch.from_numpy(w.eps).cuda()
         sim = fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor)
         sim.set_workspace(w.nsteps, W.F32, 1)                  # the largest store of the sweep; reused by every setting
@@ -92,6 +97,9 @@ def main():
     ap.add_argument("--seeds", type=int, default=3)
     ap.add_argument("--k", default="1,2,4,8,16,32")
     ap.add_argument("--no-cubic", dest="cubic", action="store_false")
+    ap.add_argument("--paper-fp8", action="store_true", help="add the paper's five unscaled float8 flavours (PAPER.md:53)")
+    ap.add_argument("--field-scale", type=float, default=1.0,
+                    help="multiply the source amplitude: the unscaled float8 casts depend on the absolute field level")
     ap.add_argument("--out", default="")
     args = ap.parse_args()
     res = run(args)

@@ -99,6 +99,88 @@ def test_dequantise_interpolate_bit_exact(dtype, interp):
         assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (dtype, interp, num, den)
 
 
+# ---- the paper's own unscaled float8 flavours: software casts on the GPU ----
+PAPER_FP8 = [W.F8E4M3B11FNUZ, W.F8E5M2FNUZ, W.F8E4M3FNUZ, W.F8E4M3, W.F8E3M4]
+
+
+@pytest.mark.parametrize("dtype", PAPER_FP8)
+def test_paper_fp8_casts_bit_exact(dtype):
+    """Every code decodes to the oracle's value; every representable value, every midpoint between neighbours (ties to
+    even), values just off the midpoints, overflow (NaN / inf codes), zeros, f32 subnormals and random slices encode to
+    the oracle's code."""
+    import torch
+    fdtd = _fdtd()
+    allc = np.arange(256, dtype=np.uint8)
+    ref = orc.decode(dtype, allc)
+    dummy = torch.from_numpy(allc).cuda()
+    got = fdtd.codec_fetch(dtype, W.LINEAR, [dummy, dummy, dummy, dummy], [1.0] * 4, 0, 4).cpu().numpy()
+    assert np.array_equal(np.isnan(got), np.isnan(ref))
+    ok = ~np.isnan(ref)
+    assert np.array_equal(got[ok].view(np.uint32), ref[ok].view(np.uint32))
+    fin = np.unique(ref[np.isfinite(ref)].astype(np.float64))
+    mids = (fin[:-1] + fin[1:]) / 2
+    mx = float(orc.format_max(dtype))
+    rng = np.random.default_rng(5 + dtype)
+    x = np.concatenate([fin, mids, np.nextafter(mids.astype(np.float32), np.float32(np.inf)),
+                        np.nextafter(mids.astype(np.float32), np.float32(-np.inf)),
+                        [0.0, -0.0, 1e-45, -1e-45, 1e-39, mx, -mx, mx * 1.03, mx * 1.07, -mx * 1.5, 1e30, -3e38, np.inf, -np.inf],
+                        rng.standard_normal(50000) * np.exp(rng.uniform(-14, 5, 50000))]).astype(np.float32)
+    codes, scale = fdtd.codec_encode(dtype, torch.from_numpy(x).cuda())
+    ref_codes, _ = orc.encode(dtype, x)
+    bad = np.nonzero(codes.cpu().numpy() != ref_codes)[0]
+    assert bad.size == 0, (dtype, x[bad[:5]], codes.cpu().numpy()[bad[:5]], ref_codes[bad[:5]])
+    assert scale == 1.0
+
+
+@pytest.mark.parametrize("dtype", PAPER_FP8)
+def test_paper_fp8_dequantise_interpolate_bit_exact(dtype):
+    import torch
+    fdtd = _fdtd()
+    n = 2049
+    xs = [_slice(n, 17 + j, 1e-2) for j in range(4)]
+    enc = [orc.encode(dtype, x) for x in xs]
+    dec = [orc.decode(dtype, c, s) for c, s in enc]
+    assert all(np.isfinite(v).all() for v in dec)
+    codes = [torch.from_numpy(c).cuda() for c, _ in enc]
+    for interp in (W.LINEAR, W.CUBIC):
+        for num, den in [(0, 16), (1, 16), (7, 16), (15, 16), (1, 3)]:
+            got = fdtd.codec_fetch(dtype, interp, codes, [1.0] * 4, num, den).cpu().numpy()
+            if num == 0:
+                ref = dec[1]
+            elif interp == W.LINEAR:
+                ref = np.array([orc.lerp(float(a), float(b), num, den) for a, b in zip(dec[1], dec[2])], dtype=np.float32)
+            else:
+                ref = np.array([orc.cubic(float(a), float(b), float(c), float(d), num, den)
+                                for a, b, c, d in zip(dec[0], dec[1], dec[2], dec[3])], dtype=np.float32)
+            assert np.array_equal(got.view(np.uint32), ref.view(np.uint32)), (dtype, interp, num, den)
+
+
+@pytest.mark.parametrize("dtype,k,scale", [(W.F8E4M3B11FNUZ, 16, 1.0), (W.F8E5M2FNUZ, 4, 1.0), (W.F8E4M3FNUZ, 8, 30.0),
+                                           (W.F8E4M3, 2, 30.0), (W.F8E3M4, 1, 300.0)])
+def test_paper_fp8_end_to_end_parity(dtype, k, scale):
+    """C1 under the paper's storage settings (e4m3b11fnuz, k = 16 is its 64x configuration): fields, every
+    store slot byte for byte, and the gradient against the float32 oracle under the identical setting.  `scale` lifts the
+    source so that the coarser formats are not all-zero (their smallest subnormal is 1e-3 .. 1.6e-2)."""
+    w = W.c1()
+    w = dataclasses.replace(w, sources=[dataclasses.replace(q, wave=(q.wave * scale).astype(np.float32)) for q in w.sources])
+    o = oracle_gradient(w, 32, dtype, k)
+    g = gpu_gradient(w, dtype, k)
+    f_err, g_err = _report(f"C1 paper-fp8 dtype={dtype} k={k}", g, o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    assert g["sim"].store_bytes() == o["sim"].store_bytes()
+    s = g["sim"]
+    s.forward(w.nsteps, w.sources, dtype, k)
+    of = make_oracle(w, 32)
+    of.forward(w.nsteps, dtype, k)
+    nz = 0
+    for j in range(of.num_slots()):
+        data, _ = s.slot(j, dtype)
+        od, _ = of.slot(j, dtype)
+        assert np.array_equal(data.cpu().numpy(), od), (dtype, j)
+        nz += int(np.count_nonzero(od & 0x7f))
+    assert nz > 0
+
+
 # ---------------------------------------------------------------------------------------------------------
 # end-to-end parity
 # ---------------------------------------------------------------------------------------------------------
