@@ -83,11 +83,11 @@ struct fdtd_sim {
   int cb = 0;
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
-  int xseg = 32;           // planes per block of the fused marching kernels
+  int xseg = 16;           // planes per block of the fused marching kernels
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
   // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
-  Split split[4]{};
+  Split split[6]{};   // + 4, 5: the slab kernels' E / H box lists of the fused forward path
 
   // run state
   int nsteps = 0, k = 1, dtype = 0;
@@ -279,7 +279,11 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
       case 0: lo = std::max(P, 1); hi = n - P; break;                 // fwd E: needs the -1 neighbours, no PEC-masked node
       case 1: lo = P; hi = std::min(n - P, n - 1); break;             // fwd H: needs the +1 neighbours
       case 2: lo = P + 1; hi = n - P; break;                          // adj H: the -1 neighbour must not be a slab cell
-      default: lo = P; hi = std::min(n - P - 1, n - 1); break;        // adj E: the +1 neighbour must not be a slab cell
+      case 3: lo = P; hi = std::min(n - P - 1, n - 1); break;         // adj E: the +1 neighbour must not be a slab cell
+      // fused forward path: the marching kernel stores [P+1, n-P); the slab kernels cover the rest plus the plain layers
+      // whose values they hand to each other (fdtd_fused.cuh, forward_fused_step)
+      case 4: lo = P + 1; hi = n - P; break;                          // fused-path E: layer P joins the slab boxes
+      default: lo = P + 1; hi = n - P - 1; break;                     // fused-path H: layers P and n-P-1 join them
     }
     if (a == 2) { lo = (lo + V - 1) / V * V; hi = hi / V * V; }
     full.lo[a] = lo; full.hi[a] = hi;
@@ -559,7 +563,7 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     a.Ein[c] = s->fb[from][c]; a.Hin[c] = s->fb[from][3 + c];
     a.Eout[c] = s->fb[to][c]; a.Hout[c] = s->fb[to][3 + c];
   }
-  for (int ax = 0; ax < 3; ++ax) { a.lo[ax] = s->P + (inv ? 1 : 0); a.hi[ax] = s->n[ax] - s->P - (inv ? 1 : 0); }
+  for (int ax = 0; ax < 3; ++ax) { a.lo[ax] = s->P + 1; a.hi[ax] = s->n[ax] - s->P - (inv ? 1 : 0); }
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
   a.xseg = s->xseg;
   const int zbase = a.lo[2] / 4 * 4, zlast = (a.hi[2] - 1) / 4 * 4, groups = (zlast - zbase) / 4 + 1;
@@ -574,26 +578,33 @@ FieldIO io_of(const fdtd_sim* s, int eb, int hb, int ob, int out_is_h) {
   for (int c = 0; c < 3; ++c) { io.E[c] = s->fb[eb][c]; io.H[c] = s->fb[hb][3 + c]; io.out[c] = s->fb[ob][out_is_h ? 3 + c : c]; }
   return io;
 }
-// Fused forward step: from (E^m incl. sources, H^{m-1/2}) in the current buffer to (E^{m+1} incl. sources, H^{m+1/2}) in the
-// other one; state m = (E^m, H^{m+1/2}) is recorded / monitored on the way (E half from the old buffer, H half from the new).
-//  alpha: {general H (cur -> other), record E half, monitor E half}   beta: fused kernel on the interior
-//  gamma: {general E of step m+1 (E cur, H other -> E other), record H half, monitor H half}, then the sources of step m+1
-void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec) {
+// Fused forward step m (fdtd_fused.cuh): from (E^m incl. sources, H^{m-1/2}) in the current buffer to (E^{m+1}, H^{m+1/2}) in
+// the other one.  Three branches that only READ the current buffer and the slab kernels' own output:
+//   1: slab kernels  H half-step of step m (cur -> other H, boxes of split 5), then E half-step of step m+1
+//      (E cur, H other -> other E, boxes of split 4).  Every H value the second one reads was written by the first one.
+//   0: marching kernel on [P+1, n-P)^3 (cur -> other); its halo cells (index P) are plain cells recomputed from cur.
+//      Where it overlaps the slab boxes (plain layers next to the slabs) both write the same bits.
+//   2: E half of state m (record if due, monitor row) and the pending H half of state m-1, all from the current buffer.
+// Then the buffers swap and the sources of step m+1 are added.
+void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec, bool* pending_h) {
   const int cur = s->cb, oth = cur ^ 1;
   const bool mon = s->has_mon && s->mon_rec;
   fork(s, 3);
-  on(s, 0); { const FieldIO io = io_of(s, cur, cur, oth, 1); launch_gen(s, 1, 0, s->split[1], &io); }
-  if (rec) { on(s, 1); launch_record(s, m_base, step_dev, 0); }
-  if (mon) { on(s, 2); launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 0); }
+  on(s, 1);
+  { const FieldIO io = io_of(s, cur, cur, oth, 1); launch_gen(s, 1, 0, s->split[5], &io); }
+  { const FieldIO io = io_of(s, cur, oth, oth, 0); launch_gen(s, 0, 0, s->split[4], &io); }
+  on(s, 0); launch_fused(s, false, cur, oth);
+  on(s, 2);
+  if (rec) launch_record(s, m_base, step_dev, 0);
+  if (*pending_h) launch_record(s, m_base - 1, step_dev, 1);
+  if (mon) {
+    launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 0);
+    launch_box(s, s->mon, s->mon_rec, m_base - 1, step_dev, 0, 1);
+  }
   join(s, 3);
-  launch_fused(s, false, cur, oth);
   set_cur(s, oth);
-  fork(s, 3);
-  on(s, 0); { const FieldIO io = io_of(s, cur, oth, oth, 0); launch_gen(s, 0, 0, s->split[0], &io); }
-  if (rec) { on(s, 1); launch_record(s, m_base, step_dev, 1); }
-  if (mon) { on(s, 2); launch_box(s, s->mon, s->mon_rec, m_base, step_dev, 0, 1); }
-  join(s, 3);
   launch_sources(s, m_base + 1, step_dev, 1.0f);
+  *pending_h = rec;
 }
 
 // Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.
@@ -706,16 +717,20 @@ fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int 
 // forward_step: state m = (E^m, H^{m+1/2}).
 bool use_fused(const fdtd_sim* s, int nsteps) {
   if (!s->can_fuse || nsteps < 2 || s->fuse_mode == 0) return false;
-  // mode -1 (auto): off.  Measured on B200 (round 1): the marching kernel alone beats the two lean kernels on the interior
-  // (C4: 1.29 ms vs 1.40 ms per step), but the slab kernels no longer overlap with it, and the whole step is slower.
-  return s->fuse_mode == 1;
+  if (s->fuse_mode == 1) return true;
+  // mode -1 (auto): only where the marching kernel has several waves of tiles (3 blocks per SM).  Measured on B200 (round 1):
+  // C4 (512^3, 7200 tiles) forward 1910 -> 1727 us per step; C3 (392 tiles) 159 -> 161; C2 (169 tiles at xseg 8) 35 -> 44.
+  long long tiles = ((s->n[2] - 2 * s->P) / 4 + FUSED_ZG - 1) / FUSED_ZG;
+  tiles *= (s->n[1] - 2 * s->P + FUSED_TR - 1) / FUSED_TR;
+  tiles *= (s->n[0] - 2 * s->P + s->xseg - 1) / s->xseg;
+  return tiles >= 4 * 3 * 148;
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
-  // state 0: E half now, H half beside the first E half-step (H is read-only there)
-  launch_record(s, 0, nullptr, 0);
+  // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
+  launch_record(s, 0, nullptr, 2);
   launch_split(s, 0, 0);
-  launch_record(s, 0, nullptr, 1);
   launch_sources(s, 1, nullptr, 1.0f);
+  bool pend = false;
   int done = 0;   // fused steps m = 1 .. nsteps-1 carried out so far
   int L = k * std::max(1, (16 + k - 1) / k);
   if (L & 1) L *= 2;   // even: the ping-pong buffer is the same at the start of every period
@@ -725,16 +740,19 @@ fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
     LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
     s->parallel = true;
     fdtd_status g = run_graph(s, periods, [&]() {
-      for (int t = 1; t <= L; ++t) forward_fused_step(s, t, step_dev, t % k == 0);
+      bool p = true;   // state 0 (first period: written again, same bytes) or the last state of the previous period
+      for (int t = 1; t <= L; ++t) forward_fused_step(s, t, step_dev, t % k == 0, &p);
       LAUNCH(s, k_tick, 1, 1, step_dev, L);
     });
     s->parallel = false;
     s->cur = s->stream;
     if (g != FDTD_OK) return g;
     done = periods * L;
+    pend = true;
   }
-  for (int m = done + 1; m <= nsteps - 1; ++m) forward_fused_step(s, m, nullptr, m % k == 0);
-  // last step: H half-step alone, then monitor and record of the final state
+  for (int m = done + 1; m <= nsteps - 1; ++m) forward_fused_step(s, m, nullptr, m % k == 0, &pend);
+  // H halves of state nsteps-1 still pending, then the last H half-step alone, then the final state whole
+  forward_flush(s, nsteps - 1, pend);
   launch_split(s, 1, 0);
   if (s->has_mon && s->mon_rec) launch_box(s, s->mon, s->mon_rec, nsteps, nullptr, 0);
   launch_record(s, nsteps, nullptr, 2);
@@ -992,7 +1010,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   }
   s->VG = s->V;
   if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2 || v == 4) && s->V == 4) s->VG = v; }
-  for (int which = 0; which < 4; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
+  for (int which = 0; which < 6; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
   build_tables(s);
   CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
   CUDA_TRY(s, cudaMemsetAsync(w + L.step, 0, 16, s->stream));

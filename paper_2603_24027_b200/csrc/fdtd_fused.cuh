@@ -8,11 +8,16 @@
 // keeping E of the next plane and the new H of the previous plane in registers.  The E update of a cell needs the NEW
 // H of its three low-side neighbours: x from the previous march step, y from the warp below through shared memory,
 // z from the lane below by shuffle.  Warp 0 and lane 0 of a block are halo workers: they recompute the new H of the
-// row / z-group just below the tile and store nothing.  Because neighbouring blocks recompute each other's cells
-// from the OLD fields, input and output are different buffers (ping-pong); cells outside the region (CPML slab cells
-// in the forward run, interface-shell cells in the reverse run) are read from the OUTPUT buffer, where the general /
-// inject kernels of the preceding phase have already put their new H.  Arithmetic is that of the lean kernels
-// (R3), so results are bit-identical to the two-kernel path.
+// row / z-group just below the tile and store nothing; the first march step of a segment does the same for the plane
+// below the segment.  E of the row above (for the H update) also comes through shared memory, written one march step
+// ahead.  Because neighbouring blocks recompute each other's cells from the OLD fields, input and output are different
+// buffers (ping-pong).
+//
+// Forward: the region [lo, hi) starts one cell inside the interior (lo = P + 1), so every halo cell (index P) is a plain
+// cell whose new H follows from the inputs alone: the kernel reads nothing that another kernel of the same step writes
+// and runs beside the slab kernels.  Reverse (INV): the region is the inner interior and the halo cells are interface
+// shell cells, whose H^{m-1/2} the inject kernel has already put into the OUTPUT buffer; they are read from there.
+// Arithmetic is that of the lean kernels (R3), so results are bit-identical to the two-kernel path.
 #pragma once
 #include "fdtd_dev.cuh"
 
@@ -26,13 +31,14 @@ struct FusedArgs {
   const float* Hin[3];
   float* Eout[3];
   float* Hout[3];
-  int lo[3], hi[3];      // region on which both half-steps are applied
+  int lo[3], hi[3];      // region on which both half-steps are applied and stored
   int xseg;              // planes per block along x
 };
 
 template <bool INV>
 __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_constant__ Dev d, const __grid_constant__ FusedArgs a) {
-  __shared__ float4 sh[2][FUSED_TR + 1][32][2];   // new Hx, Hz of the current plane, double-buffered over the march
+  __shared__ float4 shH[2][FUSED_TR + 1][32][2];   // new Hx, Hz of the current plane, double-buffered over the march
+  __shared__ float4 shE[2][FUSED_TR + 1][32][2];   // Ex, Ez of the NEXT plane (read one march step later by the row below)
   const int lane = threadIdx.x, w = threadIdx.y;
   const int ny = d.n[1], nz = d.n[2];
   const int zbase = (a.lo[2] / 4) * 4;            // first stored group of tile 0
@@ -49,7 +55,8 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
 #pragma unroll
   for (int v = 0; v < 4; ++v) zv[v] = k0 + v >= a.lo[2] && k0 + v < a.hi[2];
   const bool zfull = zv[0] && zv[1] && zv[2] && zv[3];
-  const bool low_yz = j < a.lo[1] || !zfull;      // some element takes its new H from the output buffer
+  const bool low_yz = j < a.lo[1] || !zfull;      // INV: some element takes its new H from the output buffer
+  const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];   // the warp above holds row j + 1 (not a clamped copy)
   const idx_t sx = d.sx, sy = d.sy;
   const float cH = INV ? d.S : -d.S;
   idx_t q = ((idx_t)(xs - 1) * ny + j) * nz + k0; // the march starts one plane below the segment (priming)
@@ -61,7 +68,15 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
     // ---- loads: E of the next plane (kept for the next march step), H of this plane, y+1 / z+1 neighbours of E ----
     const VF<4> exn = ldv<4>(a.Ein[0] + q + sx), eyn = ldv<4>(a.Ein[1] + q + sx), ezn = ldv<4>(a.Ein[2] + q + sx);
     VF<4> hx = ldv<4>(a.Hin[0] + q), hy = ldv<4>(a.Hin[1] + q), hz = ldv<4>(a.Hin[2] + q);
-    const VF<4> ex_yp = ldv<4>(a.Ein[0] + q + sy), ez_yp = ldv<4>(a.Ein[2] + q + sy);
+    VF<4> ex_yp, ez_yp;
+    if (yp_smem && i >= xs) {
+      const float4 t0 = shE[buf][w + 1][lane][0], t1 = shE[buf][w + 1][lane][1];
+      ex_yp.v[0] = t0.x; ex_yp.v[1] = t0.y; ex_yp.v[2] = t0.z; ex_yp.v[3] = t0.w;
+      ez_yp.v[0] = t1.x; ez_yp.v[1] = t1.y; ez_yp.v[2] = t1.z; ez_yp.v[3] = t1.w;
+    } else {
+      ex_yp = ldv<4>(a.Ein[0] + q + sy);
+      ez_yp = ldv<4>(a.Ein[2] + q + sy);
+    }
     float ex_zp = __shfl_down_sync(0xffffffffu, ex.v[0], 1), ey_zp = __shfl_down_sync(0xffffffffu, ey.v[0], 1);
     if (lane == 31 || k0raw >= zlast) {           // no lane above holds the next group
       ex_zp = a.Ein[0][q + 4];
@@ -79,20 +94,23 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
       hy.v[v] = fmaf(cH, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
       hz.v[v] = fmaf(cH, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
     }
-    if (low_yz || i < a.lo[0]) {                  // cells outside the region: their new H is already in the output buffer
+    if (INV && (low_yz || i < a.lo[0])) {         // shell cells: their new H is already in the output buffer (inject)
       const VF<4> ox = ldv<4>(a.Hout[0] + q), oy = ldv<4>(a.Hout[1] + q), oz = ldv<4>(a.Hout[2] + q);
       const bool all = j < a.lo[1] || i < a.lo[0];
 #pragma unroll
       for (int v = 0; v < 4; ++v)
         if (all || !zv[v]) { hx.v[v] = ox.v[v]; hy.v[v] = oy.v[v]; hz.v[v] = oz.v[v]; }
     }
-    // ---- hand the new H to the row above (shared memory) and to the lane above (shuffle) ----
-    sh[buf][w][lane][0] = make_float4(hx.v[0], hx.v[1], hx.v[2], hx.v[3]);
-    sh[buf][w][lane][1] = make_float4(hz.v[0], hz.v[1], hz.v[2], hz.v[3]);
+    // ---- hand the new H to the row above (shared memory) and to the lane above (shuffle); E of the next plane to the
+    //      row below for the next march step ----
+    shH[buf][w][lane][0] = make_float4(hx.v[0], hx.v[1], hx.v[2], hx.v[3]);
+    shH[buf][w][lane][1] = make_float4(hz.v[0], hz.v[1], hz.v[2], hz.v[3]);
+    shE[buf ^ 1][w][lane][0] = make_float4(exn.v[0], exn.v[1], exn.v[2], exn.v[3]);
+    shE[buf ^ 1][w][lane][1] = make_float4(ezn.v[0], ezn.v[1], ezn.v[2], ezn.v[3]);
     const float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
     __syncthreads();
     if (store_plane) {
-      const float4 t0 = sh[buf][w - 1][lane][0], t1 = sh[buf][w - 1][lane][1];
+      const float4 t0 = shH[buf][w - 1][lane][0], t1 = shH[buf][w - 1][lane][1];
       const float hx_ym[4] = {t0.x, t0.y, t0.z, t0.w}, hz_ym[4] = {t1.x, t1.y, t1.z, t1.w};
       VF<4> eo;
       VF<4> e1, e2;
