@@ -76,11 +76,13 @@ class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index):
+    def __init__(self, index, period_ms=200):
         self.lines = []
         self.proc = None
+        if period_ms <= 0:
+            return
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", str(int(period_ms)),
                                           "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -173,7 +175,7 @@ def run_gpu(args, rank, world):
     for _ in range(args.warmup):
         one_step(False)
     barrier()
-    sampler = ClockSampler(local) if rank == 0 else None
+    sampler = ClockSampler(local, args.clock_sample_ms) if rank == 0 else None
     l0 = sim.launch_count()
     t0 = time.time()
     tf, tr = [], []
@@ -368,6 +370,7 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=60, help="time steps of the cpu_baseline sample")
     ap.add_argument("--ref-steps", type=int, default=20, help="time steps per bench step of --impl reference")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--clock-sample-ms", type=int, default=200, help="nvidia-smi polling period during the timed region")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", 0))

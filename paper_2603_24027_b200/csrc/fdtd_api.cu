@@ -58,6 +58,7 @@ struct fdtd_sim {
   cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   bool parallel = false;               // auxiliary streams available
   std::vector<cudaGraphExec_t> dead_graphs;
+  cudaGraphExec_t graph_cache[3] = {nullptr, nullptr, nullptr};   // forward, fused forward, reverse
   mutable std::string err;
   const float* eps_dev = nullptr;
   double cpml[4] = {0.8, 1.0, 0.01, 3.0};
@@ -607,12 +608,15 @@ void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec, 
   *pending_h = rec;
 }
 
-// Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.
+// Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.  The
+// instantiated graph of each kind (slot 0 forward, 1 fused forward, 2 reverse) is kept in the handle: the next run
+// re-captures (pointers such as the monitor record may have changed) and patches the kept executable with
+// cudaGraphExecUpdate, which costs far less host time than a new instantiation; only a change of topology (another k,
+// another set of kernels) instantiates anew.
 template <class F>
-fdtd_status run_graph(fdtd_sim* s, int times, F body) {
+fdtd_status run_graph(fdtd_sim* s, int slot, int times, F body) {
   if (times <= 0) return FDTD_OK;
   cudaGraph_t graph = nullptr;
-  cudaGraphExec_t exec = nullptr;
   const unsigned long long before = s->launches;
   cudaStream_t user = s->stream;
   CUDA_TRY(s, cudaStreamBeginCapture(s->cap, cudaStreamCaptureModeThreadLocal));
@@ -622,15 +626,25 @@ fdtd_status run_graph(fdtd_sim* s, int times, F body) {
   cudaError_t e = cudaStreamEndCapture(s->cap, &graph);
   if (e != cudaSuccess || !graph) return fail(s, FDTD_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
   const unsigned long long per = s->launches - before;
-  e = cudaGraphInstantiate(&exec, graph, 0);
+  cudaGraphExec_t& exec = s->graph_cache[slot];
+  if (exec) {
+    cudaGraphExecUpdateResultInfo info;
+    if (cudaGraphExecUpdate(exec, graph, &info) != cudaSuccess) {
+      cudaGetLastError();
+      s->dead_graphs.push_back(exec);   // may still be in flight: destroyed at the next sync point
+      exec = nullptr;
+    }
+  }
+  if (!exec) {
+    e = cudaGraphInstantiate(&exec, graph, 0);
+    if (e != cudaSuccess) { exec = nullptr; cudaGraphDestroy(graph); return fail(s, FDTD_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e)); }
+  }
   cudaGraphDestroy(graph);
-  if (e != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
   for (int r = 0; r < times; ++r) {
     e = cudaGraphLaunch(exec, s->stream);
     if (e != cudaSuccess) break;
   }
   s->launches = before + per * (unsigned long long)times;
-  s->dead_graphs.push_back(exec);   // destroyed at the next sync point (the launches above are still in flight)
   if (e != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "graph launch failed: %s", cudaGetErrorString(e));
   return FDTD_OK;
 }
@@ -739,7 +753,7 @@ fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
     int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
     LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
     s->parallel = true;
-    fdtd_status g = run_graph(s, periods, [&]() {
+    fdtd_status g = run_graph(s, 1, periods, [&]() {
       bool p = true;   // state 0 (first period: written again, same bytes) or the last state of the previous period
       for (int t = 1; t <= L; ++t) forward_fused_step(s, t, step_dev, t % k == 0, &p);
       LAUNCH(s, k_tick, 1, 1, step_dev, L);
@@ -794,7 +808,7 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
       int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
       LAUNCH(s, k_set_int, 1, 1, step_dev, 0);
       s->parallel = true;
-      fdtd_status g = run_graph(s, periods, [&]() {
+      fdtd_status g = run_graph(s, 0, periods, [&]() {
         bool p = true;
         for (int t = 1; t <= L; ++t) forward_step(s, t, step_dev, t % k == 0, &p);
         LAUNCH(s, k_tick, 1, 1, step_dev, L);
@@ -852,7 +866,7 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
       int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
       LAUNCH(s, k_set_int, 1, 1, step_dev, s->nsteps);
       s->parallel = true;
-      fdtd_status g = run_graph(s, periods, [&]() {
+      fdtd_status g = run_graph(s, 2, periods, [&]() {
         for (int t = 0; t < L; ++t) reverse_step(s, -t, step_dev, dmon, (int)interp, t & 1);
         LAUNCH(s, k_tick, 1, 1, step_dev, -L);
       });
@@ -1252,6 +1266,8 @@ void fdtd_destroy(fdtd_sim* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
   reap_graphs(s);
+  for (int g = 0; g < 3; ++g)
+    if (s->graph_cache[g]) cudaGraphExecDestroy(s->graph_cache[g]);
   for (int b = 0; b < 3; ++b) {
     if (s->aux[b]) cudaStreamDestroy(s->aux[b]);
     if (s->ev_join[b]) cudaEventDestroy(s->ev_join[b]);
