@@ -71,6 +71,16 @@ def whole_job_value(cells, nsteps, steps, world, total_ms):
     return float(cells) * nsteps * steps * world / (total_ms * 1e-3) / 1e6
 
 
+# DRAM bytes per launch of a kernel group (read + write, summed over the group's kernels) from the committed ncu --set full
+# captures (profiles/r01c_full.md): what roofline.traffic reports beside the algorithmic bytes.  ncu flushes the caches
+# between launches, so on C2 (working set of the order of the L2) arrays that stay in L2 do not appear as writes.
+NCU_TRAFFIC = {
+    ("C2", "fwd_e"): 88.2e6, ("C2", "fwd_h"): 76.7e6, ("C2", "inv_h"): 32.2e6, ("C2", "adj_h"): 76.6e6,
+    ("C2", "grad_inv_e"): 44.3e6, ("C2", "adj_e"): 88.4e6,
+    ("C4", "fwd_fused"): 6112.8e6, ("C4", "fwd_fused_slabs"): 3242.1e6,
+}
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -234,11 +244,15 @@ def run_gpu(args, rank, world):
     peak, peak_src = load_peaks()
     sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
     nrec = sim.num_slots() - 1
-    counts = {"fwd_e": w.nsteps, "fwd_h": w.nsteps, "inv_h": w.nsteps, "adj_h": w.nsteps, "grad_inv_e": w.nsteps,
-              "adj_e": w.nsteps, "record": nrec + 1, "inject_h": w.nsteps, "inject_e": w.nsteps}
+    fused = sim.uses_fused(w.nsteps)   # large grids: H half-step of step m and E half-step of step m+1 in one marching kernel
+    counts = {"fwd_e": 1 if fused else w.nsteps, "fwd_h": 1 if fused else w.nsteps, "inv_h": w.nsteps, "adj_h": w.nsteps,
+              "grad_inv_e": w.nsteps, "adj_e": w.nsteps, "record": nrec + 1, "inject_h": w.nsteps, "inject_e": w.nsteps,
+              "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1}
     kernels = {}
     for kid, name in enumerate(fdtd.Sim.KERNELS):
-        if kid >= 6:
+        if kid >= 9 and not fused:
+            continue
+        if 6 <= kid <= 8:
             sim.forward(min(w.nsteps, 4 * w.k), w.sources, w.store_dtype, w.k, flags=flags)
         flush.fill_(1)
         ms, by = sim.profile_kernel(kid, warm=3, reps=20)
@@ -249,14 +263,21 @@ def run_gpu(args, rank, world):
         v["frac"] = v["gbs"] / peak
     dom = max(kernels, key=lambda n: kernels[n]["share"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                "frac": kernels[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch (all kernels of the group), ncu --set full, "
+                                  "profiles/r01c_full.md" if (args.workload, dom) in NCU_TRAFFIC else None,
                 "how": "kernel timed alone: 20 back-to-back launches between CUDA events on the library's stream after 3 warm-up "
                        "launches; achieved = algorithmic bytes per launch (DESIGN.md Roofline) / mean launch time",
                 "launch_us": kernels[dom]["us"], "algo_bytes": kernels[dom]["algo_bytes"]}
     # whole-pass effective bandwidth: algorithmic bytes of all stencil launches of one step / measured time
-    algo_fwd = (kernels["fwd_e"]["algo_bytes"] + kernels["fwd_h"]["algo_bytes"]) * w.nsteps + kernels["record"]["algo_bytes"] * (nrec + 1)
+    fwd_names = ("fwd_e", "fwd_h", "fwd_fused", "fwd_fused_slabs")
+    algo_fwd = sum(kernels[n]["algo_bytes"] * kernels[n]["launches_per_step"] for n in fwd_names if n in kernels) \
+        + kernels["record"]["algo_bytes"] * (nrec + 1)
     algo_rev = sum(kernels[n]["algo_bytes"] for n in ("inv_h", "adj_h", "grad_inv_e", "adj_e", "inject_h", "inject_e")) * w.nsteps
     fwd_gbs = algo_fwd / (f_ms / args.steps * 1e-3) / 1e9
+    # the same forward time against the bytes of the two-kernel form (76 B per cell): comparable across paths
+    algo_fwd2 = (kernels["fwd_e"]["algo_bytes"] + kernels["fwd_h"]["algo_bytes"]) * w.nsteps + kernels["record"]["algo_bytes"] * (nrec + 1)
+    fwd2_gbs = algo_fwd2 / (f_ms / args.steps * 1e-3) / 1e9
     rev_gbs = algo_rev / (r_ms / args.steps * 1e-3) / 1e9
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only) ----
@@ -280,7 +301,8 @@ def run_gpu(args, rank, world):
         "store_bytes": sim_store_bytes(sim, w, flags), "store_bytes_per_step": sim_store_bytes(sim, w, flags) / w.nsteps,
         "store_bytes_f32_k1": (w.nsteps + 1) * sim.slot_values() * 4,
         "effective_gbs": {"forward": fwd_gbs, "reverse": rev_gbs, "forward_frac_of_peak": fwd_gbs / peak,
-                          "reverse_frac_of_peak": rev_gbs / peak},
+                          "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused),
+                          "forward_two_kernel_equivalent": fwd2_gbs, "forward_two_kernel_equivalent_frac": fwd2_gbs / peak},
         "roofline": roofline, "kernels": kernels, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         "loss": L0, "grad_abs_max": float(grad.abs().max().item()),
     }

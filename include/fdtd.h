@@ -138,6 +138,8 @@ fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
  * by grid size (default), 0 = never, 1 = whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).
  * xseg = planes marched per block (0 keeps the current value).  Results are bit-identical in every mode. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
+/* 1 if fdtd_forward(nsteps) would take the fused path with the current settings (after fdtd_set_workspace), else 0. */
+int fdtd_uses_fused(const fdtd_sim*, int nsteps);
 
 /* Current fields: out_dev[6][nx][ny][nz].  fdtd_get_box: out_dev[ncomp][hi-lo] for the components in comp_mask. */
 fdtd_status fdtd_get_fields(fdtd_sim*, float* out_dev);
@@ -180,7 +182,8 @@ const char* fdtd_last_error(const fdtd_sim*);
 void fdtd_destroy(fdtd_sim*);
 /* Measurement aid for bench.py's roofline: launch stencil kernel `kernel_id` reps times back to back on the current
  * buffers between two CUDA events (after `warm` untimed launches) and return the mean milliseconds per launch.
- * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e.  Needs a reverse
+ * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e, 9 fused forward
+ * marching kernel, 10 slab kernels of the fused forward path (FDTD_ERR_UNSUPPORTED where the grid cannot fuse).  Needs a reverse
  * workspace and a completed forward for ids >= 2.  The field contents are garbage afterwards: call fdtd_reset.
  * Synchronises.  algo_bytes (may be NULL) receives the algorithmic bytes one launch moves. */
 fdtd_status fdtd_profile_kernel(fdtd_sim*, int kernel_id, int warm, int reps, double* ms_per_launch, double* algo_bytes);

@@ -1061,6 +1061,8 @@ fdtd_status fdtd_set_fused(fdtd_sim* s, int mode, int xseg) {
   return FDTD_OK;
 }
 
+int fdtd_uses_fused(const fdtd_sim* s, int nsteps) { return (s && s->ws && use_fused(s, nsteps)) ? 1 : 0; }
+
 fdtd_status fdtd_forward(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k) {
   return forward_impl(s, nsteps, src, nsrc, dt, k, false);
 }
@@ -1188,10 +1190,11 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* cons
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
-  if (!s || id < 0 || id > 8 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s || id < 0 || id > 10 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
-  if (id >= 6 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
+  if (id >= 6 && id <= 8 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
+  if (id >= 9 && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
   s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
   auto once = [&]() {
@@ -1204,7 +1207,13 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 5: launch_split(s, 3, 0); break;
       case 6: launch_record(s, s->nsteps, nullptr, 2); break;
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
-      default: launch_inject(s, mrev, nullptr, 0, 0); break;
+      case 8: launch_inject(s, mrev, nullptr, 0, 0); break;
+      case 9: launch_fused(s, false, s->cb, s->cb ^ 1); break;
+      default: {
+        const int cur = s->cb, oth = cur ^ 1;
+        { const FieldIO io = io_of(s, cur, cur, oth, 1); launch_gen(s, 1, 0, s->split[5], &io); }
+        { const FieldIO io = io_of(s, cur, oth, oth, 0); launch_gen(s, 0, 0, s->split[4], &io); }
+      }
     }
   };
   cudaEvent_t e0, e1;
@@ -1245,7 +1254,21 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 4: v = 40 * Ninner + 28 * dcells; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
       case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
       case 6: v = (double)s->st.slot_values * (4 + eb); break;
-      default: v = 3 * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+      case 7: case 8: v = 3 * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+      case 9: {   // fused marching kernel: E, H read once and written once, ce read: 52 B per cell of [P+1, n-P)^3
+        double c = 1;
+        for (int a = 0; a < 3; ++a) c *= std::max(0, s->n[a] - 2 * s->P - 1);
+        v = 52 * c;
+        break;
+      }
+      default: {  // slab kernels of the fused path: H half-step on the complement of split 5, E half-step on that of split 4
+        double in5 = 1, in4 = 1;
+        for (int a = 0; a < 3; ++a) {
+          in5 *= std::max(0, s->split[5].reg.hi[a] - s->split[5].reg.lo[a]);
+          in4 *= std::max(0, s->split[4].reg.hi[a] - s->split[4].reg.lo[a]);
+        }
+        v = 36 * (N - in5) + 40 * (N - in4) + 32 * slab;
+      }
     }
     *bytes_out = v;
   }

@@ -65,6 +65,7 @@ def lib():
     L.fdtd_reset.argtypes = [vp]
     L.fdtd_set_graphs.argtypes = [vp, C.c_int]
     L.fdtd_set_fused.argtypes = [vp, C.c_int, C.c_int]
+    L.fdtd_uses_fused.argtypes = [vp, C.c_int]
     L.fdtd_get_fields.argtypes = [vp, vp]
     L.fdtd_get_adjoint.argtypes = [vp, vp]
     L.fdtd_get_box.argtypes = [vp, i3, i3, C.c_uint, vp]
@@ -90,7 +91,7 @@ def lib():
 
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
-            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
+            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_uses_fused", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count"]
@@ -282,6 +283,9 @@ class Sim:
     def set_fused(self, mode, xseg=0):
         self._check(self._L.fdtd_set_fused(self._h, int(mode), int(xseg)))
 
+    def uses_fused(self, nsteps):
+        return bool(self._L.fdtd_uses_fused(self._h, int(nsteps)))
+
     def fields(self):
         out = self._torch.empty((6,) + self.shape, dtype=self._torch.float32, device=self.eps.device)
         self._check(self._L.fdtd_get_fields(self._h, C.c_void_p(out.data_ptr())))
@@ -320,7 +324,8 @@ class Sim:
     def sync(self):
         self._check(self._L.fdtd_sync(self._h))
 
-    KERNELS = ["fwd_e", "fwd_h", "inv_h", "adj_h", "grad_inv_e", "adj_e", "record", "inject_h", "inject_e"]
+    KERNELS = ["fwd_e", "fwd_h", "inv_h", "adj_h", "grad_inv_e", "adj_e", "record", "inject_h", "inject_e",
+               "fwd_fused", "fwd_fused_slabs"]   # the last two: the fused forward path (fdtd_fused.cuh), large grids only
 
     def profile_kernel(self, kernel_id, warm=5, reps=50):
         """(mean ms per launch, algorithmic bytes per launch) of one kernel timed alone, back to back (fdtd_profile_kernel)."""
