@@ -40,7 +40,18 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def make_workload(name, nsteps, seed_offset=0):
+def make_workload(name, nsteps, seed_offset=0, store=None, k=0):
+    w = _make_workload(name, nsteps, seed_offset)
+    if store is not None or k:
+        import dataclasses
+        w = dataclasses.replace(w, store_dtype=w.store_dtype if store is None else store, k=k or w.k)
+    return w
+
+
+STORE_BY_NAME = {v: k for k, v in W.DTYPE_NAMES.items()}
+
+
+def _make_workload(name, nsteps, seed_offset=0):
     f = W.BY_NAME[name]
     kw = {}
     if nsteps:
@@ -137,10 +148,12 @@ def run_gpu(args, rank, world):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
-    w = make_workload(args.workload, args.nsteps, seed_offset=replica_seed_offset(rank))
+    w = make_workload(args.workload, args.nsteps, seed_offset=replica_seed_offset(rank),
+                      store=STORE_BY_NAME[args.store] if args.store else None, k=args.k)
     flags = fdtd.WS_REVERSE | fdtd.WS_HOST_IO
     eps_dev = torch.from_numpy(w.eps).to(dev)
-    sim = fdtd.Sim(eps_dev, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor)
+    sim = fdtd.Sim(eps_dev, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor,
+                   store_mode=fdtd.STORE_TANGENTIAL if args.tangential else fdtd.STORE_ALL)
     sim.set_workspace(w.nsteps, w.store_dtype, w.k, flags)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     extra = {}
@@ -282,7 +295,7 @@ def run_gpu(args, rank, world):
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
-    if world == 1 and not args.no_cpu:
+    if world == 1 and not args.no_cpu and not args.tangential:
         cpu = cpu_baseline(args.workload, args.cpu_steps)
 
     out = {
@@ -292,6 +305,7 @@ def run_gpu(args, rank, world):
         "config": {"workload": f"{w.name}: {w.shape[0]}x{w.shape[1]}x{w.shape[2]} f32 Yee grid, {w.pml}-cell CPML, {w.nsteps} steps, "
                                f"{W.DTYPE_NAMES[w.store_dtype]} store, k={w.k}, linear interpolation, loss={w.loss}",
                    "grid": list(w.shape), "pml": w.pml, "nsteps": w.nsteps, "store_dtype": W.DTYPE_NAMES[w.store_dtype], "k": w.k,
+                   "store_components": "tangential (12 slices per slot)" if args.tangential else "all six per face (36 slices per slot)",
                    "l2": "256 MB write between timed steps flushes L2; inside a step the working set "
                          f"({13 * w.cells * 4 / 1e6:.0f} MB of fields) is what the workload itself keeps resident",
                    "replicas": world, "parallelism": "replicas only (the path runs on one GPU)"},
@@ -391,6 +405,10 @@ def main():
     ap.add_argument("--nsteps", type=int, default=0, help="override the workload's number of time steps")
     ap.add_argument("--cpu-steps", type=int, default=60, help="time steps of the cpu_baseline sample")
     ap.add_argument("--ref-steps", type=int, default=20, help="time steps per bench step of --impl reference")
+    ap.add_argument("--store", default="", choices=[""] + sorted(STORE_BY_NAME), help="override the workload's store dtype")
+    ap.add_argument("--k", type=int, default=0, help="override the workload's temporal subsampling factor")
+    ap.add_argument("--tangential", action="store_true",
+                    help="FDTD_STORE_TANGENTIAL: store only the 12 tangential slices per slot (a third of the bytes); no cpu_baseline")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--clock-sample-ms", type=int, default=200, help="nvidia-smi polling period during the timed region")
     args = ap.parse_args()

@@ -118,6 +118,16 @@ fdtd_status fdtd_set_design(fdtd_sim*, const int lo[3], const int hi[3]);
  * record_dev[(m-1)][ncomp][box] (caller-owned, >= nsteps*ncomp*box floats).  record_dev may be NULL to clear. */
 fdtd_status fdtd_set_monitor(fdtd_sim*, const int lo[3], const int hi[3], unsigned comp_mask, float* record_dev);
 
+/* What each interface face stores (before fdtd_set_workspace).  FDTD_STORE_ALL (default, R6): all six field
+ * components, 36 slices per slot.  FDTD_STORE_TANGENTIAL: only what the inner interior ever reads from the
+ * shell — the two H components tangential to each LOW face and the two E components tangential to each HIGH face, 12 slices
+ * per slot: a third of the bytes on top of dtype and k.  The shell itself is then not reconstructed in the reverse run:
+ * the design box must lie in the inner interior [P+1, n-P-1) (fdtd_reverse answers FDTD_ERR_INVALID_ARG otherwise), and
+ * the fields left after fdtd_reverse are state 0 on the inner interior only.  Slot layout: [face][2 comps ascending][u][v]. */
+#define FDTD_STORE_ALL 0
+#define FDTD_STORE_TANGENTIAL 1
+fdtd_status fdtd_set_store_mode(fdtd_sim*, int mode);
+
 /* Workspace: the caller allocates device memory, the library sub-allocates fields, psi, adjoint fields, the
  * store and staging buffers from it.  flags: bit 0 = reverse pass buffers, bit 1 = staging for the *_host calls.
  * nsrc_cells = total number of source amplitude cells (host staging only; 0 otherwise). */

@@ -344,8 +344,27 @@ template <class T> struct Sim {
   // face f = 2*axis + side; plane index P (low) or n-P-1 (high); cross-section = interior extent of the other two axes.
   int M(int a) const { return n[a] - 2 * P; }
   size_t face_size(int f) const { int a = f / 2; return (size_t)M((a + 1) % 3) * M((a + 2) % 3); }
-  size_t slot_values() const { size_t s = 0; for (int f = 0; f < 6; ++f) s += 6 * face_size(f); return s; }
-  size_t slice_offset(int f, int comp) const { size_t o = 0; for (int g = 0; g < f; ++g) o += 6 * face_size(g); return o + comp * face_size(f); }
+  // Which components a face stores.  store_mode 0 (reading R6): all six.  store_mode 1 ("tangential"): only
+  // what the inner interior ever reads from the shell — the inverse-E update reads H on the LOW faces through d^-, and
+  // only its two components tangential to the face; the inverse-H update reads E on the HIGH faces through d^+, again
+  // the two tangential ones.  12 slices instead of 36; the shell itself is then not reconstructed.
+  int store_mode = 0;
+  bool stored(int f, int comp) const {
+    if (store_mode == 0) return true;
+    const int a = f / 2, side = f % 2;
+    if (side == 0) return comp >= 3 && comp - 3 != a;
+    return comp < 3 && comp != a;
+  }
+  int ncomp_stored(int f) const { int c = 0; for (int comp = 0; comp < 6; ++comp) c += stored(f, comp); return c; }
+  int nslices() const { int c = 0; for (int f = 0; f < 6; ++f) c += ncomp_stored(f); return c; }
+  size_t slot_values() const { size_t s = 0; for (int f = 0; f < 6; ++f) s += ncomp_stored(f) * face_size(f); return s; }
+  size_t slice_offset(int f, int comp) const {
+    size_t o = 0;
+    for (int g = 0; g < f; ++g) o += ncomp_stored(g) * face_size(g);
+    int rank = 0;
+    for (int c = 0; c < comp; ++c) rank += stored(f, c);
+    return o + rank * face_size(f);
+  }
   // cell of element (u,v) of face f; (u,v) run over the two remaining axes in increasing axis order, v fastest
   size_t face_cell(int f, int u, int v) const {
     int a = f / 2, side = f % 2;  int c[3];
@@ -363,6 +382,8 @@ template <class T> struct Sim {
     const int eb = elem_bytes(dtype, sizeof(T));
     s.data.assign(slot_values() * eb, 0);
     for (int f = 0; f < 6; ++f) for (int comp = 0; comp < 6; ++comp) {
+      s.scale[f * 6 + comp] = 1.0f;
+      if (!stored(f, comp)) continue;
       const size_t fs = face_size(f), off = slice_offset(f, comp);
       const int du = face_dim(f, 0), dv = face_dim(f, 1);
       const T* F = field(comp);
@@ -440,7 +461,7 @@ template <class T> struct Sim {
   }
   size_t store_bytes() const {
     size_t b = 0;
-    for (auto& s : slots) b += s.data.size() + (dtype == DT_E4M3_SCALED ? 36 * 4 : 0);
+    for (auto& s : slots) b += s.data.size() + (dtype == DT_E4M3_SCALED ? nslices() * 4 : 0);
     return b;
   }
 
@@ -523,12 +544,21 @@ template <class T> struct Sim {
     }
   }
   void inject(int nstate, bool magnetic, int interp) {
-    // faces in descending order so that the lowest face index wins on edges and corners (reading R9)
-    for (int f = 5; f >= 0; --f) for (int cidx = 0; cidx < 3; ++cidx) {
+    // a cell on an edge or corner of the shell belongs to the lowest-index face that contains it (reading R9): only that
+    // face writes it, and it writes the components it stores
+    for (int f = 0; f < 6; ++f) for (int cidx = 0; cidx < 3; ++cidx) {
       int comp = magnetic ? 3 + cidx : cidx;  T* F = field(comp);
+      if (!stored(f, comp)) continue;
+      const int a = f / 2, side = f % 2;
+      const int b0 = (a == 0) ? 1 : 0, b1 = (a == 2) ? 1 : 2;
       const int du = face_dim(f, 0), dv = face_dim(f, 1);
-      for (int u = 0; u < du; ++u) for (int v = 0; v < dv; ++v)
+      for (int u = 0; u < du; ++u) for (int v = 0; v < dv; ++v) {
+        int c[3];  c[a] = side ? n[a] - P - 1 : P;  c[b0] = P + u;  c[b1] = P + v;
+        bool lower = side == 1 && P == n[a] - P - 1;
+        for (int g = 0; g < a; ++g) lower = lower || c[g] == P || c[g] == n[g] - P - 1;
+        if (lower) continue;
         F[face_cell(f, u, v)] = fetch(nstate, f, comp, (size_t)u * dv + v, interp);
+      }
     }
   }
   bool on_shell(const int* c) const {
@@ -766,6 +796,8 @@ void orc_reset(void* h) { DISPATCH(h, s.reset()); }
 void orc_set_design(void* h, const int* lo, const int* hi) {
   DISPATCH(h, { s.has_design = true; for (int a = 0; a < 3; ++a) { s.design.lo[a] = lo[a]; s.design.hi[a] = hi[a]; } });
 }
+// 0 = all six components on every face (reading R6), 1 = tangential only; before forward
+void orc_set_store_mode(void* h, int mode) { DISPATCH(h, s.store_mode = mode); }
 void orc_set_monitor(void* h, const int* lo, const int* hi, unsigned mask) {
   DISPATCH(h, { s.has_monitor = true; s.mon_mask = mask; for (int a = 0; a < 3; ++a) { s.monitor.lo[a] = lo[a]; s.monitor.hi[a] = hi[a]; } });
 }

@@ -19,6 +19,7 @@ from . import build as _build
 # precision; >= 10 = the paper's unscaled float8 flavours)
 F32, F16, BF16, E4M3_SCALED, NATIVE = 0, 1, 2, 3, 4
 E4M3B11FNUZ, E5M2FNUZ, E4M3FNUZ, E4M3, E3M4, E4M3FN = 10, 11, 12, 13, 14, 15
+STORE_ALL, STORE_TANGENTIAL = 0, 1
 LINEAR, CUBIC = 0, 1
 # reverse modes: the method / plain definition from store-all snapshots / pure time reversal (P = 0)
 METHOD, STORE_ALL, PURE_REVERSAL = 0, 1, 2
@@ -42,6 +43,7 @@ def lib():
     L.orc_destroy.argtypes = [vp]
     L.orc_reset.argtypes = [vp]
     L.orc_set_design.argtypes = [vp, ip, ip]
+    L.orc_set_store_mode.argtypes = [vp, C.c_int]
     L.orc_set_monitor.argtypes = [vp, ip, ip, C.c_uint]
     L.orc_clear_sources.argtypes = [vp]
     L.orc_add_source.argtypes = [vp, C.c_int, ip, ip, dp, dp, C.c_int]
@@ -146,6 +148,12 @@ class OracleSim:
         self.design = (tuple(lo), tuple(hi))
         lib().orc_set_design(self._h, _i3(lo), _i3(hi))
 
+    def set_store_mode(self, mode):
+        """STORE_ALL (0, default) or STORE_TANGENTIAL (1): only the two tangential H components on the low faces and the two
+        tangential E components on the high faces are stored and injected; the design box must then avoid the shell."""
+        self.store_mode = int(mode)
+        lib().orc_set_store_mode(self._h, int(mode))
+
     def set_monitor(self, lo, hi, comp_mask):
         self.monitor = (tuple(lo), tuple(hi), int(comp_mask))
         lib().orc_set_monitor(self._h, _i3(lo), _i3(hi), int(comp_mask))
@@ -177,6 +185,9 @@ class OracleSim:
         g = None
         if self.design is not None:
             lo, hi = self.design
+            if getattr(self, "store_mode", 0) == STORE_TANGENTIAL and mode == METHOD:
+                assert all(lo[a] >= self.P + 1 and hi[a] <= self.shape[a] - self.P - 1 for a in range(3)), \
+                    "tangential store: the design box must lie in the inner interior (the shell is not reconstructed)"
             g = np.zeros([hi[a] - lo[a] for a in range(3)], dtype=np.float64)
         lib().orc_reverse(self._h, None if df is None else _dp(df), None if dm is None else _dp(dm), int(interp),
                           int(mode), None if g is None else _dp(g))

@@ -85,6 +85,7 @@ struct fdtd_sim {
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int xseg = 16;           // planes per block of the fused marching kernels
+  int store_mode = 0;      // 0: six components per face (R6); 1: tangential only (fdtd_set_store_mode)
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
   // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
@@ -118,9 +119,11 @@ long long face_size(const fdtd_sim* s, int f) {
   const int a = f / 2;
   return (long long)(s->n[(a + 1) % 3] - 2 * s->P) * (s->n[(a + 2) % 3] - 2 * s->P);
 }
+int face_comps(const fdtd_sim* s) { return s->store_mode == 1 ? 2 : 6; }      // stored components per face
+int store_slices(const fdtd_sim* s) { return 6 * face_comps(s); }
 long long slot_values(const fdtd_sim* s) {
   long long v = 0;
-  for (int f = 0; f < 6; ++f) v += 6 * face_size(s, f);
+  for (int f = 0; f < 6; ++f) v += face_comps(s) * face_size(s, f);
   return v;
 }
 int elem_bytes_host(int dt) { return dt == DT_F32 ? 4 : ((dt == DT_F16 || dt == DT_BF16) ? 2 : 1); }
@@ -483,7 +486,8 @@ void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int*
 }
 // half: 0 = E components, 1 = H components, 2 = all six
 void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
-  const long long items = s->st.cell_off[6] * (half == 2 ? 6 : 3);
+  const long long items = s->store_mode == 1 ? s->st.cell_off[6] * (half == 2 ? 2 : 1)   // 2 components on 3 of the 6 faces
+                                             : s->st.cell_off[6] * (half == 2 ? 6 : 3);
   const unsigned g = (unsigned)((items + 255) / 256);
   if (s->dtype == DT_E4M3S) LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
   FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_record<DT>, g, 256, s->d, s->st, m_base, step_dev, half))
@@ -832,6 +836,10 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   if (!(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "workspace was sized without FDTD_WS_REVERSE");
   if ((int)interp < 0 || (int)interp > 1) return fail(s, FDTD_ERR_INVALID_ARG, "unknown interpolation %d", (int)interp);
   if (dmon && !s->has_mon) return fail(s, FDTD_ERR_INVALID_ARG, "dL_dmon given but no monitor is set");
+  if (s->store_mode == 1 && s->has_design)
+    for (int a = 0; a < 3; ++a)
+      if (s->dlo[a] < s->P + 1 || s->dhi[a] > s->n[a] - s->P - 1)
+        return fail(s, FDTD_ERR_INVALID_ARG, "tangential store: the design box must lie in the inner interior (the shell is not reconstructed)");
   const size_t N = (size_t)s->d.N;
   s->cur = s->stream;
   if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
@@ -1013,13 +1021,14 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   st.scales = reinterpret_cast<float*>(w + L.scales);
   st.amax = reinterpret_cast<unsigned*>(w + L.amax);
   st.slot_values = slot_values(s);
+  st.mode = s->store_mode;
   st.val_off[0] = st.cell_off[0] = 0;
   for (int f = 0; f < 6; ++f) {
     const int a = f / 2;
     const int b0 = a == 0 ? 1 : 0, b1 = a == 2 ? 1 : 2;
     st.du[f] = s->n[b0] - 2 * s->P;
     st.dv[f] = s->n[b1] - 2 * s->P;
-    st.val_off[f + 1] = st.val_off[f] + 6 * face_size(s, f);
+    st.val_off[f + 1] = st.val_off[f] + face_comps(s) * face_size(s, f);
     st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
   }
   s->VG = s->V;
@@ -1061,6 +1070,13 @@ fdtd_status fdtd_set_fused(fdtd_sim* s, int mode, int xseg) {
   return FDTD_OK;
 }
 
+fdtd_status fdtd_set_store_mode(fdtd_sim* s, int mode) {
+  if (!s || mode < 0 || mode > 1) return FDTD_ERR_INVALID_ARG;
+  if (s->ws) return fail(s, FDTD_ERR_STATE, "fdtd_set_store_mode must precede fdtd_set_workspace");
+  s->store_mode = mode;
+  return FDTD_OK;
+}
+
 int fdtd_uses_fused(const fdtd_sim* s, int nsteps) { return (s && s->ws && use_fused(s, nsteps)) ? 1 : 0; }
 
 fdtd_status fdtd_forward(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k) {
@@ -1073,7 +1089,7 @@ fdtd_status fdtd_reverse(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
 
 size_t fdtd_store_bytes(const fdtd_sim* s) {
   if (!s || !s->forward_done) return 0;
-  return (size_t)s->st.nslots * (s->st.slot_bytes + (s->dtype == DT_E4M3S ? 36 * 4 : 0));
+  return (size_t)s->st.nslots * (s->st.slot_bytes + (s->dtype == DT_E4M3S ? (size_t)store_slices(s) * 4 : 0));
 }
 
 fdtd_status fdtd_get_fields(fdtd_sim* s, float* out_dev) {
@@ -1254,7 +1270,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 4: v = 40 * Ninner + 28 * dcells; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
       case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
       case 6: v = (double)s->st.slot_values * (4 + eb); break;
-      case 7: case 8: v = 3 * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+      case 7: case 8: v = (s->store_mode == 1 ? 1.0 : 3.0) * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
       case 9: {   // fused marching kernel: E, H read once and written once, ce read: 52 B per cell of [P+1, n-P)^3
         double c = 1;
         for (int a = 0; a < 3; ++a) c *= std::max(0, s->n[a] - 2 * s->P - 1);

@@ -24,8 +24,9 @@ struct StoreDev {
   float* scales;        // [nslots][36]
   unsigned* amax;       // [nslots][36] bit pattern of max|x| per slice (fp8)
   int nslots, nsteps, k, dtype;
+  int mode;             // 0: all six components on every face; 1: tangential only (H on the low faces, E on the high faces)
   long long slot_values;
-  long long val_off[7];   // prefix sums of 6*face_size  (value index of face f)
+  long long val_off[7];   // prefix sums of ncomp(mode)*face_size  (value index of face f)
   long long cell_off[7];  // prefix sums of face_size    (shell-cell index of face f)
   int du[6], dv[6];
 };
@@ -198,7 +199,31 @@ __device__ __forceinline__ int record_slot(const StoreDev& s, int m) {
 // half = 0: the three E components, 1: the three H components, 2: all six.  The two halves of a slot can be written
 // by different launches: E^m is final after the E half-step, H^{m+1/2} after the H half-step.
 struct RecItem { int f, comp; long long e, vidx; };
+// Tangential store (mode 1): the inner interior reads from the shell only H tangential to the LOW faces
+// (through d^- in the inverse-E update) and E tangential to the HIGH faces (through d^+ in the inverse-H update); a face
+// keeps those two components, in increasing component order.
+__device__ __forceinline__ int tangential_comp(int axis, int rank) { return axis == 0 ? 1 + rank : (axis == 1 ? 2 * rank : rank); }
+__device__ __forceinline__ bool record_item_tangential(const StoreDev& s, long long t, int half, RecItem& it) {
+  // half 0: E on the three high faces, half 1: H on the three low faces, half 2: E part then H part
+  for (int h = (half == 2 ? 0 : half); h <= (half == 2 ? 1 : half); ++h) {
+    for (int a = 0; a < 3; ++a) {
+      const int f = 2 * a + (h == 0 ? 1 : 0);
+      const long long fs = s.cell_off[f + 1] - s.cell_off[f];
+      if (t < 2 * fs) {
+        const int rank = (int)(t / fs);
+        it.f = f;
+        it.comp = tangential_comp(a, rank) + (h == 1 ? 3 : 0);
+        it.e = t - rank * fs;
+        it.vidx = s.val_off[f] + rank * fs + it.e;
+        return true;
+      }
+      t -= 2 * fs;
+    }
+  }
+  return false;
+}
 __device__ __forceinline__ bool record_item(const StoreDev& s, long long t, int half, RecItem& it) {
+  if (s.mode == 1) return record_item_tangential(s, t, half, it);
   const int nc = half == 2 ? 6 : 3;
   if (t >= s.cell_off[6] * nc) return false;
   // t enumerates [face][comp in half][element]; cell_off = prefix sums of face sizes
@@ -275,6 +300,8 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
   for (int g = 0; g < a; ++g)
     if (c[g] == d.P || c[g] == d.n[g] - d.P - 1) return;
   if ((f & 1) && d.P == d.n[a] - d.P - 1) return;
+  const bool tang = s.mode == 1;
+  if (tang && ((f & 1) != (magnetic ? 0 : 1))) return;   // tangential store: H lives on the low faces, E on the high ones
   const FetchPlan p = make_plan(nstate, s.nsteps, s.k, s.nslots, interp);
   const long long q = ((long long)c[0] * d.n[1] + c[1]) * d.n[2] + c[2];
   const long long fs = (long long)s.du[f] * s.dv[f];
@@ -282,11 +309,24 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
 #pragma unroll
   for (int cc = 0; cc < 3; ++cc) {
     const int comp = magnetic ? 3 + cc : cc;
-    nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + comp * fs + e);
+    if (tang) {
+      if (cc == a) continue;
+      const int rank = cc > a ? cc - 1 : cc;      // position among the two components tangential to axis a
+      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + rank * fs + e);
+    } else {
+      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + comp * fs + e);
+    }
   }
   if (magnetic) {
 #pragma unroll
-    for (int cc = 0; cc < 3; ++cc) d.H[cc][q] = nv[cc];
+    for (int cc = 0; cc < 3; ++cc)
+      if (!tang || cc != a) d.H[cc][q] = nv[cc];
+    return;
+  }
+  if (tang) {   // the design box lies in the inner interior (checked on the host): no shell gradient term
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+      if (cc != a) d.E[cc][q] = nv[cc];
     return;
   }
   const bool des = d.has_design && c[0] >= d.dlo[0] && c[0] < d.dhi[0] && c[1] >= d.dlo[1] && c[1] < d.dhi[1] &&

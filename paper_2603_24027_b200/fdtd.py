@@ -13,6 +13,7 @@ F32, F16, BF16, F8E4M3_SCALED = 0, 1, 2, 3
 # the paper's unscaled float8 flavours
 F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14
 LINEAR, CUBIC = 0, 1
+STORE_ALL, STORE_TANGENTIAL = 0, 1
 WS_REVERSE, WS_HOST_IO = 1, 2
 STATUS = {0: "FDTD_OK", 1: "FDTD_ERR_INVALID_ARG", 2: "FDTD_ERR_OOM", 3: "FDTD_ERR_CUDA", 4: "FDTD_ERR_STATE",
           5: "FDTD_ERR_UNSUPPORTED"}
@@ -66,6 +67,7 @@ def lib():
     L.fdtd_set_graphs.argtypes = [vp, C.c_int]
     L.fdtd_set_fused.argtypes = [vp, C.c_int, C.c_int]
     L.fdtd_uses_fused.argtypes = [vp, C.c_int]
+    L.fdtd_set_store_mode.argtypes = [vp, C.c_int]
     L.fdtd_get_fields.argtypes = [vp, vp]
     L.fdtd_get_adjoint.argtypes = [vp, vp]
     L.fdtd_get_box.argtypes = [vp, i3, i3, C.c_uint, vp]
@@ -91,7 +93,7 @@ def lib():
 
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
-            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_uses_fused", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
+            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_uses_fused", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count"]
@@ -115,7 +117,7 @@ def _stream_ptr(torch):
 class Sim:
     """fdtd_sim handle.  eps: float32 CUDA tensor [nx,ny,nz] (kept alive by this object)."""
 
-    def __init__(self, eps, dx, dt, pml_width, design=None, monitor=None, cpml=None):
+    def __init__(self, eps, dx, dt, pml_width, design=None, monitor=None, cpml=None, store_mode=STORE_ALL):
         torch = _torch()
         self._torch = torch
         self._L = lib()
@@ -136,6 +138,9 @@ class Sim:
         self._keep = []
         if cpml is not None:
             self._check(self._L.fdtd_set_cpml(self._h, *[float(x) for x in cpml]))
+        self.store_mode = int(store_mode)
+        if store_mode != STORE_ALL:
+            self._check(self._L.fdtd_set_store_mode(self._h, int(store_mode)))
         if design is not None:
             self.design = (tuple(design[0]), tuple(design[1]))
             self._check(self._L.fdtd_set_design(self._h, _i3(design[0]), _i3(design[1])))

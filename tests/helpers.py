@@ -5,8 +5,10 @@ from oracle import fdtd_oracle as orc
 from paper_2603_24027_b200 import workloads as W
 
 
-def make_oracle(w, prec, cpml=orc.CPML_DEFAULTS, with_sources=True):
+def make_oracle(w, prec, cpml=orc.CPML_DEFAULTS, with_sources=True, store_mode=0):
     s = orc.OracleSim(prec, w.eps, w.pml, W.S, cpml)
+    if store_mode:
+        s.set_store_mode(store_mode)
     s.set_design(*w.design)
     s.set_monitor(*w.monitor)
     if with_sources:
@@ -15,12 +17,12 @@ def make_oracle(w, prec, cpml=orc.CPML_DEFAULTS, with_sources=True):
     return s
 
 
-def oracle_gradient(w, prec, dtype, k, interp=orc.LINEAR, mode=orc.METHOD, eps=None, extra=None):
+def oracle_gradient(w, prec, dtype, k, interp=orc.LINEAR, mode=orc.METHOD, eps=None, extra=None, store_mode=0):
     """forward -> loss -> reverse.  Returns dict(L, grad, final, state0, mon, sim)."""
     if eps is not None:
         import dataclasses
         w = dataclasses.replace(w, eps=np.asarray(eps))
-    s = make_oracle(w, prec)
+    s = make_oracle(w, prec, store_mode=store_mode)
     if mode == orc.STORE_ALL:
         s.set_keep_all(True)
     s.forward(w.nsteps, dtype, k)
@@ -38,11 +40,11 @@ def rel_l2(a, b):
 
 
 # ---- CUDA path (imported lazily so that CPU-only test runs never touch torch.cuda) ----
-def gpu_sim(w, cpml=None):
+def gpu_sim(w, cpml=None, store_mode=0):
     import torch
     from paper_2603_24027_b200 import fdtd
     eps = torch.from_numpy(np.ascontiguousarray(w.eps, dtype=np.float32)).cuda()
-    return fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor, cpml=cpml)
+    return fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor, cpml=cpml, store_mode=store_mode)
 
 
 def gpu_gradient(w, dtype, k, interp=0, extra=None, sim=None):

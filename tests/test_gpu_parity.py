@@ -262,6 +262,57 @@ def test_fused_marching_path_matches_two_kernel_path(dtype, k, xseg, graphs):
             assert np.array_equal(sa.cpu().numpy(), sb.cpu().numpy()), j
 
 
+def _inner_design(w):
+    P = w.pml
+    return dataclasses.replace(w, design=(tuple([P + 1] * 3), tuple(n - P - 1 for n in w.shape)))
+
+
+@pytest.mark.parametrize("which,dtype,k,interp", [("tiny", W.F32, 1, W.LINEAR), ("tiny", W.F8E4M3_SCALED, 3, W.LINEAR),
+                                                  ("mid", W.BF16, 4, W.CUBIC), ("mid", W.F8E4M3B11FNUZ, 8, W.LINEAR)])
+def test_tangential_only_store_parity(which, dtype, k, interp):
+    """FDTD_STORE_TANGENTIAL (12 of the 36 slices): every slot byte for byte, store bytes (a third), the reconstructed inner
+    interior and the gradient against the float32 oracle in the same mode; and the gradient against the all-components
+    store of the same run (same injected values reach the inner interior)."""
+    w = _inner_design(W.tiny(nsteps=26) if which == "tiny" else mid_workload(dtype=dtype, k=k))
+    o = oracle_gradient(w, 32, dtype, k, interp, store_mode=orc.STORE_TANGENTIAL)
+    s = gpu_sim(w, store_mode=1)
+    g = gpu_gradient(w, dtype, k, interp, sim=s)
+    P = w.pml
+    inner = (slice(None),) + tuple(slice(P + 1, n - P - 1) for n in w.shape)
+    assert rel_l2(g["final"], o["final"]) <= FIELD_TOL
+    assert rel_l2(g["grad"], o["grad"]) <= GRAD_TOL
+    peak = np.abs(o["final"]).max()
+    assert np.abs((g["state0"] - o["state0"])[inner]).max() <= 1e-5 * peak
+    assert s.store_bytes() == o["sim"].store_bytes()
+    full = gpu_gradient(w, dtype, k, interp)
+    assert full["sim"].slot_values() == 3 * s.slot_values()
+    assert rel_l2(g["grad"], full["grad"]) <= 1e-5
+    s.forward(w.nsteps, w.sources, dtype, k)
+    of = make_oracle(w, 32, store_mode=orc.STORE_TANGENTIAL)
+    of.forward(w.nsteps, dtype, k)
+    assert s.num_slots() == of.num_slots() and s.slot_values() == of.slot_values()
+    for j in range(of.num_slots()):
+        data, scales = s.slot(j, dtype)
+        od, osc = of.slot(j, dtype)
+        assert np.array_equal(data.cpu().numpy(), od), (dtype, j)
+        if dtype == W.F8E4M3_SCALED:
+            stored = [f * 6 + (0 if f % 2 else 3) + b for f in range(6) for b in range(3) if b != f // 2]   # H low, E high
+            assert len(stored) == 12
+            assert np.array_equal(scales.cpu().numpy()[stored], osc[stored]), (dtype, j)
+    print(f"[parity] tangential store {which} dtype={dtype} k={k}: grad rel-L2 {rel_l2(g['grad'], o['grad']):.3e}, "
+          f"vs all-components store {rel_l2(g['grad'], full['grad']):.3e}, bytes {s.store_bytes()}")
+
+
+def test_tangential_store_rejects_a_design_on_the_shell():
+    fdtd = _fdtd()
+    w = W.tiny(nsteps=8)       # its design box touches the shell
+    s = gpu_sim(w, store_mode=1)
+    mon = s.forward(w.nsteps, w.sources, W.F32, 1)
+    with pytest.raises(fdtd.FdtdError) as e:
+        s.reverse(None, mon * 0 + 1.0, W.LINEAR)
+    assert e.value.status == 1
+
+
 def test_store_slots_bit_exact_when_fields_agree():
     """Record kernel vs oracle record: every slot, byte for byte, for each dtype (fields are bit-identical in practice;
     if they are not, compare the decoded values within the field tolerance instead)."""

@@ -137,3 +137,41 @@ def test_last_interval_when_nsteps_not_multiple_of_k():
     a, b = np.float32(vals[off + 3]), np.float32(v6[off + 3])
     mid = s.fetch(21, 2, 4, 3)                             # halfway through the short interval [20, 22]
     assert abs(mid - 0.5 * (float(a) + float(b))) <= 1e-7 * max(abs(float(a)), abs(float(b)), 1e-30)
+
+
+def _inner_design(w):
+    P = w.pml
+    return dataclasses.replace(w, design=(tuple([P + 1] * 3), tuple(n - P - 1 for n in w.shape)))
+
+
+@pytest.mark.parametrize("shape,P", [((14, 13, 12), 3), ((11, 12, 10), 2)])
+def test_tangential_only_store_reconstructs_the_inner_interior_and_the_gradient(shape, P):
+    """the inner interior reads from the shell only H tangential to the LOW faces and E tangential to the HIGH
+    faces.  Pins: (1) with those 12 slices alone (f64, k = 1) the reverse run returns the inner interior to state 0 to
+    rounding; (2) its gradient equals back-propagation through stored states (plain definition) and the all-six-components
+    run; (3) the store is exactly 1/3 (equal-sized slices per face)."""
+    w = _inner_design(W.tiny(shape=shape, P=P, nsteps=30))
+    full = oracle_gradient(w, 64, orc.NATIVE, 1)
+    tang = oracle_gradient(w, 64, orc.NATIVE, 1, store_mode=orc.STORE_TANGENTIAL)
+    plain = oracle_gradient(w, 64, orc.NATIVE, 1, mode=orc.STORE_ALL)
+    peak = np.abs(full["final"]).max()
+    inner = (slice(None),) + tuple(slice(P + 1, n - P - 1) for n in shape)
+    assert np.abs(tang["state0"][inner]).max() <= 1e-13 * peak
+    assert np.abs(plain["grad"]).max() > 0
+    assert rel_l2(tang["grad"], plain["grad"]) < 1e-10
+    assert rel_l2(tang["grad"], full["grad"]) < 1e-10
+    assert tang["sim"].slot_values() * 3 == full["sim"].slot_values()
+    assert tang["sim"].store_bytes() * 3 == full["sim"].store_bytes()
+    # the forward run is untouched by the store mode
+    assert np.array_equal(tang["final"], full["final"]) and tang["L"] == full["L"]
+
+
+def test_tangential_only_store_compressed_matches_full_store_on_the_inner_interior():
+    """Under compression (bf16, k = 4; fp8+scale, k = 3) the inner interior sees the same injected values in both store
+    modes, so the float32 gradient is the same to rounding of the accumulation; scales are per slice in both."""
+    w = _inner_design(W.tiny(nsteps=26))
+    for dtype, k in [(orc.BF16, 4), (orc.E4M3_SCALED, 3)]:
+        full = oracle_gradient(w, 32, dtype, k)
+        tang = oracle_gradient(w, 32, dtype, k, store_mode=orc.STORE_TANGENTIAL)
+        assert rel_l2(tang["grad"], full["grad"]) < 1e-6
+        assert tang["sim"].slot_values() * 3 == full["sim"].slot_values()
