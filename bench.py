@@ -313,7 +313,7 @@ def run_gpu(args, rank, world):
         "reverse_mcells_per_s": whole_job_value(w.cells, w.nsteps, args.steps, world, r_ms),
         "forward_ms": f_ms / args.steps, "reverse_ms": r_ms / args.steps,
         "store_bytes": sim_store_bytes(sim, w, flags), "store_bytes_per_step": sim_store_bytes(sim, w, flags) / w.nsteps,
-        "store_bytes_f32_k1": (w.nsteps + 1) * sim.slot_values() * 4,
+        "store_bytes_f32_k1": (w.nsteps + 1) * sim.slot_values() * (3 if args.tangential else 1) * 4,   # all six components
         "effective_gbs": {"forward": fwd_gbs, "reverse": rev_gbs, "forward_frac_of_peak": fwd_gbs / peak,
                           "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused),
                           "forward_two_kernel_equivalent": fwd2_gbs, "forward_two_kernel_equivalent_frac": fwd2_gbs / peak},
