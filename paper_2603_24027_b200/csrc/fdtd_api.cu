@@ -58,7 +58,7 @@ struct fdtd_sim {
   cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
   bool parallel = false;               // auxiliary streams available
   std::vector<cudaGraphExec_t> dead_graphs;
-  cudaGraphExec_t graph_cache[3] = {nullptr, nullptr, nullptr};   // forward, fused forward, reverse
+  cudaGraphExec_t graph_cache[4] = {nullptr, nullptr, nullptr, nullptr};   // forward, fused forward, reverse, fused reverse
   mutable std::string err;
   const float* eps_dev = nullptr;
   double cpml[4] = {0.8, 1.0, 0.01, 3.0};
@@ -84,6 +84,7 @@ struct fdtd_sim {
   int cb = 0;
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
+  int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 16;           // planes per block of the fused marching kernels
   int store_mode = 0;      // 0: six components per face (R6); 1: tangential only (fdtd_set_store_mode)
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
@@ -463,7 +464,7 @@ void launch_grad(fdtd_sim* s) {
   const long long cells = (long long)ext[0] * ext[1] * ext[2];
   LAUNCH(s, k_grad, (unsigned)((cells + 255) / 256), 256, s->d);
 }
-void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, int x0 = 0, int x1 = 1 << 30) {
+void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, int x0 = 0, int x1 = 1 << 30, int buffer = -1) {
   if (s->nsrc == 0) return;
   bool any = false;
   for (int i = 0; i < s->nsrc; ++i) any = any || (s->src_host[i].lo[0] < x1 && s->src_host[i].hi[0] > x0);
@@ -475,7 +476,10 @@ void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, in
   }
   const int threads = maxc >= 128 ? 128 : 32;
   const dim3 g((unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024), (unsigned)s->nsrc);
-  LAUNCH(s, k_sources, g, threads, s->d, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
+  Dev dd = s->d;
+  if (buffer >= 0)
+    for (int c = 0; c < 3; ++c) dd.E[c] = s->fb[buffer][c];
+  LAUNCH(s, k_sources, g, threads, dd, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
          reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign, x0, x1);
 }
 void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode, int half = 2) {
@@ -492,9 +496,16 @@ void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
   if (s->dtype == DT_E4M3S) LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
   FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_record<DT>, g, 256, s->d, s->st, m_base, step_dev, half))
 }
-void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp) {
+// from / to: buffer that holds the shell E of state m / buffer that receives the injected values (-1 = the current one)
+void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp, int from = -1, int to = -1) {
   const unsigned g = (unsigned)((s->st.cell_off[6] + 255) / 256);
-  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_inject<DT>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp))
+  InjIO io;
+  for (int c = 0; c < 3; ++c) {
+    io.Eold[c] = from < 0 ? s->d.E[c] : s->fb[from][c];
+    io.Eout[c] = to < 0 ? s->d.E[c] : s->fb[to][c];
+    io.Hout[c] = to < 0 ? s->d.H[c] : s->fb[to][3 + c];
+  }
+  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_inject<DT>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp, io))
 }
 
 // One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
@@ -578,6 +589,23 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   if (inv) LAUNCH(s, k_fused_he<true>, g, b, s->d, a);
   else LAUNCH(s, k_fused_he<false>, g, b, s->d, a);
 }
+// inverse-E update of the source cells redone in the canonical order after the reverse marching kernel (k_inv_e_sources)
+void launch_inv_e_sources(fdtd_sim* s, int m_base, const int* step_dev, int from, int to) {
+  if (s->nsrc == 0) return;
+  long long maxc = 1;
+  for (int i = 0; i < s->nsrc; ++i) {
+    const SrcDev& q = s->src_host[i];
+    maxc = std::max(maxc, (long long)(q.hi[0] - q.lo[0]) * (q.hi[1] - q.lo[1]) * (q.hi[2] - q.lo[2]));
+  }
+  InvFixArgs a;
+  for (int c = 0; c < 3; ++c) { a.Eold[c] = s->fb[from][c]; a.Hnew[c] = s->fb[to][3 + c]; a.Eout[c] = s->fb[to][c]; }
+  a.src = reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc);
+  a.waves = reinterpret_cast<const float*>(s->ws + s->L.waves);
+  a.nsrc = s->nsrc; a.m_base = m_base; a.step_dev = step_dev;
+  const int threads = maxc >= 128 ? 128 : 32;
+  const dim3 g((unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024), (unsigned)s->nsrc);
+  LAUNCH(s, k_inv_e_sources, g, threads, s->d, a);
+}
 FieldIO io_of(const fdtd_sim* s, int eb, int hb, int ob, int out_is_h) {
   FieldIO io;
   for (int c = 0; c < 3; ++c) { io.E[c] = s->fb[eb][c]; io.H[c] = s->fb[hb][3 + c]; io.out[c] = s->fb[ob][out_is_h ? 3 + c : c]; }
@@ -610,6 +638,39 @@ void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec, 
   set_cur(s, oth);
   launch_sources(s, m_base + 1, step_dev, 1.0f);
   *pending_h = rec;
+}
+
+// Reverse step with the fused inverse kernel (fdtd_fused.cuh, INV): the primal goes from the current buffer (E^m, H^{m+1/2})
+// to the other one (E^{m-1}, H^{m-1/2}) in one marching pass over the inner interior.
+//  1: {monitor cotangent then adjoint-H general, adjoint-H lean, [inject H into the other buffer, then the marching kernel,
+//      which subtracts the sources of step m itself between its two half-steps]}
+//  2: {adjoint-E lean, adjoint-E general, gradient (new H), [sources subtracted from the OLD shell E, then inject E: old shell
+//      E for the gradient term, new values into the other buffer]}
+void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
+  const bool cot = dmon && s->has_mon;
+  const int cur = s->cb, oth = cur ^ 1;
+  fork(s, 3);
+  on(s, 1);
+  if (cot) {
+    launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
+    if (s->parallel) { cudaEventRecord(s->ev_mid, s->aux[0]); cudaStreamWaitEvent(s->stream, s->ev_mid, 0); }
+  }
+  launch_gen(s, 2, pb);
+  on(s, 0); launch_lean(s, 2);
+  on(s, 2);
+  launch_inject(s, m_base, step_dev, 1, interp, cur, oth);
+  launch_fused(s, true, cur, oth);
+  launch_inv_e_sources(s, m_base, step_dev, cur, oth);
+  join(s, 3);
+  set_cur(s, oth);
+  fork(s, 4);
+  on(s, 0); launch_lean(s, 3);
+  on(s, 1); launch_gen(s, 3, pb);
+  on(s, 2); launch_grad(s);
+  on(s, 3);
+  launch_sources(s, m_base, step_dev, -1.0f, 0, 1 << 30, cur);
+  launch_inject(s, m_base, step_dev, 0, interp, cur, oth);
+  join(s, 4);
 }
 
 // Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.  The
@@ -743,6 +804,13 @@ bool use_fused(const fdtd_sim* s, int nsteps) {
   tiles *= (s->n[0] - 2 * s->P + s->xseg - 1) / s->xseg;
   return tiles >= 4 * 3 * 148;
 }
+bool use_fused_reverse(const fdtd_sim* s) {
+  if (s->fuse_rev_mode == 0) return false;
+  // mode -1 (auto): off.  Measured on B200 (round 1, C4): bit-identical to the two-kernel reverse primal and 2.5 GB fewer
+  // bytes per step, but the step is not faster (3406 vs 3395 us): beside the adjoint kernels the marching kernel runs at
+  // 1.23 ms instead of the 1.03 ms of its forward twin.  Kept as an option (fdtd_set_fused mode 1).
+  return s->fuse_rev_mode == 1 && s->can_fuse;
+}
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
   launch_record(s, 0, nullptr, 2);
@@ -867,6 +935,7 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   s->state_final = false;
   int pb = 0;
   int top = s->nsteps;
+  const bool rf = use_fused_reverse(s);   // inverse-H + inverse-E of the primal in one marching kernel (ping-pong buffers)
   {
     const int L = 16;   // even, so the psi ping-pong parity is the same at the start of every period
     const int periods = (s->use_graphs && s->aux[0]) ? s->nsteps / L : 0;
@@ -874,8 +943,11 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
       int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
       LAUNCH(s, k_set_int, 1, 1, step_dev, s->nsteps);
       s->parallel = true;
-      fdtd_status g = run_graph(s, 2, periods, [&]() {
-        for (int t = 0; t < L; ++t) reverse_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+      fdtd_status g = run_graph(s, rf ? 3 : 2, periods, [&]() {
+        for (int t = 0; t < L; ++t) {
+          if (rf) reverse_fused_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+          else reverse_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+        }
         LAUNCH(s, k_tick, 1, 1, step_dev, -L);
       });
       s->parallel = false;
@@ -884,7 +956,10 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
       top -= periods * L;
     }
   }
-  for (int m = top; m >= 1; --m, pb ^= 1) reverse_step(s, m, nullptr, dmon, (int)interp, pb);
+  for (int m = top; m >= 1; --m, pb ^= 1) {
+    if (rf) reverse_fused_step(s, m, nullptr, dmon, (int)interp, pb);
+    else reverse_step(s, m, nullptr, dmon, (int)interp, pb);
+  }
   if (grad_dev && s->has_design)
     LAUNCH(s, k_grad_finalize, (unsigned)((design_cells(s) + 255) / 256), 256, s->d, s->eps_dev, grad_dev);
   CUDA_TRY(s, cudaGetLastError());
@@ -913,6 +988,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   s->cur = s->stream;
   if (const char* e = std::getenv("FDTD_FUSE")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_mode = v; }
+  if (const char* e = std::getenv("FDTD_FUSE_REV")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_rev_mode = v; }
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
@@ -1065,7 +1141,7 @@ fdtd_status fdtd_set_graphs(fdtd_sim* s, int enabled) {
 
 fdtd_status fdtd_set_fused(fdtd_sim* s, int mode, int xseg) {
   if (!s || mode < -1 || mode > 1 || xseg < 0) return FDTD_ERR_INVALID_ARG;
-  s->fuse_mode = mode;
+  s->fuse_mode = s->fuse_rev_mode = mode;
   if (xseg > 0) s->xseg = xseg;
   return FDTD_OK;
 }
@@ -1305,7 +1381,7 @@ void fdtd_destroy(fdtd_sim* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
   reap_graphs(s);
-  for (int g = 0; g < 3; ++g)
+  for (int g = 0; g < 4; ++g)
     if (s->graph_cache[g]) cudaGraphExecDestroy(s->graph_cache[g]);
   for (int b = 0; b < 3; ++b) {
     if (s->aux[b]) cudaStreamDestroy(s->aux[b]);

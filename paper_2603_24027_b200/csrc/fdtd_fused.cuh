@@ -16,10 +16,12 @@
 // Forward: the region [lo, hi) starts one cell inside the interior (lo = P + 1), so every halo cell (index P) is a plain
 // cell whose new H follows from the inputs alone: the kernel reads nothing that another kernel of the same step writes
 // and runs beside the slab kernels.  Reverse (INV): the region is the inner interior and the halo cells are interface
-// shell cells, whose H^{m-1/2} the inject kernel has already put into the OUTPUT buffer; they are read from there.
+// shell cells, whose H^{m-1/2} the inject kernel has already put into the OUTPUT buffer; they are read from there.  The
+// sources of step m are ignored here and the (few) source cells redone afterwards by k_inv_e_sources.
 // Arithmetic is that of the lean kernels (R3), so results are bit-identical to the two-kernel path.
 #pragma once
 #include "fdtd_dev.cuh"
+#include "fdtd_store.cuh"
 
 namespace fdtd {
 
@@ -36,7 +38,7 @@ struct FusedArgs {
 };
 
 template <bool INV>
-__global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_constant__ Dev d, const __grid_constant__ FusedArgs a) {
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __grid_constant__ Dev d, const __grid_constant__ FusedArgs a) {
   __shared__ float4 shH[2][FUSED_TR + 1][32][2];   // new Hx, Hz of the current plane, double-buffered over the march
   __shared__ float4 shE[2][FUSED_TR + 1][32][2];   // Ex, Ez of the NEXT plane (read one march step later by the row below)
   const int lane = threadIdx.x, w = threadIdx.y;
@@ -55,7 +57,6 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
 #pragma unroll
   for (int v = 0; v < 4; ++v) zv[v] = k0 + v >= a.lo[2] && k0 + v < a.hi[2];
   const bool zfull = zv[0] && zv[1] && zv[2] && zv[3];
-  const bool low_yz = j < a.lo[1] || !zfull;      // INV: some element takes its new H from the output buffer
   const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];   // the warp above holds row j + 1 (not a clamped copy)
   const idx_t sx = d.sx, sy = d.sy;
   const float cH = INV ? d.S : -d.S;
@@ -85,6 +86,7 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
     VF<4> ce;
     const bool store_plane = own && i >= xs;
     if (store_plane) ce = ldv<4>(d.ce + q);
+
     // ---- H half-step ----
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
@@ -94,12 +96,20 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
       hy.v[v] = fmaf(cH, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
       hz.v[v] = fmaf(cH, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
     }
-    if (INV && (low_yz || i < a.lo[0])) {         // shell cells: their new H is already in the output buffer (inject)
-      const VF<4> ox = ldv<4>(a.Hout[0] + q), oy = ldv<4>(a.Hout[1] + q), oz = ldv<4>(a.Hout[2] + q);
-      const bool all = j < a.lo[1] || i < a.lo[0];
-#pragma unroll
-      for (int v = 0; v < 4; ++v)
-        if (all || !zv[v]) { hx.v[v] = ox.v[v]; hy.v[v] = oy.v[v]; hz.v[v] = oz.v[v]; }
+    if (INV) {
+      // Shell cells next to the region take their new H from the output buffer (inject has put H^{m-1/2} there).  Only
+      // what an E update inside the region reads is needed: Hx, Hz of the row below (d_y^-), Hy, Hz of the plane below
+      // (d_x^-), Hx, Hy of the cell below in z (d_z^-).  The shell cell above the last group is read by nobody.
+      if (j < a.lo[1]) {
+        hx = ldv<4>(a.Hout[0] + q);
+        hz = ldv<4>(a.Hout[2] + q);
+      } else if (i < a.lo[0]) {
+        hy = ldv<4>(a.Hout[1] + q);
+        hz = ldv<4>(a.Hout[2] + q);
+      } else if (!zv[0]) {
+        hx.v[0] = a.Hout[0][q];
+        hy.v[0] = a.Hout[1][q];
+      }
     }
     // ---- hand the new H to the row above (shared memory) and to the lane above (shuffle); E of the next plane to the
     //      row below for the next march step ----
@@ -137,6 +147,55 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1)) k_fused_he(const __grid_c
     }
     hy_xm = hy; hz_xm = hz;
     ex = exn; ey = eyn; ez = ezn;
+  }
+}
+
+// Source cells of the reverse variant.  The canonical order (R9) subtracts the source of step m from E^m BEFORE the
+// inverse-E update, while the marching kernel's inverse-H update needs the untouched E^m; so the marching kernel ignores
+// the sources and this small kernel redoes the inverse-E update of the (few) source cells of the inner interior afterwards,
+// from the same inputs in the canonical order:  E^{m-1} = fma(-ce, curl^-(H^{m-1/2}), E^m - src).  blockIdx.y = source; a
+// cell covered by several sources is written by the lowest-numbered one, which subtracts all of them in index order.
+struct InvFixArgs {
+  const float* Eold[3];   // E^m (input buffer of the marching kernel)
+  const float* Hnew[3];   // H^{m-1/2} (its output buffer)
+  float* Eout[3];
+  const SrcDev* src;
+  const float* waves;
+  int nsrc, m_base;
+  const int* step_dev;
+};
+__global__ void k_inv_e_sources(const __grid_constant__ Dev d, const __grid_constant__ InvFixArgs a) {
+  const SrcDev S = a.src[blockIdx.y];
+  const int P = d.P, ey_ = S.hi[1] - S.lo[1], ez_ = S.hi[2] - S.lo[2];
+  const long long cells = (long long)(S.hi[0] - S.lo[0]) * ey_ * ez_;
+  const int m = a.m_base + (a.step_dev ? *a.step_dev : 0);
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < cells; t += (long long)gridDim.x * blockDim.x) {
+    const int c[3] = {S.lo[0] + (int)(t / ((long long)ez_ * ey_)), S.lo[1] + (int)((t / ez_) % ey_), S.lo[2] + (int)(t % ez_)};
+    bool inner = true;
+#pragma unroll
+    for (int ax = 0; ax < 3; ++ax) inner = inner && c[ax] >= P + 1 && c[ax] < d.n[ax] - P - 1;
+    if (!inner) continue;                       // shell cells are overwritten by inject
+    const idx_t q = ((idx_t)c[0] * d.n[1] + c[1]) * d.n[2] + c[2];
+    float e[3] = {a.Eold[0][q], a.Eold[1][q], a.Eold[2][q]};
+    bool touched[3] = {false, false, false};
+    bool first = true;
+    for (int u = 0; u < a.nsrc; ++u) {
+      const SrcDev U = a.src[u];
+      if (c[0] < U.lo[0] || c[0] >= U.hi[0] || c[1] < U.lo[1] || c[1] >= U.hi[1] || c[2] < U.lo[2] || c[2] >= U.hi[2]) continue;
+      if (u < (int)blockIdx.y) { first = false; break; }
+      const long long ti = ((long long)(c[0] - U.lo[0]) * (U.hi[1] - U.lo[1]) + (c[1] - U.lo[1])) * (U.hi[2] - U.lo[2]) + (c[2] - U.lo[2]);
+      const float v = (U.amp ? U.amp[ti] : 1.0f) * a.waves[U.wave_off + m - 1];
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+        if (U.comp == cc) { e[cc] += -1.0f * v; touched[cc] = true; }
+    }
+    if (!first) continue;
+    const idx_t sx = d.sx, sy = d.sy;
+    const float hx = a.Hnew[0][q], hy = a.Hnew[1][q], hz = a.Hnew[2][q];
+    const float ce = d.ce[q];
+    if (touched[0]) a.Eout[0][q] = fmaf(-ce, (hz - a.Hnew[2][q - sy]) - (hy - a.Hnew[1][q - 1]), e[0]);
+    if (touched[1]) a.Eout[1][q] = fmaf(-ce, (hx - a.Hnew[0][q - 1]) - (hz - a.Hnew[2][q - sx]), e[1]);
+    if (touched[2]) a.Eout[2][q] = fmaf(-ce, (hy - a.Hnew[1][q - sx]) - (hx - a.Hnew[0][q - sy]), e[2]);
   }
 }
 

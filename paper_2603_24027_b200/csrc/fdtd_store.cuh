@@ -285,9 +285,17 @@ __global__ void __launch_bounds__(256) k_record(const __grid_constant__ Dev d, c
 // E injection also takes the shell-cell gradient term in its dE form:
 //   acc += sum_c lE_c * (E_old - E_new)_c / ce      on design ∩ shell.
 // ---------------------------------------------------------------------------------------------------------
+// Eold: where the shell E of state m sits (read for the gradient term); Eout / Hout: where the injected values go.  The same
+// arrays in the in-place path; old / new buffer in the fused reverse path (fdtd_fused.cuh).
+struct InjIO {
+  const float* Eold[3];
+  float* Eout[3];
+  float* Hout[3];
+};
 template <int DT>
 __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
-                                                int m_base, const int* step_dev, int magnetic, int interp) {
+                                                int m_base, const int* step_dev, int magnetic, int interp,
+                                                const __grid_constant__ InjIO io) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= s.cell_off[6]) return;
   const int nstate = cur_step(m_base, step_dev) - 1;
@@ -320,13 +328,13 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
   if (magnetic) {
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc)
-      if (!tang || cc != a) d.H[cc][q] = nv[cc];
+      if (!tang || cc != a) io.Hout[cc][q] = nv[cc];
     return;
   }
   if (tang) {   // the design box lies in the inner interior (checked on the host): no shell gradient term
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc)
-      if (cc != a) d.E[cc][q] = nv[cc];
+      if (cc != a) io.Eout[cc][q] = nv[cc];
     return;
   }
   const bool des = d.has_design && c[0] >= d.dlo[0] && c[0] < d.dhi[0] && c[1] >= d.dlo[1] && c[1] < d.dhi[1] &&
@@ -336,7 +344,7 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
     double sacc = 0.0;
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) {
-      const float dE = d.E[cc][q] - nv[cc];
+      const float dE = io.Eold[cc][q] - nv[cc];
       sacc += (double)d.lE[cc][q] * ((double)dE / ce);
     }
     const long long ei = ((long long)(c[0] - d.dlo[0]) * (d.dhi[1] - d.dlo[1]) + (c[1] - d.dlo[1])) * (d.dhi[2] - d.dlo[2]) +
@@ -344,7 +352,7 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
     d.acc[ei] += sacc;
   }
 #pragma unroll
-  for (int cc = 0; cc < 3; ++cc) d.E[cc][q] = nv[cc];
+  for (int cc = 0; cc < 3; ++cc) io.Eout[cc][q] = nv[cc];
 }
 
 // ---------------------------------------------------------------------------------------------------------
