@@ -316,6 +316,27 @@ def test_tangential_store_rejects_a_design_on_the_shell():
     assert e.value.status == 1
 
 
+def test_kept_graph_executables_follow_every_change_of_settings():
+    """The library keeps its instantiated CUDA graphs and patches them (cudaGraphExecUpdate) on later runs.  One handle driven
+    through changes of store dtype, k, interpolation, run length, fused mode and fresh monitor / cotangent tensors must give,
+    bit for bit, what a fresh handle gives for each setting."""
+    w0 = mid_workload(nsteps=70)
+    s = gpu_sim(w0)
+    seq = [(W.BF16, 4, W.LINEAR, 70, 0), (W.BF16, 4, W.LINEAR, 70, 0), (W.F16, 8, W.CUBIC, 70, 0), (W.F32, 1, W.LINEAR, 50, 0),
+           (W.F8E4M3_SCALED, 3, W.LINEAR, 70, 1), (W.BF16, 4, W.LINEAR, 70, 1), (W.F8E5M2FNUZ, 5, W.CUBIC, 66, 0)]
+    for dtype, k, interp, nsteps, fused in seq:
+        w = mid_workload(nsteps=nsteps, dtype=dtype, k=k)
+        s.set_fused(fused, 7)
+        a = gpu_gradient(w, dtype, k, interp, sim=s)
+        fresh = gpu_sim(w)
+        fresh.set_fused(fused, 7)
+        b = gpu_gradient(w, dtype, k, interp, sim=fresh)
+        for key in ("final", "mon", "grad"):
+            assert np.array_equal(a[key], b[key]), (dtype, k, interp, nsteps, fused, key)
+        assert s.store_bytes() == fresh.store_bytes()
+        fresh.destroy()
+
+
 def test_store_slots_bit_exact_when_fields_agree():
     """Record kernel vs oracle record: every slot, byte for byte, for each dtype (fields are bit-identical in practice;
     if they are not, compare the decoded values within the field tolerance instead)."""

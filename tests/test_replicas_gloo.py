@@ -72,3 +72,29 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["unit"] == "Mcell-updates/s"
+
+
+def test_design_map_chain_rule_matches_finite_differences():
+    """optimize.py (harness): filter + projection + broadcast and their hand-written backward pass."""
+    import numpy as np
+    from paper_2603_24027_b200 import optimize as O, workloads as W
+    w = W.c2(nsteps=8)
+    des = O.Design(w)
+    rng = np.random.default_rng(3)
+    rho = rng.uniform(0.2, 0.8, (des.nx, des.ny))
+    c = rng.standard_normal((des.nx, des.ny, des.nzl))           # loss = <c, eps on the design box>
+    lo, hi = w.design
+    box = (slice(lo[0], hi[0]), slice(lo[1], hi[1]), slice(lo[2], hi[2]))
+
+    def loss(r):
+        eps, _ = des.forward(r, 3.0)
+        return float(np.sum(c * eps[box].astype(np.float64)))
+    des.forward(rho, 3.0)
+    g = des.backward(c)
+    for (i, j) in [(0, 0), (5, 17), (40, 63), (63, 31)]:
+        h = 1e-3
+        rp, rm = rho.copy(), rho.copy()
+        rp[i, j] += h
+        rm[i, j] -= h
+        fd = (loss(rp) - loss(rm)) / (2 * h)
+        assert abs(fd - g[i, j]) <= 2e-3 * max(abs(fd), 1e-3), (i, j, fd, g[i, j])
