@@ -311,10 +311,11 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
     B.G[b] = G; B.RW[b] = RW;
     B.ginv[b] = make_ginv(G);
     B.nbx[b] = (groups + G - 1) / G;
-    B.nby[b] = (y1 - y0 + TY * RW - 1) / (TY * RW);
-    B.dnbx[b] = make_fastdiv((unsigned)B.nbx[b], (unsigned)B.nbx[b] * B.nby[b] * (unsigned)(bx1 - bx0));
-    B.dnby[b] = make_fastdiv((unsigned)B.nby[b], (unsigned)B.nby[b] * (unsigned)(bx1 - bx0));
-    B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b] * (bx1 - bx0);
+    B.rows[b] = (bx1 - bx0) * (y1 - y0);
+    B.nby[b] = (B.rows[b] + TY * RW - 1) / (TY * RW);
+    B.dnbx[b] = make_fastdiv((unsigned)B.nbx[b], (unsigned)B.nbx[b] * B.nby[b]);
+    B.drow[b] = make_fastdiv((unsigned)(y1 - y0), (unsigned)(B.nby[b] * TY * RW));
+    B.off[b + 1] = B.off[b] + B.nbx[b] * B.nby[b];
   };
   const int nx = s->n[0], ny = s->n[1], nz = s->n[2];
   // classes: the x range of the lean region holds no x-slab cell, no wall plane and (adjoint) no cell whose x

@@ -55,8 +55,9 @@ struct BoxList {
   int cls[6];
   int G[6], RW[6];
   unsigned ginv[6];        // (lane * ginv) >> 16 == lane / G for lane < 32
-  int nbx[6], nby[6];      // blocks along z and along y per x plane
-  FastDiv dnbx[6], dnby[6];
+  int nbx[6], nby[6];      // blocks along z; blocks along the flattened (x plane, y row) index
+  int rows[6];             // (x planes) * (y rows) of the box
+  FastDiv dnbx[6], drow[6];   // division by nbx; by the number of y rows per plane
   int off[7];
 };
 __device__ __forceinline__ unsigned fast_div(unsigned x, const FastDiv f) { return f.d == 1u ? x : __umulhi(x, f.mul); }

@@ -15,8 +15,9 @@ namespace fdtd {
 
 constexpr int TY = 8;
 
-// block / thread -> box b and (i, j, first k) inside the box list of a GENERAL kernel.  One x plane per block;
-// a warp covers G z-groups x RW rows of its box (thin z slabs pack several rows into one warp).
+// block / thread -> box b and (i, j, first k) inside the box list of a GENERAL kernel.  The (x plane, y row) pairs of a box
+// are numbered consecutively and cut into blocks of TY * RW rows, so that thin boxes (a y slab has only P rows per plane,
+// a z slab packs RW rows into a warp) leave no half-empty block per plane; a warp covers G z-groups x RW rows.
 template <int V>
 __device__ __forceinline__ bool box_decode(const BoxList& B, int& b, int& i, int& j, int& k0) {
   const unsigned blk = blockIdx.x;
@@ -24,16 +25,16 @@ __device__ __forceinline__ bool box_decode(const BoxList& B, int& b, int& i, int
 #pragma unroll
   for (int g = 1; g < 6; ++g) b += (g < B.nb && blk >= (unsigned)B.off[g]);
   const unsigned local = blk - B.off[b];
-  const unsigned t = fast_div(local, B.dnbx[b]);
-  const unsigned bx = local - t * B.nbx[b];
-  const unsigned bz = fast_div(t, B.dnby[b]);
-  const unsigned by = t - bz * B.nby[b];
+  const unsigned by = fast_div(local, B.dnbx[b]);          // block along the flattened rows
+  const unsigned bx = local - by * B.nbx[b];               // block along z
   const int G = B.G[b], RW = B.RW[b];
   const int yl = (int)((threadIdx.x * B.ginv[b]) >> 16), zl = (int)threadIdx.x - yl * G;
-  j = B.lo[b][1] + ((int)by * TY + (int)threadIdx.y) * RW + yl;
+  const unsigned row = (by * TY + threadIdx.y) * RW + yl;  // flattened (plane, row) index inside the box
+  const unsigned pl = fast_div(row, B.drow[b]);
+  i = B.lo[b][0] + (int)pl;
+  j = B.lo[b][1] + (int)(row - pl * B.drow[b].d);
   k0 = B.lo[b][2] + ((int)bx * G + zl) * V;
-  i = B.lo[b][0] + (int)bz;
-  return yl < RW && j < B.hi[b][1] && k0 < B.hi[b][2];
+  return yl < RW && row < (unsigned)B.rows[b] && k0 < B.hi[b][2];
 }
 
 // A general kernel body is instantiated per box class: HX / HY say whether CPML terms of the x / y axis (and, for
