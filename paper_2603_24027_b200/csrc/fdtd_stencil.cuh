@@ -13,7 +13,10 @@
 
 namespace fdtd {
 
-constexpr int TY = 8;
+#ifndef FDTD_TY
+#define FDTD_TY 4
+#endif
+constexpr int TY = FDTD_TY;   // rows per block, one warp per row (4: measured best of 2 / 4 / 8 / 16 on C2, C3, C4)
 
 // block / thread -> box b and (i, j, first k) inside the box list of a GENERAL kernel.  The (x plane, y row) pairs of a box
 // are numbered consecutively and cut into blocks of TY * RW rows, so that thin boxes (a y slab has only P rows per plane,
