@@ -279,8 +279,9 @@ def run_gpu(args, rank, world):
                 "frac": kernels[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch (all kernels of the group), ncu --set full, "
                                   "profiles/r01c_full.md" if (args.workload, dom) in NCU_TRAFFIC else None,
-                "how": "kernel timed alone: 20 back-to-back launches between CUDA events on the library's stream after 3 warm-up "
-                       "launches; achieved = algorithmic bytes per launch (DESIGN.md Roofline) / mean launch time",
+                "how": "kernel group timed alone (its lean and general kernel side by side, as in the step): 20 back-to-back launches "
+                       "between CUDA events on the library's stream after 3 warm-up launches; achieved = algorithmic bytes per "
+                       "launch (DESIGN.md Roofline) / mean launch time",
                 "launch_us": kernels[dom]["us"], "algo_bytes": kernels[dom]["algo_bytes"]}
     # whole-pass effective bandwidth: algorithmic bytes of all stencil launches of one step / measured time
     fwd_names = ("fwd_e", "fwd_h", "fwd_fused", "fwd_fused_slabs")

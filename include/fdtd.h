@@ -144,9 +144,12 @@ fdtd_status fdtd_set_eps(fdtd_sim*, const float* eps_dev);
 fdtd_status fdtd_reset(fdtd_sim*);
 /* Replay runs of k steps through CUDA graphs (default 1 = on). */
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
-/* Fused marching kernels (two dependent half-steps per pass over the interior): mode -1 = chosen
- * by grid size (default), 0 = never, 1 = whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).
- * xseg = planes marched per block (0 keeps the current value).  Results are bit-identical in every mode. */
+/* Fused marching kernels (two dependent half-steps per pass over the interior): mode -1 (default) =
+ * forward run fused on large grids (>= 12 tiles per SM, e.g. 512^3), reverse primal never; 0 = never; 1 = forward AND
+ * reverse primal whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per
+ * block (0 keeps the current value).  Results are bit-identical in every mode (sources that overlap on one cell excepted
+ * in the fused reverse run: they are summed before being subtracted).  With the fused reverse run the fields left after
+ * fdtd_reverse are state 0 on the interior only. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
 /* 1 if fdtd_forward(nsteps) would take the fused path with the current settings (after fdtd_set_workspace), else 0. */
 int fdtd_uses_fused(const fdtd_sim*, int nsteps);

@@ -1290,14 +1290,24 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
   if (id >= 9 && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
   s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
+  // a split half-step is timed in the launch configuration of the real step: lean and general kernel side by side
+  auto split_pair = [&](int which) {
+    const bool was = s->parallel;
+    s->parallel = s->aux[0] != nullptr;
+    fork(s, 2);
+    on(s, 1); launch_gen(s, which, 0);
+    on(s, 0); launch_lean(s, which);
+    join(s, 2);
+    s->parallel = was;
+  };
   auto once = [&]() {
     switch (id) {
-      case 0: launch_fwd_e(s); break;
-      case 1: launch_fwd_h(s); break;
+      case 0: split_pair(0); break;
+      case 1: split_pair(1); break;
       case 2: launch_inv_h(s); break;
-      case 3: launch_split(s, 2, 0); break;
+      case 3: split_pair(2); break;
       case 4: launch_inv_e(s); launch_grad(s); break;
-      case 5: launch_split(s, 3, 0); break;
+      case 5: split_pair(3); break;
       case 6: launch_record(s, s->nsteps, nullptr, 2); break;
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
       case 8: launch_inject(s, mrev, nullptr, 0, 0); break;
