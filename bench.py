@@ -225,7 +225,7 @@ def run_gpu(args, rank, world):
         sim.set_eps_host(eps_host)
         sim.forward_host(w.nsteps, w.sources, w.store_dtype, w.k, mon_host)
         L, d = W.loss_and_cotangent(w, mon_host.numpy(), extra)
-        dmon_host.copy_(torch.from_numpy(d.astype(np.float32)))
+        dmon_host.copy_(torch.from_numpy(np.ascontiguousarray(d, dtype=np.float32)))
         sim.reverse_host(dmon_host, W.LINEAR, grad_host)
         return L
     e2e_step()

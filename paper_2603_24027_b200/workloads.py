@@ -179,16 +179,23 @@ BY_NAME = {"C1": c1, "C2": c2, "C3": c3, "C4": c4, "tiny": tiny}
 # E and H are taken as stored (co-indexed, half a step apart): synthetic objectives (R19).
 # ----------------------------------------------------------------------------------------------------
 def loss_and_cotangent(w: Workload, mon: np.ndarray, extra: Optional[dict] = None):
-    mon = np.asarray(mon, dtype=np.float64)
+    mon = np.asarray(mon)
+    # float32 records (the CUDA path's own output) keep their type where the cotangent is a copy / sign flip / doubling of
+    # the record (exact in float32): no 8-byte copy of a 30 MB record on the host.  Sums are accumulated in float64.
+    if not (mon.dtype == np.float32 and w.loss in ("final_E2", "flux_x")):
+        mon = mon.astype(np.float64, copy=False)
     assert mon.shape == w.monitor_shape(), (mon.shape, w.monitor_shape())
-    d = np.zeros_like(mon)
+    d = np.empty_like(mon) if w.loss == "flux_x" else np.zeros_like(mon)   # flux_x fills every component
     if w.loss == "final_E2":                       # L = sum_c sum_plane E_c(T)^2
-        L = float(np.sum(mon[-1] ** 2))
+        L = float(np.sum(mon[-1].astype(np.float64) ** 2))
         d[-1] = 2.0 * mon[-1]
     elif w.loss == "flux_x":                       # mask Ey,Ez,Hy,Hz -> record order (Ey,Ez,Hy,Hz); L = -sum (Ey*Hz - Ez*Hy)
         ey, ez, hy, hz = mon[:, 0], mon[:, 1], mon[:, 2], mon[:, 3]
-        L = float(-np.sum(ey * hz - ez * hy))
-        d[:, 0], d[:, 1], d[:, 2], d[:, 3] = -hz, hy, ez, -ey
+        L = float(-(np.einsum("mxyz,mxyz->", ey, hz, dtype=np.float64) - np.einsum("mxyz,mxyz->", ez, hy, dtype=np.float64)))
+        np.negative(hz, out=d[:, 0])
+        d[:, 1] = hy
+        d[:, 2] = ez
+        np.negative(ey, out=d[:, 3])
     elif w.loss == "pulse_shape":                  # a_m = sum A*Ey^m ; L = sum_m (a_m - T_m)^2
         A = np.asarray(w.extra["A"], dtype=np.float64).reshape(mon.shape[2:])
         a = np.tensordot(mon[:, 0], A, axes=3)
