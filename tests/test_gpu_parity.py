@@ -380,6 +380,46 @@ def test_c2_shaped_short_run_sampled_parity():
     assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
 
 
+def test_c3_shaped_short_run_sampled_parity():
+    """BASELINE.json configs[2] grid and launch configuration (256x256x128, P = 16, float16, k = 8, pulse-shape loss) on a
+    run short enough for the oracle.  Monitor and design box are moved next to the source plane so that field, cotangent
+    and gradient are non-zero after 40 steps; fields compared on sampled planes, gradient on the whole design box."""
+    w = W.c3(nsteps=40)
+    w = dataclasses.replace(w, design=((26, 108, 54), (58, 149, 73)), monitor=((30, 108, 54), (31, 149, 73), 0b000010))
+    o = oracle_gradient(w, 32, w.store_dtype, w.k)
+    g = gpu_gradient(w, w.store_dtype, w.k)
+    f_err, g_err = _report("C3-shaped 40 steps", g, o)
+    assert np.abs(o["grad"]).max() > 0
+    for sl in (np.s_[:, 27], np.s_[:, :, 128], np.s_[:, :, :, 63]):
+        assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    assert g["sim"].store_bytes() == o["sim"].store_bytes()
+
+
+def test_c4_shaped_fused_launch_configuration_parity():
+    """BASELINE.json configs[3] shape (multi-slab eps, 8x8 dipole array, bf16 k = 4) on a 320^3 grid, the smallest on which
+    the library picks, by itself, the launch configuration bench.py times on 512^3 (fused forward marching kernel beside
+    the slab kernels).  Design box and monitor plane moved next to the dipole plane so that 12 steps give a non-zero
+    gradient; fields on sampled planes, gradient on the whole design box, every store slot byte for byte."""
+    w = W.c4(nsteps=12, n=320)
+    w = dataclasses.replace(w, design=((80, 80, 20), (240, 240, 44)), monitor=((80, 80, 34), (240, 240, 35), 0b000111))
+    s = gpu_sim(w)
+    s.set_workspace(w.nsteps, w.store_dtype, w.k)
+    assert s.uses_fused(w.nsteps)
+    g = gpu_gradient(w, w.store_dtype, w.k, sim=s)
+    o = oracle_gradient(w, 32, w.store_dtype, w.k)
+    f_err, g_err = _report("C4-shaped 320^3, 12 steps", g, o)
+    assert np.abs(o["grad"]).max() > 0
+    for sl in (np.s_[:, 128], np.s_[:, :, 17], np.s_[:, :, :, 30], np.s_[:, :, :, 303]):
+        assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    s.forward(w.nsteps, w.sources, w.store_dtype, w.k)
+    of = make_oracle(w, 32)
+    of.forward(w.nsteps, w.store_dtype, w.k)
+    for j in range(of.num_slots()):
+        assert np.array_equal(s.slot(j, w.store_dtype)[0].cpu().numpy(), of.slot(j, w.store_dtype)[0]), j
+
+
 def test_final_state_cotangent_box_and_get_box():
     """dL/dfinal given as a box cotangent (fdtd_cotangent) instead of a monitor cotangent gives the same gradient."""
     import torch
