@@ -25,7 +25,8 @@
 // Pin status (see tests/test_oracle_*.py): Yee update -> discrete dispersion closed form; energy
 // invariant; forward/reverse round trip; adjoint -> dot-product test and store-all back-propagation;
 // gradient -> central finite differences (f64); codec -> exhaustive + torch / ml_dtypes / numpy casts;
-// interpolation -> polynomial exactness and sinusoid error bound; dt -> the paper's printed value.
+// interpolation -> polynomial exactness and sinusoid error bound; dt -> the paper's printed value;
+// tangential-only store (store_mode 1) -> inner interior back to state 0 and gradient = store-all back-propagation.
 // CPML constants: PARITY UNPINNED against the paper (it prints none); pinned only by "sigma=0 reduces
 // to plain Yee" and a reflection bound.
 //
