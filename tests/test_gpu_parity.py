@@ -420,6 +420,35 @@ def test_c4_shaped_fused_launch_configuration_parity():
         assert np.array_equal(s.slot(j, w.store_dtype)[0].cpu().numpy(), of.slot(j, w.store_dtype)[0]), j
 
 
+@pytest.mark.parametrize("fused", [0, 1])
+def test_second_forward_call_extends_the_run(fused):
+    """fdtd_forward from the CURRENT state (no reset): a 30-step run followed by a 22-step run (sources replayed from their
+    first sample, store recorded anew) and its reverse run, against the oracle doing the same — in the two-kernel and in
+    the fused configuration (whose first half-step then starts from non-zero fields in either buffer)."""
+    import torch
+    w = mid_workload(nsteps=30, dtype=W.BF16, k=4)
+    o = make_oracle(w, 32)
+    o.forward(30, W.BF16, 4)
+    o.forward(22, W.BF16, 4)
+    mon_o = o.monitor_record()
+    w2 = dataclasses.replace(w, nsteps=22)
+    L, d = W.loss_and_cotangent(w2, mon_o)
+    of = o.fields()
+    og = o.reverse(None, d, orc.LINEAR)
+    s = gpu_sim(w)
+    s.set_fused(fused, 6)
+    s.forward(30, w.sources, W.BF16, 4)
+    mon = s.forward(22, w.sources, W.BF16, 4, reset=False)
+    assert np.array_equal(s.fields().cpu().numpy().astype(np.float64), of)
+    assert np.array_equal(mon.cpu().numpy().astype(np.float64), mon_o)
+    g = s.reverse(None, torch.from_numpy(d.astype(np.float32)).cuda(), W.LINEAR).cpu().numpy().astype(np.float64)
+    assert rel_l2(g, og) <= GRAD_TOL
+    P = w.pml
+    interior = (slice(None),) + tuple(slice(P, n - P) for n in w.shape)
+    peak = np.abs(of).max()
+    assert np.abs((s.fields().cpu().numpy().astype(np.float64) - o.fields())[interior]).max() <= 1e-5 * peak
+
+
 def test_final_state_cotangent_box_and_get_box():
     """dL/dfinal given as a box cotangent (fdtd_cotangent) instead of a monitor cotangent gives the same gradient."""
     import torch
