@@ -16,14 +16,21 @@ namespace fdtd {
 #ifndef FDTD_TY
 #define FDTD_TY 4
 #endif
+#ifndef FDTD_SWEEP_FLIP
+#define FDTD_SWEEP_FLIP 1
+#endif
+constexpr bool SWEEP_FLIP = FDTD_SWEEP_FLIP != 0;
 constexpr int TY = FDTD_TY;   // rows per block, one warp per row (4: measured best of 2 / 4 / 8 / 16 on C2, C3, C4)
 
 // block / thread -> box b and (i, j, first k) inside the box list of a GENERAL kernel.  The (x plane, y row) pairs of a box
 // are numbered consecutively and cut into blocks of TY * RW rows, so that thin boxes (a y slab has only P rows per plane,
 // a z slab packs RW rows into a warp) leave no half-empty block per plane; a warp covers G z-groups x RW rows.
-template <int V>
+// FLIP: the kernel walks its blocks in the opposite order.  The H-type half-steps (forward H, adjoint of E, inverse E) sweep the
+// grid downwards and the E-type ones upwards, so that each phase starts on the planes the previous phase touched last and
+// finds them in L2 (an LRU cache swept cyclically by a working set larger than itself hits almost never).
+template <int V, bool FLIP = false>
 __device__ __forceinline__ bool box_decode(const BoxList& B, int& b, int& i, int& j, int& k0) {
-  const unsigned blk = blockIdx.x;
+  const unsigned blk = FLIP ? (unsigned)B.off[B.nb] - 1u - blockIdx.x : blockIdx.x;
   b = 0;
 #pragma unroll
   for (int g = 1; g < 6; ++g) b += (g < B.nb && blk >= (unsigned)B.off[g]);
@@ -346,7 +353,7 @@ __global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d
   const int klo = P + 1, khi = nz - P - 1;
   const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
   const int j = P + 1 + blockIdx.y * TY + threadIdx.y;
-  const int i = P + 1 + blockIdx.z;
+  const int i = SWEEP_FLIP ? nx - P - 2 - (int)blockIdx.z : P + 1 + (int)blockIdx.z;
   if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
@@ -759,7 +766,7 @@ template <int V>
 __global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B,
                                                    const __grid_constant__ FieldIO io) {
   int b, i, j, k0;
-  if (!box_decode<V>(B, b, i, j, k0)) return;
+  if (!box_decode<V, SWEEP_FLIP>(B, b, i, j, k0)) return;
   FDTD_CLASS_DISPATCH(gen_h_body, d, i, j, k0, io)
 }
 template <int V>
@@ -771,7 +778,7 @@ __global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ D
 template <int V>
 __global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
   int b, i, j, k0;
-  if (!box_decode<V>(B, b, i, j, k0)) return;
+  if (!box_decode<V, SWEEP_FLIP>(B, b, i, j, k0)) return;
   FDTD_CLASS_DISPATCH(gen_adj_e_body, d, i, j, k0, pb)
 }
 
@@ -780,11 +787,11 @@ __global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ D
 // applies, and — for the adjoint — no neighbour W term either).  Grid: x = z groups, y = row tiles, z = planes.
 // Same canonical arithmetic as the general kernels (R3), so results are bit-identical to them.
 // ---------------------------------------------------------------------------------------------------------
-template <int V>
+template <int V, bool FLIP = false>
 __device__ __forceinline__ bool lean_decode(const Region& r, int& i, int& j, int& k0) {
   k0 = r.lo[2] + (blockIdx.x * 32 + threadIdx.x) * V;
   j = r.lo[1] + blockIdx.y * TY + threadIdx.y;
-  i = r.lo[0] + blockIdx.z;
+  i = FLIP ? r.hi[0] - 1 - (int)blockIdx.z : r.lo[0] + (int)blockIdx.z;
   return k0 < r.hi[2] && j < r.hi[1];
 }
 
@@ -824,7 +831,7 @@ __global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ 
 template <int V>
 __global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
   int i, j, k0;
-  if (!lean_decode<V>(r, i, j, k0)) return;
+  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
@@ -850,7 +857,7 @@ __global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev 
 template <int V>
 __global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
   int i, j, k0;
-  if (!lean_decode<V>(r, i, j, k0)) return;
+  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ce = ldv<V>(d.ce + q), ce_xp = ldv<V>(d.ce + q + sx), ce_yp = ldv<V>(d.ce + q + sy);
