@@ -86,6 +86,8 @@ struct fdtd_sim {
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 16;           // planes per block of the fused marching kernels
+  int zalign = 0;          // z alignment (cells) of the lean regions, chosen at create: 32 (128-byte lines) on grids that stream
+                           // from HBM, 16 on grids that live in L2 (more cells for the slower general kernels otherwise)
   int store_mode = 0;      // 0: six components per face (R6); 1: tangential only (fdtd_set_store_mode)
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
@@ -290,7 +292,14 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
       case 4: lo = P + 1; hi = n - P; break;                          // fused-path E: layer P joins the slab boxes
       default: lo = P + 1; hi = n - P - 1; break;                     // fused-path H: layers P and n-P-1 join them
     }
-    if (a == 2) { lo = (lo + V - 1) / V * V; hi = hi / V * V; }
+    if (a == 2) {
+      // z range of the lean region: whole groups of V cells, and (zalign > V) whole 128-byte lines, so that neither the lean
+      // nor the z-slab kernels fetch half-used lines (a row of the lean region then starts and ends on a line boundary)
+      const int za = (which < 4 && s->zalign > V && n % s->zalign == 0) ? s->zalign : V;
+      int lo2 = (lo + za - 1) / za * za, hi2 = hi / za * za;
+      if (hi2 - lo2 < za) { lo2 = (lo + V - 1) / V * V; hi2 = hi / V * V; }
+      lo = lo2; hi = hi2;
+    }
     full.lo[a] = lo; full.hi[a] = hi;
   }
   const bool full_lean = full.hi[0] > full.lo[0] && full.hi[1] > full.lo[1] && full.hi[2] > full.lo[2];
@@ -990,6 +999,17 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   s->cur = s->stream;
   if (const char* e = std::getenv("FDTD_FUSE")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_mode = v; }
   if (const char* e = std::getenv("FDTD_FUSE_REV")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_rev_mode = v; }
+  {
+    // DRAM is fetched in whole 128-byte lines: a lean region that starts 64 bytes into a row (P = 16) costs the lean AND the
+    // z-slab kernel a half-used line per row end (measured on C3: reads 33 % above the arrays' size, profiles/r01d_c3.md)
+    int dev = 0, l2 = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    cudaGetLastError();
+    const double fwd_bytes = 7.0 * 4.0 * (double)nx * ny * nz;
+    s->zalign = (l2 > 0 && fwd_bytes > 1.5 * (double)l2) ? 32 : 16;
+  }
+  if (const char* e = std::getenv("FDTD_ZALIGN")) s->zalign = atoi(e);
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
