@@ -83,13 +83,13 @@ def whole_job_value(cells, nsteps, steps, world, total_ms):
 
 
 # DRAM bytes per launch of a kernel group (read + write, summed over the group's kernels) from the committed ncu --set full
-# captures (profiles/r01d_c2.md, r01d_c3.md, r01c_full.md): what roofline.traffic reports beside the algorithmic bytes.  ncu flushes the caches
+# captures (profiles/r01d_c2.md, r01e_c3_c2.md, r01c_full.md): what roofline.traffic reports beside the algorithmic bytes.  ncu flushes the caches
 # between launches, so on C2 (working set of the order of the L2) arrays that stay in L2 do not appear as writes.
 NCU_TRAFFIC = {
     ("C2", "fwd_e"): 88.2e6, ("C2", "fwd_h"): 76.7e6, ("C2", "inv_h"): 32.2e6, ("C2", "adj_h"): 76.6e6,
     ("C2", "grad_inv_e"): 44.3e6, ("C2", "adj_e"): 88.4e6,
-    ("C3", "fwd_e"): 439.8e6, ("C3", "fwd_h"): 383.5e6, ("C3", "inv_h"): 175.6e6, ("C3", "adj_h"): 391.8e6,
-    ("C3", "grad_inv_e"): 231.8e6, ("C3", "adj_e"): 447.2e6,
+    ("C3", "fwd_e"): 364.7e6, ("C3", "fwd_h"): 314.7e6, ("C3", "inv_h"): 175.6e6, ("C3", "adj_h"): 335.2e6,
+    ("C3", "grad_inv_e"): 231.8e6, ("C3", "adj_e"): 382.7e6,
     ("C4", "fwd_fused"): 6112.8e6, ("C4", "fwd_fused_slabs"): 3242.1e6,
 }
 
@@ -280,7 +280,7 @@ def run_gpu(args, rank, world):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": kernels[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
                 "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch (all kernels of the group), ncu --set full, "
-                                  "profiles/r01d_c2.md, r01d_c3.md, r01c_full.md" if (args.workload, dom) in NCU_TRAFFIC else None,
+                                  "profiles/r01d_c2.md, r01e_c3_c2.md, r01c_full.md" if (args.workload, dom) in NCU_TRAFFIC else None,
                 "how": "kernel group timed alone (its lean and general kernel side by side, as in the step): 20 back-to-back launches "
                        "between CUDA events on the library's stream after 3 warm-up launches; achieved = algorithmic bytes per "
                        "launch (DESIGN.md Roofline) / mean launch time",
