@@ -26,7 +26,8 @@
 // invariant; forward/reverse round trip; adjoint -> dot-product test and store-all back-propagation;
 // gradient -> central finite differences (f64); codec -> exhaustive + torch / ml_dtypes / numpy casts;
 // interpolation -> polynomial exactness and sinusoid error bound; dt -> the paper's printed value;
-// tangential-only store (store_mode 1) -> inner interior back to state 0 and gradient = store-all back-propagation.
+// tangential-only store (store_mode 1) -> inner interior back to state 0 and gradient = store-all back-propagation;
+// micro-scaled e4m3 (dtype 5) -> ml_dtypes float8_e4m3fn / float8_e8m0fnu casts, error bound, scale equivariance.
 // CPML constants: PARITY UNPINNED against the paper (it prints none); pinned only by "sigma=0 reduces
 // to plain Yee" and a reflection bound.
 //
@@ -53,7 +54,9 @@ enum Flavour { IEEE = 0, FN = 1, FNUZ = 2 };
 struct Fmt { int ebits, mbits, bias, flavour; };
 
 // store dtype ids (0..3 are the product's; >= 10 are the paper's unscaled float8 flavours, oracle only)
-enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3_SCALED = 3, DT_NATIVE = 4,
+// 5 = micro-scaled e4m3: blocks of 32 values share one power-of-two scale (SURVEY 8(f)-1 "finer scale granularity";
+// DESIGN.md reading R20)
+enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3_SCALED = 3, DT_NATIVE = 4, DT_E4M3_MX32 = 5,
        DT_E4M3B11FNUZ = 10, DT_E5M2FNUZ = 11, DT_E4M3FNUZ = 12, DT_E4M3 = 13, DT_E3M4 = 14, DT_E4M3FN = 15 };
 
 bool fmt_of(int dtype, Fmt* f) {
@@ -61,6 +64,7 @@ bool fmt_of(int dtype, Fmt* f) {
     case DT_F16:         *f = {5, 10, 15, IEEE};  return true;
     case DT_BF16:        *f = {8, 7, 127, IEEE};  return true;
     case DT_E4M3_SCALED:
+    case DT_E4M3_MX32:
     case DT_E4M3FN:      *f = {4, 3, 7, FN};      return true;
     case DT_E4M3B11FNUZ: *f = {4, 3, 11, FNUZ};   return true;
     case DT_E5M2FNUZ:    *f = {5, 2, 16, FNUZ};   return true;
@@ -161,6 +165,38 @@ void encode_slice(int dtype, const float* x, size_t n, uint8_t* out, float* scal
     return;
   }
   for (size_t i = 0; i < n; ++i) put_code(out, i, eb, fmt_encode(f, (double)x[i]));
+}
+
+// Micro-scaled e4m3 (DT_E4M3_MX32; PAPER.md:35 cast to 8 bits, SURVEY 8(f)-1 finer scale granularity; reading R20).
+// The slice is cut into blocks of 32 consecutive values (the last one may be shorter).  Per block:
+//   amax = max|x|;  X = clamp(floor(log2 amax) - 8, -127, 127)  (8 = exponent of e4m3's largest binade; amax = 0 -> X = -127);
+//   code_i = e4m3fn_rne(clamp(x_i * 2^-X, -448, 448));  the block scale is stored as one byte X + 127.
+// Decoding: value = e4m3fn(code) * 2^X.  Both multiplications are by powers of two and exact.
+const int MX_BLOCK = 32;
+size_t mx_blocks(size_t n) { return (n + MX_BLOCK - 1) / MX_BLOCK; }
+int mx_block_exponent(const float* x, size_t n) {
+  float amax = 0.0f;
+  for (size_t i = 0; i < n; ++i) amax = std::max(amax, std::fabs(x[i]));
+  if (!(amax > 0.0f)) return -127;
+  int ex;  std::frexp((double)amax, &ex);            // amax = m * 2^ex, m in [0.5,1)  =>  floor(log2 amax) = ex-1
+  return std::min(127, std::max(-127, ex - 1 - 8));
+}
+void encode_slice_mx(const float* x, size_t n, uint8_t* codes, uint8_t* bscale) {
+  Fmt f;  fmt_of(DT_E4M3_MX32, &f);
+  for (size_t b = 0; b < mx_blocks(n); ++b) {
+    const size_t i0 = b * MX_BLOCK, i1 = std::min(n, i0 + MX_BLOCK);
+    const int X = mx_block_exponent(x + i0, i1 - i0);
+    bscale[b] = (uint8_t)(X + 127);
+    for (size_t i = i0; i < i1; ++i) {
+      double y = std::ldexp((double)x[i], -X);
+      y = std::min(448.0, std::max(-448.0, y));
+      codes[i] = (uint8_t)fmt_encode(f, y);
+    }
+  }
+}
+float decode_value_mx(const uint8_t* codes, const uint8_t* bscale, size_t i) {
+  Fmt f;  fmt_of(DT_E4M3_MX32, &f);
+  return (float)std::ldexp(fmt_decode(f, codes[i]), (int)bscale[i / MX_BLOCK] - 127);
 }
 
 // "We convert the stored values back to the larger bit-widths".
@@ -359,6 +395,17 @@ template <class T> struct Sim {
   int ncomp_stored(int f) const { int c = 0; for (int comp = 0; comp < 6; ++comp) c += stored(f, comp); return c; }
   int nslices() const { int c = 0; for (int f = 0; f < 6; ++f) c += ncomp_stored(f); return c; }
   size_t slot_values() const { size_t s = 0; for (int f = 0; f < 6; ++f) s += ncomp_stored(f) * face_size(f); return s; }
+  // micro-scaled store: a slot is [codes: slot_values bytes][block scales: slot_blocks bytes]; the blocks of a slice follow
+  // the slices' own order
+  size_t face_blocks(int f) const { return mx_blocks(face_size(f)); }
+  size_t slot_blocks() const { size_t s = 0; for (int f = 0; f < 6; ++f) s += ncomp_stored(f) * face_blocks(f); return s; }
+  size_t block_offset(int f, int comp) const {
+    size_t o = 0;
+    for (int g = 0; g < f; ++g) o += ncomp_stored(g) * face_blocks(g);
+    int rank = 0;
+    for (int c = 0; c < comp; ++c) rank += stored(f, c);
+    return o + rank * face_blocks(f);
+  }
   size_t slice_offset(int f, int comp) const {
     size_t o = 0;
     for (int g = 0; g < f; ++g) o += ncomp_stored(g) * face_size(g);
@@ -381,7 +428,7 @@ template <class T> struct Sim {
   void record(int m) {
     Slot s;  s.step = m;
     const int eb = elem_bytes(dtype, sizeof(T));
-    s.data.assign(slot_values() * eb, 0);
+    s.data.assign(slot_values() * eb + (dtype == DT_E4M3_MX32 ? slot_blocks() : 0), 0);
     for (int f = 0; f < 6; ++f) for (int comp = 0; comp < 6; ++comp) {
       s.scale[f * 6 + comp] = 1.0f;
       if (!stored(f, comp)) continue;
@@ -395,7 +442,8 @@ template <class T> struct Sim {
       } else {
         std::vector<float> tmp(fs);
         for (int u = 0; u < du; ++u) for (int v = 0; v < dv; ++v) tmp[(size_t)u * dv + v] = (float)F[face_cell(f, u, v)];
-        encode_slice(dtype, tmp.data(), fs, &s.data[off * eb], &s.scale[f * 6 + comp]);
+        if (dtype == DT_E4M3_MX32) encode_slice_mx(tmp.data(), fs, &s.data[off], &s.data[slot_values() + block_offset(f, comp)]);
+        else encode_slice(dtype, tmp.data(), fs, &s.data[off * eb], &s.scale[f * 6 + comp]);
       }
     }
     slots.push_back(std::move(s));
@@ -405,6 +453,7 @@ template <class T> struct Sim {
   template <class X> X slot_value(const Slot& s, int f, int comp, size_t e) const {
     size_t off = slice_offset(f, comp);
     if (dtype == DT_NATIVE) { T v; std::memcpy(&v, &s.data[(off + e) * sizeof(T)], sizeof(T)); return (X)v; }
+    if (dtype == DT_E4M3_MX32) return (X)decode_value_mx(&s.data[off], &s.data[slot_values() + block_offset(f, comp)], e);
     return (X)decode_value(dtype, &s.data[off * elem_bytes(dtype, 4)], e, s.scale[f * 6 + comp]);
   }
   template <class X> X fetch_x(int nstate, int f, int comp, size_t e, int interp) const {
@@ -824,6 +873,8 @@ int orc_slot_step(void* h, int j) { int r = 0; DISPATCH(h, r = s.slots[j].step);
 void orc_get_slot(void* h, int j, uint8_t* data, float* scales) {
   DISPATCH(h, { std::memcpy(data, s.slots[j].data.data(), s.slots[j].data.size()); std::memcpy(scales, s.slots[j].scale, 36 * sizeof(float)); });
 }
+size_t orc_slot_bytes(void* h, int j) { size_t r = 0; DISPATCH(h, r = s.slots[j].data.size()); return r; }
+size_t orc_block_offset(void* h, int face, int comp) { size_t r = 0; DISPATCH(h, r = s.block_offset(face, comp)); return r; }
 size_t orc_slice_offset(void* h, int face, int comp) { size_t r = 0; DISPATCH(h, r = s.slice_offset(face, comp)); return r; }
 size_t orc_face_size(void* h, int face) { size_t r = 0; DISPATCH(h, r = s.face_size(face)); return r; }
 // value the reverse run would inject for (state, face, comp, element)
@@ -846,6 +897,8 @@ int orc_get_threads() { return omp_get_max_threads(); }
 // ---- standalone codec entry points ----
 int orc_elem_bytes(int dtype) { return elem_bytes(dtype, 4); }
 void orc_encode(int dtype, const float* x, size_t n, uint8_t* out, float* scale) { encode_slice(dtype, x, n, out, scale); }
+void orc_encode_mx(const float* x, size_t n, uint8_t* codes, uint8_t* bscale) { encode_slice_mx(x, n, codes, bscale); }
+void orc_decode_mx(const uint8_t* codes, const uint8_t* bscale, size_t n, float* out) { for (size_t i = 0; i < n; ++i) out[i] = decode_value_mx(codes, bscale, i); }
 void orc_decode(int dtype, const uint8_t* in, size_t n, float scale, float* out) { for (size_t i = 0; i < n; ++i) out[i] = decode_value(dtype, in, i, scale); }
 double orc_decode_code(int dtype, unsigned code) { Fmt f; if (!fmt_of(dtype, &f)) return 0; return fmt_decode(f, code); }
 unsigned orc_encode_value(int dtype, double x) { Fmt f; if (!fmt_of(dtype, &f)) return 0; return fmt_encode(f, x); }

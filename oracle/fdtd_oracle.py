@@ -18,6 +18,9 @@ from . import build as _build
 # store dtype ids (0..3 = the product's; 4 = "native", i.e. an uncompressed copy in the oracle's own
 # precision; >= 10 = the paper's unscaled float8 flavours)
 F32, F16, BF16, E4M3_SCALED, NATIVE = 0, 1, 2, 3, 4
+# 5 = micro-scaled e4m3: blocks of 32 values share a power-of-two scale, stored as one byte X + 127 after the codes
+E4M3_MX32 = 5
+MX_BLOCK = 32
 E4M3B11FNUZ, E5M2FNUZ, E4M3FNUZ, E4M3, E3M4, E4M3FN = 10, 11, 12, 13, 14, 15
 STORE_ALL, STORE_TANGENTIAL = 0, 1
 LINEAR, CUBIC = 0, 1
@@ -63,6 +66,12 @@ def lib():
     L.orc_slot_values.argtypes = [vp]
     L.orc_slot_step.argtypes = [vp, C.c_int]
     L.orc_get_slot.argtypes = [vp, C.c_int, C.c_void_p, C.c_void_p]
+    L.orc_slot_bytes.restype = C.c_size_t
+    L.orc_slot_bytes.argtypes = [vp, C.c_int]
+    L.orc_block_offset.restype = C.c_size_t
+    L.orc_block_offset.argtypes = [vp, C.c_int, C.c_int]
+    L.orc_encode_mx.argtypes = [C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p]
+    L.orc_decode_mx.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p]
     L.orc_slice_offset.restype = C.c_size_t
     L.orc_slice_offset.argtypes = [vp, C.c_int, C.c_int]
     L.orc_face_size.restype = C.c_size_t
@@ -231,12 +240,15 @@ class OracleSim:
         return lib().orc_slot_step(self._h, j)
 
     def slot(self, j, dtype):
-        """(raw bytes as uint8 array, 36 float32 scales) of stored slot j."""
-        eb = 4 if dtype == F32 else (self.prec // 8 if dtype == NATIVE else lib().orc_elem_bytes(dtype))
-        data = np.empty(self.slot_values() * eb, dtype=np.uint8)
+        """(raw bytes as uint8 array, 36 float32 scales) of stored slot j.  E4M3_MX32: the bytes are the slot_values codes
+        followed by the block-scale bytes (block_offset gives a slice's first block)."""
+        data = np.empty(lib().orc_slot_bytes(self._h, j), dtype=np.uint8)
         scales = np.empty(36, dtype=np.float32)
         lib().orc_get_slot(self._h, j, data.ctypes.data, scales.ctypes.data)
         return data, scales
+
+    def block_offset(self, face, comp):
+        return lib().orc_block_offset(self._h, face, comp)
 
     def slice_offset(self, face, comp):
         return lib().orc_slice_offset(self._h, face, comp)
@@ -290,6 +302,23 @@ def decode(dtype, codes, scale=1.0):
     n = codes.size // elem_bytes(dtype)
     out = np.empty(n, dtype=np.float32)
     lib().orc_decode(dtype, codes.ctypes.data, n, float(scale), out.ctypes.data)
+    return out
+
+
+def encode_mx(x):
+    """Micro-scaled e4m3 of one slice: (codes uint8 [n], block-scale bytes uint8 [ceil(n/32)], byte = X + 127)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    codes = np.empty(x.size, dtype=np.uint8)
+    bs = np.empty((x.size + MX_BLOCK - 1) // MX_BLOCK, dtype=np.uint8)
+    lib().orc_encode_mx(x.ctypes.data, x.size, codes.ctypes.data, bs.ctypes.data)
+    return codes, bs
+
+
+def decode_mx(codes, bscale):
+    codes = np.ascontiguousarray(codes, dtype=np.uint8)
+    bscale = np.ascontiguousarray(bscale, dtype=np.uint8)
+    out = np.empty(codes.size, dtype=np.float32)
+    lib().orc_decode_mx(codes.ctypes.data, bscale.ctypes.data, codes.size, out.ctypes.data)
     return out
 
 

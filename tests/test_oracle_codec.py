@@ -102,6 +102,92 @@ def test_scaled_e4m3_slice_codec():
     assert sc == 0.0 and not z.any() and not orc.decode(orc.E4M3_SCALED, z, sc).any()
 
 
+def test_microscaled_e4m3_slice_codec():
+    """DESIGN.md R20: blocks of 32 values, block scale 2^X with X = clamp(floor(log2 amax) - 8, -127, 127) stored as X + 127,
+    code = e4m3fn(clamp(x * 2^-X, +-448)).  References: ml_dtypes' float8_e8m0fnu (the scale byte) and float8_e4m3fn (the
+    element cast), torch's e4m3fn cast, and properties no formula-retyping can fake (error bound, scale equivariance, block
+    independence, ragged tail)."""
+    rng = np.random.default_rng(7)
+    n = 32 * 40 + 13                                                     # ragged last block
+    x = (rng.standard_normal(n) * np.exp(rng.uniform(-25, 6, n))).astype(np.float32)
+    x[64:96] = 0.0                                                       # an all-zero block
+    x[96:128] *= np.float32(1e-38)                                       # a block of f32 subnormals / tiny values
+    x[128] = np.float32(3.0e38)                                          # near the f32 maximum
+    x[160:192] = np.float32(2.0 ** -5) * np.arange(-16, 16, dtype=np.float32)   # exactly representable: must round-trip
+    codes, bs = orc.encode_mx(x)
+    assert codes.shape == (n,) and bs.shape == (41,)
+    assert not np.any((codes & 0x7F) == 0x7F)                            # never the NaN code
+    back = orc.decode_mx(codes, bs)
+    nb = len(bs)
+    pad = np.zeros(nb * 32, np.float32)
+    pad[:n] = x
+    amax = np.abs(pad).reshape(nb, 32).max(axis=1)
+    # the scale byte, read as ml_dtypes' e8m0: a power of two with  amax / 2^9 < scale <= amax / 2^8  (unless clamped)
+    scale = bs.view(ml_dtypes.float8_e8m0fnu).astype(np.float64)
+    assert np.array_equal(scale, 2.0 ** (bs.astype(np.int64) - 127))
+    nz = amax > 2.0 ** -118
+    assert np.all(scale[nz] * 2.0 ** 8 <= amax[nz]) and np.all(amax[nz] < scale[nz] * 2.0 ** 9)
+    assert np.all(bs[amax == 0] == 0) and np.all(bs[~nz] == 0)           # X clamps at -127
+    # elements: the library cast of the scaled, clamped value
+    y = np.clip(pad.astype(np.float64) / np.repeat(scale, 32), -448, 448).astype(np.float32)[:n]
+    assert np.array_equal(codes, y.astype(ml_dtypes.float8_e4m3fn).view(np.uint8))
+    assert np.array_equal(codes, torch.from_numpy(y).to(torch.float8_e4m3fn).view(torch.uint8).numpy())
+    assert np.array_equal(back.astype(np.float64), codes.view(ml_dtypes.float8_e4m3fn).astype(np.float64) * np.repeat(scale, 32)[:n])
+    # error bound: 3 mantissa bits -> 2^-4 relative (2^-3 where the value was clamped from (448, 512) * scale), or half
+    # the subnormal step 2^-10 * scale
+    sc_el = np.repeat(scale, 32)[:n]
+    err = np.abs(back.astype(np.float64) - x.astype(np.float64))
+    assert np.all(err <= np.maximum(2.0 ** -3 * np.abs(x.astype(np.float64)), 2.0 ** -10 * sc_el))
+    unclamped = np.abs(y) < 448
+    assert np.all(err[unclamped] <= np.maximum(2.0 ** -4 * np.abs(x[unclamped].astype(np.float64)), 2.0 ** -10 * sc_el[unclamped]))
+    assert np.array_equal(back[160:192], x[160:192]) and not back[64:96].any()
+    # the largest value of each block keeps at least its leading bit: never flushed
+    imax = np.abs(pad).reshape(nb, 32).argmax(axis=1) + 32 * np.arange(nb)
+    keep = imax[nz]
+    assert np.all(np.abs(np.pad(back, (0, nb * 32 - n))[keep]) >= 0.5 * np.abs(pad[keep]))
+    # power-of-two equivariance: x * 2^j -> same codes, scale byte + j
+    c2, b2 = orc.encode_mx((x[:64] * np.float32(2.0 ** 11)).astype(np.float32))
+    assert np.array_equal(c2, codes[:64]) and np.array_equal(b2.astype(int), bs[:2].astype(int) + 11)
+    # block independence: changing block 5 leaves every other block's bytes alone
+    x2 = x.copy()
+    x2[5 * 32:6 * 32] *= np.float32(1000.0)
+    c3, b3 = orc.encode_mx(x2)
+    other = np.ones(n, bool)
+    other[5 * 32:6 * 32] = False
+    assert np.array_equal(c3[other], codes[other]) and np.array_equal(np.delete(b3, 5), np.delete(bs, 5))
+    # a field-sized value next to a 10^6 times larger one in ANOTHER block survives (the per-slice scale would flush it, R13)
+    z = np.zeros(64, np.float32)
+    z[0], z[40] = 1.0, 1.0e-6
+    cz, bz = orc.encode_mx(z)
+    assert abs(orc.decode_mx(cz, bz)[40] / 1.0e-6 - 1) < 2.0 ** -4
+    cs, sc = orc.encode(orc.E4M3_SCALED, z)
+    assert orc.decode(orc.E4M3_SCALED, cs, sc)[40] == 0.0
+
+
+def test_microscaled_store_bytes_and_fetch():
+    """Slot = slot_values codes + one byte per block of 32 (per slice, ragged tail counted); fetch decodes through it."""
+    eps = np.ones((14, 13, 12))
+    s = orc.OracleSim(32, eps, 2, W.S)
+    wave = np.sin(0.3 * np.arange(24))
+    s.add_source(2, (6, 6, 6), (7, 7, 7), None, wave)
+    s.forward(24, orc.E4M3_MX32, 4)
+    blocks = sum(6 * ((s.face_size(f) + 31) // 32) for f in range(6))
+    assert s.store_bytes() == s.num_slots() * (s.slot_values() + blocks)
+    data, _ = s.slot(3, orc.E4M3_MX32)
+    assert data.size == s.slot_values() + blocks
+    f, comp = 4, 2
+    fs, off, bo = s.face_size(f), s.slice_offset(f, comp), s.block_offset(f, comp)
+    vals = orc.decode_mx(data[off:off + fs], data[s.slot_values() + bo:s.slot_values() + bo + (fs + 31) // 32])
+    assert np.array_equal(vals.astype(np.float64), s.fetch_face(12, f, comp))     # state 12 = slot 3, exact
+    assert np.abs(vals).max() > 0
+    # against the uncompressed run: within the codec's error bound of the true slice
+    t = orc.OracleSim(32, eps, 2, W.S)
+    t.add_source(2, (6, 6, 6), (7, 7, 7), None, wave)
+    t.forward(24, orc.F32, 4)
+    true = t.fetch_face(12, f, comp)
+    assert np.all(np.abs(vals - true) <= 2.0 ** -3 * np.abs(true) + 2.0 ** -9 * np.abs(true).max())
+
+
 def test_paper_formats_fail_by_underflow_unscaled():
     """PAPER.md:63 ranking has a cause the oracle reproduces: e4m3fnuz / e4m3 / e3m4 flush field-sized values
     (1e-3) to zero, e4m3b11fnuz / e5m2fnuz keep them."""
