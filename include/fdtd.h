@@ -42,6 +42,10 @@ typedef enum {
  * float32 absmax scale per (slot, face, component) slice — DESIGN.md R13/R14. */
 typedef enum {
   FDTD_F32 = 0, FDTD_F16 = 1, FDTD_BF16 = 2, FDTD_F8E4M3_SCALED = 3,
+  /* Micro-scaled E4M3 (SURVEY 8(f)-1 "finer scale granularity"; R20): every slice is cut into blocks of 32
+   * consecutive values that share one power-of-two scale 2^X, X = the smallest integer with amax * 2^-X <= 448 (clamped
+   * to [-127, 127]), stored as the byte X + 127 behind the slot's codes: slot = [slot_values codes][sum over slices of ceil(face/32) scale bytes]. */
+  FDTD_F8E4M3_MX32 = 5,
   /* The paper's own float8 flavours, cast WITHOUT a scale, exactly like an array astype: round to
    * nearest even, subnormals kept; a value above the largest finite one becomes NaN ("fn"/"fnuz": no infinities) or
    * inf (e4m3, e3m4).  e4m3b11fnuz with k = 16 is the paper's 64x configuration.  Software casts (no hardware cvt). */
@@ -102,7 +106,8 @@ fdtd_status fdtd_reverse(fdtd_sim*, const fdtd_cotangent* dL_dfinal, const float
                          float* grad_eps_dev);
 
 /* Bytes of the interface store of the last forward run, scales included:
- * nslots * (slot_values * sizeof(store_dtype) + (FDTD_F8E4M3_SCALED ? 36*4 : 0)); 0 before any forward. */
+ * nslots * (slot_values * sizeof(store_dtype) + (FDTD_F8E4M3_SCALED ? slices*4 : 0) + (FDTD_F8E4M3_MX32 ? blocks : 0));
+ * 0 before any forward. */
 size_t fdtd_store_bytes(const fdtd_sim*);
 
 /* ---------------------------------------------------------------------------------------------------------
@@ -165,6 +170,9 @@ fdtd_status fdtd_get_adjoint(fdtd_sim*, float* out_dev);
 int fdtd_num_slots(const fdtd_sim*);
 size_t fdtd_slot_values(const fdtd_sim*);
 fdtd_status fdtd_slot_ptr(const fdtd_sim*, int j, const void** data_dev, const float** scales_dev /* [36] */);
+/* Bytes one slot occupies at data_dev for the given store dtype (codes, plus the block-scale bytes of FDTD_F8E4M3_MX32;
+ * the float32 slice scales of FDTD_F8E4M3_SCALED live in scales_dev and are not counted).  0 for an unknown dtype. */
+size_t fdtd_slot_bytes(const fdtd_sim*, fdtd_dtype store_dtype);
 
 /* ---------------------------------------------------------------------------------------------------------
  * Host-buffer variants (end-to-end path): same computation, host<->device copies inside the call, synchronous.
@@ -182,11 +190,13 @@ fdtd_status fdtd_reverse_host(fdtd_sim*, const float* dmon_host, fdtd_interp int
  * quantise, dequantise and interpolate can be checked bit for bit on identical slices.
  * ------------------------------------------------------------------------------------------------------- */
 /* Encode one slice x_dev[n] (float32) to codes_dev[n * sizeof(dtype)]; scale_dev[1] receives the slice scale
- * (1 unless FDTD_F8E4M3_SCALED).  scratch_dev: one uint32 used for the absmax reduction. */
+ * (1 unless FDTD_F8E4M3_SCALED).  scratch_dev: one uint32 used for the absmax reduction.  FDTD_F8E4M3_MX32: codes_dev
+ * must hold n + ceil(n/32) bytes — the codes, then one scale byte per block of 32 values (the slot convention). */
 fdtd_status fdtd_codec_encode(fdtd_dtype dtype, const float* x_dev, size_t n, void* codes_dev, float* scale_dev,
                               unsigned* scratch_dev, void* cuda_stream);
 /* Dequantise and interpolate: out_dev[i] = value at (num/den) between slices 1 and 2 (linear: slices 1,2; cubic:
- * slices 0..3 = steps -1,0,1,2).  num == 0 returns slice 1 exactly.  scales[4] are HOST floats. */
+ * slices 0..3 = steps -1,0,1,2).  num == 0 returns slice 1 exactly.  scales[4] are HOST floats (ignored by
+ * FDTD_F8E4M3_MX32, whose block-scale bytes follow the n codes in each codes_dev[j]). */
 fdtd_status fdtd_codec_fetch(fdtd_dtype dtype, fdtd_interp interp, const void* const codes_dev[4],
                              const float scales[4], int num, int den, size_t n, float* out_dev, void* cuda_stream);
 

@@ -169,7 +169,8 @@ void encode_slice(int dtype, const float* x, size_t n, uint8_t* out, float* scal
 
 // Micro-scaled e4m3 (DT_E4M3_MX32; PAPER.md:35 cast to 8 bits, SURVEY 8(f)-1 finer scale granularity; reading R20).
 // The slice is cut into blocks of 32 consecutive values (the last one may be shorter).  Per block:
-//   amax = max|x|;  X = clamp(floor(log2 amax) - 8, -127, 127)  (8 = exponent of e4m3's largest binade; amax = 0 -> X = -127);
+//   amax = max|x|;  X = the smallest integer with amax * 2^-X <= 448 (e4m3's largest value), clamped to [-127, 127]
+//   (amax = 0 -> X = -127), so the block maximum lands in (224, 448] and nothing is ever clipped;
 //   code_i = e4m3fn_rne(clamp(x_i * 2^-X, -448, 448));  the block scale is stored as one byte X + 127.
 // Decoding: value = e4m3fn(code) * 2^X.  Both multiplications are by powers of two and exact.
 const int MX_BLOCK = 32;
@@ -179,7 +180,9 @@ int mx_block_exponent(const float* x, size_t n) {
   for (size_t i = 0; i < n; ++i) amax = std::max(amax, std::fabs(x[i]));
   if (!(amax > 0.0f)) return -127;
   int ex;  std::frexp((double)amax, &ex);            // amax = m * 2^ex, m in [0.5,1)  =>  floor(log2 amax) = ex-1
-  return std::min(127, std::max(-127, ex - 1 - 8));
+  int X = ex - 1 - 8;                                // 8 = exponent of e4m3's top binade [256, 512)
+  if (std::ldexp((double)amax, -X) > 448.0) X += 1;  // the top binade ends at 448
+  return std::min(127, std::max(-127, X));
 }
 void encode_slice_mx(const float* x, size_t n, uint8_t* codes, uint8_t* bscale) {
   Fmt f;  fmt_of(DT_E4M3_MX32, &f);

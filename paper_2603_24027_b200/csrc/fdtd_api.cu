@@ -130,7 +130,17 @@ long long slot_values(const fdtd_sim* s) {
   return v;
 }
 int elem_bytes_host(int dt) { return dt == DT_F32 ? 4 : ((dt == DT_F16 || dt == DT_BF16) ? 2 : 1); }
-bool dtype_ok(int dt) { return (dt >= 0 && dt <= 3) || (dt >= DT_E4M3B11FNUZ && dt <= DT_E3M4); }
+bool dtype_ok(int dt) { return (dt >= 0 && dt <= 3) || dt == DT_MX32 || (dt >= DT_E4M3B11FNUZ && dt <= DT_E3M4); }
+// micro-scaled store (DT_MX32): one scale byte per block of 32 values of a slice, kept behind the slot's codes
+long long face_blocks(const fdtd_sim* s, int f) { return (face_size(s, f) + 31) / 32; }
+long long slot_blocks(const fdtd_sim* s) {
+  long long b = 0;
+  for (int f = 0; f < 6; ++f) b += face_comps(s) * face_blocks(s, f);
+  return b;
+}
+size_t slot_bytes_host(const fdtd_sim* s, int dt) {
+  return (size_t)slot_values(s) * elem_bytes_host(dt) + (dt == DT_MX32 ? (size_t)slot_blocks(s) : 0);
+}
 // run STMT with DT bound to the compile-time store dtype
 #define FDTD_DT_SWITCH(dt, STMT)                                                   \
   switch (dt) {                                                                    \
@@ -138,6 +148,7 @@ bool dtype_ok(int dt) { return (dt >= 0 && dt <= 3) || (dt >= DT_E4M3B11FNUZ && 
     case DT_F16: { constexpr int DT = DT_F16; STMT; } break;                       \
     case DT_BF16: { constexpr int DT = DT_BF16; STMT; } break;                     \
     case DT_E4M3S: { constexpr int DT = DT_E4M3S; STMT; } break;                   \
+    case DT_MX32: { constexpr int DT = DT_MX32; STMT; } break;                     \
     case DT_E4M3B11FNUZ: { constexpr int DT = DT_E4M3B11FNUZ; STMT; } break;       \
     case DT_E5M2FNUZ: { constexpr int DT = DT_E5M2FNUZ; STMT; } break;             \
     case DT_E4M3FNUZ: { constexpr int DT = DT_E4M3FNUZ; STMT; } break;             \
@@ -178,7 +189,7 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   L.waves = take((size_t)kMaxSources * nsteps * 4);
   const int slots = num_slots(nsteps, k);
   L.slots_cap = slots;
-  L.store_cap = (size_t)slots * slot_values(s) * elem_bytes_host(dtype);
+  L.store_cap = (size_t)slots * slot_bytes_host(s, dtype);
   L.store = take(L.store_cap);
   L.scales = take((size_t)slots * 36 * 4);
   L.amax = take((size_t)slots * 36 * 4);
@@ -502,6 +513,11 @@ void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int*
 void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
   const long long items = s->store_mode == 1 ? s->st.cell_off[6] * (half == 2 ? 2 : 1)   // 2 components on 3 of the 6 faces
                                              : s->st.cell_off[6] * (half == 2 ? 6 : 3);
+  if (s->dtype == DT_MX32) {   // one warp per block of 32 values; the slices in the half are 'items / face cells' many
+    const long long warps = s->st.blkc_off[6] * (items / s->st.cell_off[6]);
+    LAUNCH(s, k_record_mx, (unsigned)((warps * 32 + 255) / 256), 256, s->d, s->st, m_base, step_dev, half);
+    return;
+  }
   const unsigned g = (unsigned)((items + 255) / 256);
   if (s->dtype == DT_E4M3S) LAUNCH(s, k_record_amax, g, 256, s->d, s->st, m_base, step_dev, half);
   FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_record<DT>, g, 256, s->d, s->st, m_base, step_dev, half))
@@ -862,7 +878,7 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
   if (k < 1) return fail(s, FDTD_ERR_INVALID_ARG, "k must be >= 1");
   if (!dtype_ok((int)dt)) return fail(s, FDTD_ERR_INVALID_ARG, "unknown store dtype %d", (int)dt);
   const int slots = num_slots(nsteps, k);
-  const size_t need = (size_t)slots * slot_values(s) * elem_bytes_host(dt);
+  const size_t need = (size_t)slots * slot_bytes_host(s, (int)dt);
   if (nsteps > s->max_nsteps || slots > s->L.slots_cap || need > s->L.store_cap)
     return fail(s, FDTD_ERR_OOM, "workspace too small: store needs %zu bytes in %d slots, has %zu in %d (nsteps %d, max %d)",
                 need, slots, s->L.store_cap, s->L.slots_cap, nsteps, s->max_nsteps);
@@ -871,7 +887,7 @@ fdtd_status forward_impl(fdtd_sim* s, int nsteps, const fdtd_source* src, int ns
   if (r != FDTD_OK) return r;
   s->nsteps = nsteps; s->k = k; s->dtype = (int)dt;
   s->st.nslots = slots; s->st.nsteps = nsteps; s->st.k = k; s->st.dtype = (int)dt;
-  s->st.slot_bytes = (size_t)slot_values(s) * elem_bytes_host(dt);
+  s->st.slot_bytes = slot_bytes_host(s, (int)dt);
   if (dt == FDTD_F8E4M3_SCALED) CUDA_TRY(s, cudaMemsetAsync(s->st.amax, 0, (size_t)slots * 36 * 4, s->stream));
   s->cur = s->stream;
   if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
@@ -1126,6 +1142,8 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     st.du[f] = s->n[b0] - 2 * s->P;
     st.dv[f] = s->n[b1] - 2 * s->P;
     st.val_off[f + 1] = st.val_off[f] + face_comps(s) * face_size(s, f);
+    st.blk_off[f + 1] = st.blk_off[f] + face_comps(s) * face_blocks(s, f);
+    st.blkc_off[f + 1] = st.blkc_off[f] + face_blocks(s, f);
     st.cell_off[f + 1] = st.cell_off[f] + face_size(s, f);
   }
   s->VG = s->V;
@@ -1232,6 +1250,7 @@ fdtd_status fdtd_slot_ptr(const fdtd_sim* s, int j, const void** data_dev, const
   if (scales_dev) *scales_dev = s->st.scales + (size_t)j * 36;
   return FDTD_OK;
 }
+size_t fdtd_slot_bytes(const fdtd_sim* s, fdtd_dtype dt) { return (s && dtype_ok((int)dt)) ? slot_bytes_host(s, (int)dt) : 0; }
 
 // ---- host-buffer variants ----
 fdtd_status fdtd_set_eps_host(fdtd_sim* s, const float* eps_host) {
@@ -1280,6 +1299,13 @@ fdtd_status fdtd_codec_encode(fdtd_dtype dt, const float* x_dev, size_t n, void*
   if (!x_dev || !codes_dev || !scale_dev || !dtype_ok((int)dt)) return FDTD_ERR_INVALID_ARG;
   cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
   const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
+  if ((int)dt == DT_MX32) {   // codes_dev holds n codes followed by ceil(n/32) scale bytes
+    const unsigned gm = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 148 * 8);
+    k_codec_encode_mx<<<gm, 256, 0, (cudaStream_t)cuda_stream>>>(x_dev, n, reinterpret_cast<unsigned char*>(codes_dev));
+    const float one = 1.0f;
+    if (cudaMemcpyAsync(scale_dev, &one, 4, cudaMemcpyHostToDevice, (cudaStream_t)cuda_stream) != cudaSuccess) return FDTD_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
+  }
   if ((int)dt == DT_E4M3S) {
     if (!scratch_dev) return FDTD_ERR_INVALID_ARG;
     if (cudaMemsetAsync(scratch_dev, 0, 4, st) != cudaSuccess) return FDTD_ERR_CUDA;
@@ -1376,7 +1402,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 3: v = 36 * N + 16 * slab; break;          // lE rw + lH; lpsiH read (old) + written (new)
       case 4: v = 40 * Ninner + 28 * dcells; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
       case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
-      case 6: v = (double)s->st.slot_values * (4 + eb); break;
+      case 6: v = (double)s->st.slot_values * 4 + (double)slot_bytes_host(s, s->dtype); break;   // f32 gathered, slot written (block scales included)
       case 7: case 8: v = (s->store_mode == 1 ? 1.0 : 3.0) * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
       case 9: {   // fused marching kernel: E, H read once and written once, ce read: 52 B per cell of [P+1, n-P)^3
         double c = 1;

@@ -12,7 +12,8 @@
 namespace fdtd {
 
 // 0..3: BASELINE.json's store types.  10..14: the paper's five unscaled float8 flavours (ids as in fdtd.h).
-enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3S = 3,
+// 5: micro-scaled E4M3 (blocks of 32 values share a power-of-two scale byte; R20).
+enum { DT_F32 = 0, DT_F16 = 1, DT_BF16 = 2, DT_E4M3S = 3, DT_MX32 = 5,
        DT_E4M3B11FNUZ = 10, DT_E5M2FNUZ = 11, DT_E4M3FNUZ = 12, DT_E4M3 = 13, DT_E3M4 = 14 };
 
 // Interface store: slot j = state min(j*k, nsteps); inside a slot
@@ -29,6 +30,9 @@ struct StoreDev {
   long long val_off[7];   // prefix sums of ncomp(mode)*face_size  (value index of face f)
   long long cell_off[7];  // prefix sums of face_size    (shell-cell index of face f)
   int du[6], dv[6];
+  // micro-scaled store (DT_MX32): a slot is [codes: slot_values bytes][block scales]; a slice has ceil(face/32) blocks
+  long long blk_off[7];   // prefix sums of ncomp(mode)*blocks(face): block index of face f inside a slot
+  long long blkc_off[7];  // prefix sums of blocks(face)  (what cell_off is for cells)
 };
 
 __device__ __forceinline__ int elem_bytes(int dt) { return dt == DT_F32 ? 4 : ((dt == DT_F16 || dt == DT_BF16) ? 2 : 1); }
@@ -62,6 +66,19 @@ template <> struct Codec<DT_E4M3S> {   // OCP E4M3 (max 448) after a per-slice s
     return __half2float(__half(h)) * scale;
   }
 };
+
+// Micro-scaled E4M3 (R20): the element cast is the scaled one's, the scale is 2^X per block of 32 values with
+// X = the smallest integer with amax * 2^-X <= 448, clamped to [-127, 127], stored as the byte X + 127 (the block maximum lands
+// in (224, 448], nothing is clipped).  Multiplying by 2^-X / 2^X is exact.
+template <> struct Codec<DT_MX32> : Codec<DT_E4M3S> {};
+__device__ __forceinline__ int mx_exponent(unsigned amax_bits) {   // f32 bits of max|x|
+  // floor(log2 amax) - 8, one more where the mantissa is above 1.75 (448 = 1.75 * 2^8); f32 subnormals fall below the clamp
+  return max((int)(amax_bits >> 23) - 135 + ((amax_bits & 0x7fffffu) > 0x600000u ? 1 : 0), -127);
+}
+__device__ __forceinline__ float mx_pow2(int k) {   // 2^k, k in [-127, 127] (2^-127 is an f32 subnormal)
+  return k > -127 ? __uint_as_float((unsigned)(k + 127) << 23) : __uint_as_float(0x00400000u);
+}
+__device__ __forceinline__ float mx_scale(unsigned char byte) { return mx_pow2((int)byte - 127); }
 
 // Software minifloat cast for the paper's unscaled float8 flavours (e4m3b11fnuz, e5m2fnuz, e4m3fnuz, e4m3,
 // e3m4; "f" = finite only, "n" = a NaN code exists, "uz" = no negative zero).  EB exponent bits, MB mantissa bits.
@@ -156,11 +173,14 @@ __device__ __host__ __forceinline__ FetchPlan make_plan(int nstate, int nsteps, 
 }
 
 template <int DT>
-__device__ __forceinline__ float fetch_value(const StoreDev& s, const FetchPlan& p, int slice, long long vidx) {
+__device__ __forceinline__ float fetch_value(const StoreDev& s, const FetchPlan& p, int slice, long long vidx, long long bidx) {
   typedef typename Codec<DT>::code_t code_t;
   auto val = [&](int j) {
-    const code_t c = reinterpret_cast<const code_t*>(s.base + (size_t)j * s.slot_bytes)[vidx];
-    const float sc = DT == DT_E4M3S ? s.scales[(size_t)j * 36 + slice] : 1.0f;
+    const char* slot = s.base + (size_t)j * s.slot_bytes;
+    const code_t c = reinterpret_cast<const code_t*>(slot)[vidx];
+    float sc = 1.0f;
+    if (DT == DT_E4M3S) sc = s.scales[(size_t)j * 36 + slice];
+    if (DT == DT_MX32) sc = mx_scale(reinterpret_cast<const unsigned char*>(slot)[s.slot_values + bidx]);
     return Codec<DT>::dec(c, sc);
   };
   const float a = val(p.j[1]);
@@ -198,23 +218,24 @@ __device__ __forceinline__ int record_slot(const StoreDev& s, int m) {
 // ---------------------------------------------------------------------------------------------------------
 // half = 0: the three E components, 1: the three H components, 2: all six.  The two halves of a slot can be written
 // by different launches: E^m is final after the E half-step, H^{m+1/2} after the H half-step.
-struct RecItem { int f, comp; long long e, vidx; };
+// coff: prefix sums of the per-face slice length that t enumerates — cell_off (t = value) or blkc_off (t = block of 32 values).
+struct RecItem { int f, comp, rank; long long e; };   // rank: position of the component among those the face stores
 // Tangential store (mode 1): the inner interior reads from the shell only H tangential to the LOW faces
 // (through d^- in the inverse-E update) and E tangential to the HIGH faces (through d^+ in the inverse-H update); a face
 // keeps those two components, in increasing component order.
 __device__ __forceinline__ int tangential_comp(int axis, int rank) { return axis == 0 ? 1 + rank : (axis == 1 ? 2 * rank : rank); }
-__device__ __forceinline__ bool record_item_tangential(const StoreDev& s, long long t, int half, RecItem& it) {
+__device__ __forceinline__ bool record_item_tangential(const long long* coff, long long t, int half, RecItem& it) {
   // half 0: E on the three high faces, half 1: H on the three low faces, half 2: E part then H part
   for (int h = (half == 2 ? 0 : half); h <= (half == 2 ? 1 : half); ++h) {
     for (int a = 0; a < 3; ++a) {
       const int f = 2 * a + (h == 0 ? 1 : 0);
-      const long long fs = s.cell_off[f + 1] - s.cell_off[f];
+      const long long fs = coff[f + 1] - coff[f];
       if (t < 2 * fs) {
         const int rank = (int)(t / fs);
         it.f = f;
+        it.rank = rank;
         it.comp = tangential_comp(a, rank) + (h == 1 ? 3 : 0);
         it.e = t - rank * fs;
-        it.vidx = s.val_off[f] + rank * fs + it.e;
         return true;
       }
       t -= 2 * fs;
@@ -222,28 +243,31 @@ __device__ __forceinline__ bool record_item_tangential(const StoreDev& s, long l
   }
   return false;
 }
-__device__ __forceinline__ bool record_item(const StoreDev& s, long long t, int half, RecItem& it) {
-  if (s.mode == 1) return record_item_tangential(s, t, half, it);
+__device__ __forceinline__ bool record_item(const StoreDev& s, const long long* coff, long long t, int half, RecItem& it) {
+  if (s.mode == 1) return record_item_tangential(coff, t, half, it);
   const int nc = half == 2 ? 6 : 3;
-  if (t >= s.cell_off[6] * nc) return false;
-  // t enumerates [face][comp in half][element]; cell_off = prefix sums of face sizes
+  if (t >= coff[6] * nc) return false;
+  // t enumerates [face][comp in half][element]; coff = prefix sums of face sizes
   int f = 0;
 #pragma unroll
-  for (int g = 1; g < 6; ++g) f += (t >= s.cell_off[g] * nc);
-  const long long fs = s.cell_off[f + 1] - s.cell_off[f];
-  const long long r = t - s.cell_off[f] * nc;
+  for (int g = 1; g < 6; ++g) f += (t >= coff[g] * nc);
+  const long long fs = coff[f + 1] - coff[f];
+  const long long r = t - coff[f] * nc;
   it.f = f;
   it.comp = (int)(r / fs) + (half == 1 ? 3 : 0);
+  it.rank = it.comp;
   it.e = r % fs;
-  it.vidx = s.val_off[f] + it.comp * fs + it.e;
   return true;
+}
+__device__ __forceinline__ long long value_index(const StoreDev& s, const RecItem& it, long long e) {
+  return s.val_off[it.f] + it.rank * (s.cell_off[it.f + 1] - s.cell_off[it.f]) + e;
 }
 
 __global__ void __launch_bounds__(256) k_record_amax(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
                                                       int m_base, const int* step_dev, int half) {
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   RecItem it;
-  if (!record_item(s, t, half, it)) return;
+  if (!record_item(s, s.cell_off, t, half, it)) return;
   const int slot = record_slot(s, cur_step(m_base, step_dev));
   const int f = it.f, comp = it.comp;
   int c[3];
@@ -263,7 +287,7 @@ __global__ void __launch_bounds__(256) k_record(const __grid_constant__ Dev d, c
   typedef typename Codec<DT>::code_t code_t;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   RecItem it;
-  if (!record_item(s, t, half, it)) return;
+  if (!record_item(s, s.cell_off, t, half, it)) return;
   const int slot = record_slot(s, cur_step(m_base, step_dev));
   const int f = it.f, comp = it.comp;
   const long long e = it.e;
@@ -276,7 +300,31 @@ __global__ void __launch_bounds__(256) k_record(const __grid_constant__ Dev d, c
     inv = amax > 0.0f ? 448.0f / amax : 0.0f;
     if (e == 0) s.scales[(size_t)slot * 36 + f * 6 + comp] = amax > 0.0f ? amax / 448.0f : 0.0f;
   }
-  reinterpret_cast<code_t*>(s.base + (size_t)slot * s.slot_bytes)[it.vidx] = Codec<DT>::enc(x, inv);
+  reinterpret_cast<code_t*>(s.base + (size_t)slot * s.slot_bytes)[value_index(s, it, e)] = Codec<DT>::enc(x, inv);
+}
+
+// Micro-scaled record (DT_MX32, R20): one warp = one block of 32 consecutive values of a slice; the block's absmax
+// is one redux.max over the lanes, so there is no slice-wide pass and no atomic.  Lane 0 writes the scale byte behind the codes.
+__global__ void __launch_bounds__(256) k_record_mx(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
+                                                   int m_base, const int* step_dev, int half) {
+  const long long w = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  RecItem it;
+  if (!record_item(s, s.blkc_off, w, half, it)) return;   // warp-uniform
+  const int slot = record_slot(s, cur_step(m_base, step_dev));
+  const int f = it.f;
+  const long long fs = s.cell_off[f + 1] - s.cell_off[f];
+  const long long e = it.e * 32 + lane;
+  float x = 0.0f;
+  if (e < fs) {
+    int c[3];
+    face_cell(d, s, f, e, c);
+    x = field_ptr(d, it.comp)[((long long)c[0] * d.n[1] + c[1]) * d.n[2] + c[2]];
+  }
+  const int X = mx_exponent(__reduce_max_sync(0xffffffffu, __float_as_uint(fabsf(x))));
+  unsigned char* slotp = reinterpret_cast<unsigned char*>(s.base + (size_t)slot * s.slot_bytes);
+  if (e < fs) slotp[value_index(s, it, e)] = Codec<DT_MX32>::enc(x, mx_pow2(-X));
+  if (lane == 0) slotp[s.slot_values + s.blk_off[f] + it.rank * (s.blkc_off[f + 1] - s.blkc_off[f]) + it.e] = (unsigned char)(X + 127);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -313,6 +361,7 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
   const FetchPlan p = make_plan(nstate, s.nsteps, s.k, s.nslots, interp);
   const long long q = ((long long)c[0] * d.n[1] + c[1]) * d.n[2] + c[2];
   const long long fs = (long long)s.du[f] * s.dv[f];
+  const long long nb = s.blkc_off[f + 1] - s.blkc_off[f], b0 = s.blk_off[f] + (e >> 5);   // DT_MX32: block of element e
   float nv[3];
 #pragma unroll
   for (int cc = 0; cc < 3; ++cc) {
@@ -320,9 +369,9 @@ __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, c
     if (tang) {
       if (cc == a) continue;
       const int rank = cc > a ? cc - 1 : cc;      // position among the two components tangential to axis a
-      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + rank * fs + e);
+      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + rank * fs + e, b0 + rank * nb);
     } else {
-      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + comp * fs + e);
+      nv[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + comp * fs + e, b0 + comp * nb);
     }
   }
   if (magnetic) {
@@ -468,6 +517,18 @@ __global__ void k_codec_encode(const float* __restrict__ x, size_t n, void* code
   for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x)
     reinterpret_cast<code_t*>(codes)[t] = Codec<DT>::enc(x[t], inv);
 }
+// DT_MX32: codes[n] followed by ceil(n/32) scale bytes in the same buffer (the slot convention); one warp per block
+__global__ void k_codec_encode_mx(const float* __restrict__ x, size_t n, unsigned char* codes) {
+  const size_t nblk = (n + 31) / 32;
+  const int lane = threadIdx.x & 31;
+  for (size_t b = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < nblk; b += ((size_t)gridDim.x * blockDim.x) >> 5) {
+    const size_t t = b * 32 + lane;
+    const float v = t < n ? x[t] : 0.0f;
+    const int X = mx_exponent(__reduce_max_sync(0xffffffffu, __float_as_uint(fabsf(v))));
+    if (t < n) codes[t] = Codec<DT_MX32>::enc(v, mx_pow2(-X));
+    if (lane == 0) codes[n + b] = (unsigned char)(X + 127);
+  }
+}
 struct FetchArgs {
   const void* codes[4];
   float scales[4];
@@ -476,7 +537,10 @@ template <int DT>
 __global__ void k_codec_fetch(const __grid_constant__ FetchArgs a, int mode, int num, int den, size_t n, float* out) {
   typedef typename Codec<DT>::code_t code_t;
   for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
-    auto val = [&](int j) { return Codec<DT>::dec(reinterpret_cast<const code_t*>(a.codes[j])[t], a.scales[j]); };
+    auto val = [&](int j) {
+      const float sc = DT == DT_MX32 ? mx_scale(reinterpret_cast<const unsigned char*>(a.codes[j])[n + (t >> 5)]) : a.scales[j];
+      return Codec<DT>::dec(reinterpret_cast<const code_t*>(a.codes[j])[t], sc);
+    };
     const float v0 = val(1);
     float r = v0;
     if (mode == 1) r = lerp_value(v0, val(2), num, den);

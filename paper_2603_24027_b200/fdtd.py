@@ -10,6 +10,8 @@ import os
 import numpy as np
 
 F32, F16, BF16, F8E4M3_SCALED = 0, 1, 2, 3
+# micro-scaled E4M3: blocks of 32 values share a power-of-two scale byte kept behind the slot's codes (R20)
+F8E4M3_MX32 = 5
 # the paper's unscaled float8 flavours
 F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14
 LINEAR, CUBIC = 0, 1
@@ -17,7 +19,7 @@ STORE_ALL, STORE_TANGENTIAL = 0, 1
 WS_REVERSE, WS_HOST_IO = 1, 2
 STATUS = {0: "FDTD_OK", 1: "FDTD_ERR_INVALID_ARG", 2: "FDTD_ERR_OOM", 3: "FDTD_ERR_CUDA", 4: "FDTD_ERR_STATE",
           5: "FDTD_ERR_UNSUPPORTED"}
-ELEM_BYTES = {F32: 4, F16: 2, BF16: 2, F8E4M3_SCALED: 1, F8E4M3B11FNUZ: 1, F8E5M2FNUZ: 1, F8E4M3FNUZ: 1, F8E4M3: 1,
+ELEM_BYTES = {F32: 4, F16: 2, BF16: 2, F8E4M3_SCALED: 1, F8E4M3_MX32: 1, F8E4M3B11FNUZ: 1, F8E5M2FNUZ: 1, F8E4M3FNUZ: 1, F8E4M3: 1,
               F8E3M4: 1}
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -75,6 +77,8 @@ def lib():
     L.fdtd_slot_values.restype = C.c_size_t
     L.fdtd_slot_values.argtypes = [vp]
     L.fdtd_slot_ptr.argtypes = [vp, C.c_int, C.POINTER(vp), C.POINTER(vp)]
+    L.fdtd_slot_bytes.restype = C.c_size_t
+    L.fdtd_slot_bytes.argtypes = [vp, C.c_int]
     L.fdtd_set_eps_host.argtypes = [vp, vp]
     L.fdtd_forward_host.argtypes = [vp, C.c_int, C.POINTER(_Source), C.c_int, C.c_int, C.c_int, vp]
     L.fdtd_reverse_host.argtypes = [vp, vp, C.c_int, vp]
@@ -94,7 +98,7 @@ def lib():
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
             "fdtd_set_graphs", "fdtd_set_fused", "fdtd_uses_fused", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
-            "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
+            "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_slot_bytes", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count"]
 
@@ -184,7 +188,7 @@ class Sim:
         if self.ws is not None and self.ws_key is not None:
             n0, d0, k0, f0 = self.ws_key
             if (f0 & flags) == flags and nsteps <= n0 and slots(nsteps, k) <= slots(n0, k0) and \
-                    slots(nsteps, k) * ELEM_BYTES[dtype] <= slots(n0, k0) * ELEM_BYTES[d0]:
+                    slots(nsteps, k) * self.slot_bytes(dtype) <= slots(n0, k0) * self.slot_bytes(d0):
                 return
         self.set_workspace(nsteps, dtype, k, flags)
 
@@ -313,12 +317,16 @@ class Sim:
     def slot_values(self):
         return self._L.fdtd_slot_values(self._h)
 
+    def slot_bytes(self, dtype):
+        return self._L.fdtd_slot_bytes(self._h, int(dtype))
+
     def slot(self, j, dtype):
-        """(raw bytes uint8 CUDA tensor copy, 36 float32 scales) of stored slot j."""
+        """(raw bytes uint8 CUDA tensor copy, 36 float32 scales) of stored slot j.  F8E4M3_MX32: the bytes are the slot_values
+        codes followed by the block-scale bytes."""
         torch = self._torch
         dp, sp = C.c_void_p(), C.c_void_p()
         self._check(self._L.fdtd_slot_ptr(self._h, int(j), C.byref(dp), C.byref(sp)))
-        nbytes = self.slot_values() * ELEM_BYTES[dtype]
+        nbytes = self.slot_bytes(dtype)
         off = dp.value - self.ws.data_ptr()
         soff = sp.value - self.ws.data_ptr()
         self.sync()
@@ -348,7 +356,8 @@ def codec_encode(dtype, x):
     torch = _torch()
     L = lib()
     x = x.contiguous()
-    codes = torch.empty(x.numel() * ELEM_BYTES[dtype], dtype=torch.uint8, device=x.device)
+    nbytes = x.numel() * ELEM_BYTES[dtype] + ((x.numel() + 31) // 32 if dtype == F8E4M3_MX32 else 0)
+    codes = torch.empty(nbytes, dtype=torch.uint8, device=x.device)
     scale = torch.zeros(1, dtype=torch.float32, device=x.device)
     scratch = torch.zeros(1, dtype=torch.int32, device=x.device)
     st = L.fdtd_codec_encode(int(dtype), C.c_void_p(x.data_ptr()), x.numel(), C.c_void_p(codes.data_ptr()),
@@ -358,12 +367,15 @@ def codec_encode(dtype, x):
     return codes, float(scale.item())
 
 
-def codec_fetch(dtype, interp, codes, scales, num, den):
-    """codes: list of 4 uint8 CUDA tensors (or None) for steps -1, 0, 1, 2; scales: 4 floats."""
+def codec_fetch(dtype, interp, codes, scales, num, den, n=None):
+    """codes: list of 4 uint8 CUDA tensors (or None) for steps -1, 0, 1, 2; scales: 4 floats.  F8E4M3_MX32: each tensor holds
+    n codes followed by ceil(n/32) scale bytes, and n must be given."""
     torch = _torch()
     L = lib()
     ref = codes[1]
-    n = ref.numel() // ELEM_BYTES[dtype]
+    if n is None:
+        assert dtype != F8E4M3_MX32
+        n = ref.numel() // ELEM_BYTES[dtype]
     ptrs = (C.c_void_p * 4)(*[C.c_void_p(c.data_ptr()) if c is not None else None for c in codes])
     sc = (C.c_float * 4)(*[float(s) for s in scales])
     out = torch.empty(n, dtype=torch.float32, device=ref.device)

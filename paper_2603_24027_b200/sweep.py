@@ -1,7 +1,7 @@
 """Accuracy / memory sweep of the interface store (BASELINE.json configs[4]; the shape of the paper's Fig. 3).
 
 For one workload (default C3, 256x256x128) and a few seeded designs: store dtype in {float32, float16, bfloat16,
-float8_e4m3+scale} x k in {1,2,4,8,16,32} x {linear, cubic}; --paper-fp8 adds the paper's five unscaled float8
+float8_e4m3+scale, float8_e4m3+mx32 (a scale byte per 32 values)} x k in {1,2,4,8,16,32} x {linear, cubic}; --paper-fp8 adds the paper's five unscaled float8
 flavours (e4m3b11fnuz, e5m2fnuz, e4m3fnuz, e4m3, e3m4).  Reports, per setting, the store bytes
 (fdtd_store_bytes), the paper's compression factor (32/bits)*k, the gradient throughput and the
 cosine similarity (eq. 2) of grad_eps against the (float32, k = 1, linear) gradient of the same design,
@@ -26,7 +26,7 @@ def run(args):
     import torch
     from . import fdtd
     base_seed = {"C1": 1001, "C2": 1002, "C3": 1003, "C4": 1004}[args.workload]
-    dtypes = [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED] + (list(W.PAPER_FP8) if args.paper_fp8 else [])
+    dtypes = [W.F32, W.F16, W.BF16, W.F8E4M3_SCALED, W.F8E4M3_MX32] + (list(W.PAPER_FP8) if args.paper_fp8 else [])
     ks = [int(x) for x in args.k.split(",")]
     interps = [W.LINEAR, W.CUBIC] if args.cubic else [W.LINEAR]
     acc = {}
@@ -82,11 +82,12 @@ def run(args):
 
 def to_markdown(res):
     out = [f"Sweep on {res['workload']} {res['grid']} x {res['nsteps']} steps, {res['seeds']} seeded design(s); cosine vs (float32, k=1, linear)\n",
-           "| dtype | k | interp | store MB | bytes ratio | (32/bits)*k | cosine mean | cosine min | Mcell-upd/s (incl. host loss) |",
-           "|---|---|---|---|---|---|---|---|---|"]
+           "| dtype | k | interp | store MB | bytes ratio | (32/bits)*k | cosine mean | cosine min | 1 - cosine mean | Mcell-upd/s (incl. host loss) |",
+           "|---|---|---|---|---|---|---|---|---|---|"]
     for r in res["rows"]:
         out.append(f"| {r['dtype']} | {r['k']} | {r['interp']} | {r['store_bytes'] / 1e6:.1f} | {r['byte_ratio_vs_f32_k1']:.2f} | "
-                   f"{r['paper_factor']} | {r['cosine_mean']:.6f} | {r['cosine_min']:.6f} | {r['mcells_per_s_incl_host_loss']:.0f} |")
+                   f"{r['paper_factor']} | {r['cosine_mean']:.6f} | {r['cosine_min']:.6f} | {1.0 - r['cosine_mean']:.2e} | "
+                   f"{r['mcells_per_s_incl_host_loss']:.0f} |")
     return "\n".join(out)
 
 

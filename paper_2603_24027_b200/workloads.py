@@ -29,13 +29,15 @@ EPS_SI, EPS_SIO2 = 12.25, 2.085
 
 # store dtypes / interpolation (the ids of include/fdtd.h)
 F32, F16, BF16, F8E4M3_SCALED = 0, 1, 2, 3
+F8E4M3_MX32 = 5    # micro-scaled E4M3: a power-of-two scale byte per block of 32 values (R20)
 F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14   # the paper's unscaled flavours
 PAPER_FP8 = (F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4)
 LINEAR, CUBIC = 0, 1
 DTYPE_NAMES = {F32: "float32", F16: "float16", BF16: "bfloat16", F8E4M3_SCALED: "float8_e4m3+scale",
+               F8E4M3_MX32: "float8_e4m3+mx32",
                F8E4M3B11FNUZ: "float8_e4m3b11fnuz", F8E5M2FNUZ: "float8_e5m2fnuz", F8E4M3FNUZ: "float8_e4m3fnuz",
                F8E4M3: "float8_e4m3", F8E3M4: "float8_e3m4"}
-DTYPE_BITS = {F32: 32, F16: 16, BF16: 16, F8E4M3_SCALED: 8, **{d: 8 for d in PAPER_FP8}}
+DTYPE_BITS = {F32: 32, F16: 16, BF16: 16, F8E4M3_SCALED: 8, F8E4M3_MX32: 8, **{d: 8 for d in PAPER_FP8}}
 
 
 @dataclass

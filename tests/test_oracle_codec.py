@@ -103,8 +103,8 @@ def test_scaled_e4m3_slice_codec():
 
 
 def test_microscaled_e4m3_slice_codec():
-    """DESIGN.md R20: blocks of 32 values, block scale 2^X with X = clamp(floor(log2 amax) - 8, -127, 127) stored as X + 127,
-    code = e4m3fn(clamp(x * 2^-X, +-448)).  References: ml_dtypes' float8_e8m0fnu (the scale byte) and float8_e4m3fn (the
+    """DESIGN.md R20: blocks of 32 values, block scale 2^X with X = the smallest integer such that amax * 2^-X <= 448 (clamped to
+    [-127, 127]) stored as X + 127, code = e4m3fn(clamp(x * 2^-X, +-448)).  References: ml_dtypes' float8_e8m0fnu (the scale byte) and float8_e4m3fn (the
     element cast), torch's e4m3fn cast, and properties no formula-retyping can fake (error bound, scale equivariance, block
     independence, ragged tail)."""
     rng = np.random.default_rng(7)
@@ -114,6 +114,8 @@ def test_microscaled_e4m3_slice_codec():
     x[96:128] *= np.float32(1e-38)                                       # a block of f32 subnormals / tiny values
     x[128] = np.float32(3.0e38)                                          # near the f32 maximum
     x[160:192] = np.float32(2.0 ** -5) * np.arange(-16, 16, dtype=np.float32)   # exactly representable: must round-trip
+    x[192:224] = np.float32(448.0 * 2.0 ** -20) * np.linspace(-1, 1, 32, dtype=np.float32)   # amax exactly 448 * 2^X: lower X
+    x[224:256] = np.float32(449.0 * 2.0 ** -20) * np.linspace(-1, 1, 32, dtype=np.float32)   # just above: X one higher
     codes, bs = orc.encode_mx(x)
     assert codes.shape == (n,) and bs.shape == (41,)
     assert not np.any((codes & 0x7F) == 0x7F)                            # never the NaN code
@@ -122,25 +124,25 @@ def test_microscaled_e4m3_slice_codec():
     pad = np.zeros(nb * 32, np.float32)
     pad[:n] = x
     amax = np.abs(pad).reshape(nb, 32).max(axis=1)
-    # the scale byte, read as ml_dtypes' e8m0: a power of two with  amax / 2^9 < scale <= amax / 2^8  (unless clamped)
+    # the scale byte, read as ml_dtypes' e8m0: a power of two with  224 * scale < amax <= 448 * scale  (unless clamped)
     scale = bs.view(ml_dtypes.float8_e8m0fnu).astype(np.float64)
     assert np.array_equal(scale, 2.0 ** (bs.astype(np.int64) - 127))
-    nz = amax > 2.0 ** -118
-    assert np.all(scale[nz] * 2.0 ** 8 <= amax[nz]) and np.all(amax[nz] < scale[nz] * 2.0 ** 9)
+    nz = amax > 448.0 * 2.0 ** -127
+    assert np.all(scale[nz] * 224.0 < amax[nz]) and np.all(amax[nz] <= scale[nz] * 448.0)
+    assert np.any(amax[nz] > scale[nz] * 256.0) and np.any(amax[nz] <= scale[nz] * 256.0)     # both binades occur
     assert np.all(bs[amax == 0] == 0) and np.all(bs[~nz] == 0)           # X clamps at -127
     # elements: the library cast of the scaled, clamped value
     y = np.clip(pad.astype(np.float64) / np.repeat(scale, 32), -448, 448).astype(np.float32)[:n]
     assert np.array_equal(codes, y.astype(ml_dtypes.float8_e4m3fn).view(np.uint8))
     assert np.array_equal(codes, torch.from_numpy(y).to(torch.float8_e4m3fn).view(torch.uint8).numpy())
     assert np.array_equal(back.astype(np.float64), codes.view(ml_dtypes.float8_e4m3fn).astype(np.float64) * np.repeat(scale, 32)[:n])
-    # error bound: 3 mantissa bits -> 2^-4 relative (2^-3 where the value was clamped from (448, 512) * scale), or half
-    # the subnormal step 2^-10 * scale
+    # error bound: 3 mantissa bits -> 2^-4 relative, or half the subnormal step 2^-10 * scale; nothing is ever clipped
     sc_el = np.repeat(scale, 32)[:n]
     err = np.abs(back.astype(np.float64) - x.astype(np.float64))
-    assert np.all(err <= np.maximum(2.0 ** -3 * np.abs(x.astype(np.float64)), 2.0 ** -10 * sc_el))
-    unclamped = np.abs(y) < 448
-    assert np.all(err[unclamped] <= np.maximum(2.0 ** -4 * np.abs(x[unclamped].astype(np.float64)), 2.0 ** -10 * sc_el[unclamped]))
+    assert np.all(err <= np.maximum(2.0 ** -4 * np.abs(x.astype(np.float64)), 2.0 ** -10 * sc_el))
+    assert np.all(np.abs(pad.astype(np.float64) / np.repeat(scale, 32)) <= 448.0)
     assert np.array_equal(back[160:192], x[160:192]) and not back[64:96].any()
+    assert int(bs[6]) == 127 - 20 and int(bs[7]) == 127 - 19 and (codes[192] & 0x7F) == 0x7E      # 0x7E = 448
     # the largest value of each block keeps at least its leading bit: never flushed
     imax = np.abs(pad).reshape(nb, 32).argmax(axis=1) + 32 * np.arange(nb)
     keep = imax[nz]
