@@ -454,8 +454,6 @@ void launch_split(fdtd_sim* s, int which, int pb) {
   launch_lean(s, which);
   launch_gen(s, which, pb);
 }
-void launch_fwd_e(fdtd_sim* s) { launch_split(s, 0, 0); }
-void launch_fwd_h(fdtd_sim* s) { launch_split(s, 1, 0); }
 void launch_inv_h(fdtd_sim* s) {
   dim3 gi;
   if (!grid_inner(s, &gi)) return;
