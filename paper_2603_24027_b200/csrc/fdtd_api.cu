@@ -1124,6 +1124,12 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     d.acc = reinterpret_cast<double*>(w + L.acc);
   }
   d.has_design = s->has_design ? 1 : 0;
+  {   // ce resident in L2 during the reverse run where it fits a third of it (fdtd_dev.cuh, ldv_ce)
+    int dev = 0, l2 = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess) l2 = 0;
+    d.ce_keep = ((long long)d.N * 4 <= (long long)l2 / 3) ? 1 : 0;
+    if (const char* e = std::getenv("FDTD_CE_KEEP")) d.ce_keep = atoi(e) ? 1 : 0;
+  }
   for (int a = 0; a < 3; ++a) { d.dlo[a] = s->dlo[a]; d.dhi[a] = s->dhi[a]; }
   // store geometry
   StoreDev& st = s->st;

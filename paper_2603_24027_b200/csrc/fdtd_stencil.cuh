@@ -362,7 +362,7 @@ __global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d
   const VF<V> hx_ym = ldv<V>(d.H[0] + q - sy), hz_ym = ldv<V>(d.H[2] + q - sy);
   const float hx_z0 = d.H[0][q - 1], hy_z0 = d.H[1][q - 1];   // k0 >= 1: the inner interior starts at P + 1
   VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
-  const VF<V> ce = ldv<V>(d.ce + q);
+  const VF<V> ce = ldv_ce<V>(d, d.ce + q);
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
@@ -594,18 +594,18 @@ __device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const 
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const int nb = pb ^ 1;
-  const VF<V> ce = ldv<V>(d.ce + q);
+  const VF<V> ce = ldv_ce<V>(d, d.ce + q);
   VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
   VF<V> gy_xp = zerov<V>(), gz_xp = zerov<V>(), gx_yp = zerov<V>(), gz_yp = zerov<V>();
   VF<V> ce_xp = zerov<V>(), ce_yp = zerov<V>();
   float gx_zp = 0.0f, gy_zp = 0.0f, ce_zp = 0.0f;
   if (i + 1 < nx) {
-    ce_xp = ldv<V>(d.ce + q + sx);
+    ce_xp = ldv_ce<V>(d, d.ce + q + sx);
     gy_xp = ldv<V>(d.lE[1] + q + sx);
     gz_xp = ldv<V>(d.lE[2] + q + sx);
   }
   if (j + 1 < ny) {
-    ce_yp = ldv<V>(d.ce + q + sy);
+    ce_yp = ldv_ce<V>(d, d.ce + q + sy);
     gx_yp = ldv<V>(d.lE[0] + q + sy);
     gz_yp = ldv<V>(d.lE[2] + q + sy);
   }
@@ -860,7 +860,7 @@ __global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ 
   if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
-  const VF<V> ce = ldv<V>(d.ce + q), ce_xp = ldv<V>(d.ce + q + sx), ce_yp = ldv<V>(d.ce + q + sy);
+  const VF<V> ce = ldv_ce<V>(d, d.ce + q), ce_xp = ldv_ce<V>(d, d.ce + q + sx), ce_yp = ldv_ce<V>(d, d.ce + q + sy);
   const float ce_zp = d.ce[q + V];
   VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
   VF<V> gy_xp = ldv<V>(d.lE[1] + q + sx), gz_xp = ldv<V>(d.lE[2] + q + sx);
