@@ -28,8 +28,13 @@
 // interpolation -> polynomial exactness and sinusoid error bound; dt -> the paper's printed value;
 // tangential-only store (store_mode 1) -> inner interior back to state 0 and gradient = store-all back-propagation;
 // micro-scaled e4m3 (dtype 5) -> ml_dtypes float8_e4m3fn / float8_e8m0fnu casts, error bound, scale equivariance.
+// fetch path (slot choice of the cubic option, fall-back to linear on the first / last / short interval, exact return at
+// stored steps) -> a run with Courant number 0 whose interface values are a known cubic polynomial in the step index
+// (tests/test_oracle_codec.py::test_cubic_fetch_path_slot_choice_and_fallbacks).
 // CPML constants: PARITY UNPINNED against the paper (it prints none); pinned only by "sigma=0 reduces
 // to plain Yee" and a reflection bound.
+// Edge / corner ownership at injection ("the lowest-numbered face that contains the cell wins", reading R7/R9; it only
+// matters under per-slice scales, where two faces hold differently rounded copies of one cell): PARITY UNPINNED, a reading.
 //
 // Build: g++ -O2 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py).
 

@@ -266,3 +266,62 @@ def test_compression_factor_matches_paper(golden):
     assert ratio == pytest.approx(4 * (T + 1) / (T // 16 + 1))
     assert abs(ratio / g["compression_e4m3_k16"] - 1) < 0.02           # -> 64 as T grows (slot-0 overhead)
     assert sizes[(orc.F32, 1)] / sizes[(orc.BF16, 4)] == pytest.approx(2 * (T + 1) / (T // 4 + 1))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# The fetch PATH of the cubic option (slot choice j0-1 .. j0+2 and the fall-back rules of DESIGN.md R11 / SURVEY c-7),
+# pinned through the real record -> fetch route.  With a Courant number of 0 the curl terms vanish, so a source with
+# wave[m-1] = p(m) - p(m-1) leaves E^m = p(m) on its box: the interface values are a known cubic polynomial in the step
+# index (integers, exact in f32 and f64).  Expected values come from p alone: p(n) where R11 says "cubic", the chord
+# between the two bracketing stored values where it says "linear" (first interval, last interval, any interval whose
+# neighbouring slots are not k apart), p(n) at stored steps.  A one-slot shift or a wrong fall-back condition fails it.
+# ---------------------------------------------------------------------------------------------------------
+def _p_cubic(m):
+    m = np.asarray(m, dtype=np.float64)
+    return 2.0 * m ** 3 - 45.0 * m ** 2 + 210.0 * m
+
+
+@pytest.mark.parametrize("prec,dtype", [(64, orc.NATIVE), (32, orc.F32), (32, orc.NATIVE)])
+@pytest.mark.parametrize("T,k", [(23, 4), (24, 4), (17, 5), (9, 3), (7, 4), (3, 4)])
+def test_cubic_fetch_path_slot_choice_and_fallbacks(prec, dtype, T, k):
+    n, P = 8, 2
+    s = orc.OracleSim(prec, np.ones((n, n, n)), P, 0.0)
+    wave = _p_cubic(np.arange(1, T + 1)) - _p_cubic(np.arange(0, T))
+    # Ez on the whole low-x interface plane (face 0: plane i = P, cross-section [P, n-P)^2)
+    s.add_source(2, (P, P, P), (P + 1, n - P, n - P), None, wave)
+    s.forward(T, dtype, k)
+    stored = list(range(0, T + 1, k)) + ([T] if T % k else [])
+    assert [s.slot_step(j) for j in range(s.num_slots())] == stored
+    face, comp = 0, 2
+    nfs = s.face_size(face)
+    for nstate in range(T + 1):
+        if nstate in stored:
+            kind, want = "exact", float(_p_cubic(nstate))
+        else:
+            j0 = nstate // k
+            m0, m1 = stored[j0], stored[j0 + 1]
+            cubic = j0 >= 1 and j0 + 2 < len(stored) and m1 - m0 == k and stored[j0 + 2] - m1 == k
+            if cubic:
+                kind, want = "cubic", float(_p_cubic(nstate))
+            else:
+                kind = "linear"
+                want = float(_p_cubic(m0) + (nstate - m0) / (m1 - m0) * (_p_cubic(m1) - _p_cubic(m0)))
+        got = s.fetch_face(nstate, face, comp, orc.CUBIC)
+        assert got.shape == (nfs,)
+        tol = (1e-6 if prec == 32 or dtype == orc.F32 else 1e-12) * max(1.0, float(np.max(np.abs(_p_cubic(stored)))))
+        if kind == "exact":
+            tol = 0.0
+        assert np.max(np.abs(got - want)) <= tol, (T, k, nstate, kind, float(got[0]), want)
+        # the linear option on the same store: chord everywhere between stored steps
+        lin = s.fetch(nstate, face, comp, 0, orc.LINEAR)
+        if nstate not in stored:
+            j0 = nstate // k
+            m0, m1 = stored[j0], stored[j0 + 1]
+            chord = float(_p_cubic(m0) + (nstate - m0) / (m1 - m0) * (_p_cubic(m1) - _p_cubic(m0)))
+            assert abs(lin - chord) <= max(tol, 1e-12)
+    # the cubic and the chord differ on the cubic intervals (the test can tell them apart)
+    if len(stored) >= 5 and k > 1:
+        n_mid = stored[1] + 1
+        assert abs(float(_p_cubic(n_mid)) - s.fetch(n_mid, face, comp, 0, orc.LINEAR)) > 1.0
+    # components that have no source stay zero in every slot
+    assert np.all(s.fetch_face(min(T, k + 1), face, 0, orc.CUBIC) == 0.0)
