@@ -91,8 +91,11 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
  * CPML psi_E, sources, H half-step with psi_H (R1-R5), monitor write, and the record step:
  * state m is cast to store_dtype and written to the interface store when m % k == 0 or m == nsteps, state 0
  * included (R6,R7,R10).  FDTD_ERR_OOM if the workspace is too small,
- * FDTD_ERR_INVALID_ARG for nsteps < 1, k < 1 or a source outside the interior.  A second call restarts the store
- * (the run is NOT extended). */
+ * FDTD_ERR_INVALID_ARG for nsteps < 1, k < 1 or a source outside the interior.
+ * Repeated calls without fdtd_reset in between (R21; SURVEY 8(b) sketched "extend the run"): the FIELDS continue
+ * from the current state, but every call opens a new SEGMENT — the store is recorded anew from this call's first state, the
+ * monitor rows and the source samples are counted from this call's step 1 — and fdtd_reverse unwinds the last segment only
+ * (the gradient of a loss on that segment with the segment's initial state held fixed). */
 fdtd_status fdtd_forward(fdtd_sim*, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype store_dtype, int k);
 
 /* Reverse run (step order DESIGN.md R9): starting from the live final state, for m = nsteps..1
@@ -203,17 +206,6 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dtype, fdtd_interp interp, const void* c
 fdtd_status fdtd_sync(fdtd_sim*);
 const char* fdtd_last_error(const fdtd_sim*);
 void fdtd_destroy(fdtd_sim*);
-/* Measurement aid for bench.py's roofline: launch stencil kernel `kernel_id` reps times back to back on the current
- * buffers between two CUDA events (after `warm` untimed launches) and return the mean milliseconds per launch.
- * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e, 9 fused forward
- * marching kernel, 10 slab kernels of the fused forward path (FDTD_ERR_UNSUPPORTED where the grid cannot fuse).  Needs a reverse
- * workspace and a completed forward for ids >= 2.  The field contents are garbage afterwards: call fdtd_reset.
- * Synchronises.  algo_bytes (may be NULL) receives the algorithmic bytes one launch moves. */
-fdtd_status fdtd_profile_kernel(fdtd_sim*, int kernel_id, int warm, int reps, double* ms_per_launch, double* algo_bytes);
-
-/* Number of kernels this library has launched on behalf of the handle since create (bench.py's gpu_launches). */
-unsigned long long fdtd_launch_count(const fdtd_sim*);
-
 #ifdef __cplusplus
 }
 #endif

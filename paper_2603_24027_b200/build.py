@@ -12,7 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdtd_b200.so")
 SOURCES = [os.path.join(CSRC, "fdtd_api.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fdtd_dev.cuh", "fdtd_stencil.cuh", "fdtd_store.cuh", "fdtd_fused.cuh")] + [
-    os.path.join(os.path.dirname(HERE), "include", "fdtd.h")]
+    os.path.join(os.path.dirname(HERE), "include", f) for f in ("fdtd.h", "fdtd_bench.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-fmad=false",
          "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]

@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "../../include/fdtd.h"
+#include "../../include/fdtd_bench.h"
 #include "fdtd_stencil.cuh"
 #include "fdtd_store.cuh"
 #include "fdtd_fused.cuh"
@@ -61,6 +62,7 @@ struct fdtd_sim {
   cudaGraphExec_t graph_cache[4] = {nullptr, nullptr, nullptr, nullptr};   // forward, fused forward, reverse, fused reverse
   mutable std::string err;
   const float* eps_dev = nullptr;
+  bool eps_owned = false;              // eps_dev points into the workspace (fdtd_set_eps_host)
   double cpml[4] = {0.8, 1.0, 0.01, 3.0};
   bool has_design = false;
   int dlo[3] = {0, 0, 0}, dhi[3] = {0, 0, 0};
@@ -1023,7 +1025,10 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
     const double fwd_bytes = 7.0 * 4.0 * (double)nx * ny * nz;
     s->zalign = (l2 > 0 && fwd_bytes > 1.5 * (double)l2) ? 32 : 16;
   }
-  if (const char* e = std::getenv("FDTD_ZALIGN")) s->zalign = atoi(e);
+  if (const char* e = std::getenv("FDTD_ZALIGN")) {   // debug knob: only multiples of 4 that are >= V keep the float4 accesses aligned
+    const int v = atoi(e);
+    if (v >= s->V && v % 4 == 0) s->zalign = v;
+  }
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
@@ -1081,6 +1086,16 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   if (reinterpret_cast<uintptr_t>(ws_dev) % 256) return fail(s, FDTD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
   const Layout L = make_layout(s, nsteps, (int)dt, k, flags);
   if (bytes < L.total) return fail(s, FDTD_ERR_OOM, "workspace too small: need %zu bytes, got %zu", L.total, bytes);
+  if (s->eps_owned) {
+    // eps came through fdtd_set_eps_host and lives in the PREVIOUS workspace, at an offset the new layout moves (or in a
+    // buffer the caller may already have freed): it cannot be carried over.
+    s->eps_owned = false;
+    s->eps_dev = nullptr;
+  }
+  if (!s->eps_dev) {
+    s->ws = nullptr;
+    return fail(s, FDTD_ERR_STATE, "eps was set through fdtd_set_eps_host into the previous workspace: call fdtd_set_eps first");
+  }
   s->ws = static_cast<char*>(ws_dev);
   s->ws_bytes = bytes; s->L = L; s->flags = flags;
   s->max_nsteps = nsteps; s->max_k = k; s->max_dtype = (int)dt;
@@ -1164,6 +1179,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
 fdtd_status fdtd_set_eps(fdtd_sim* s, const float* eps_dev) {
   if (!s || !eps_dev) return FDTD_ERR_INVALID_ARG;
   s->eps_dev = eps_dev;
+  s->eps_owned = false;
   if (!s->ws) return FDTD_OK;
   fdtd_status r = make_ce(s);
   if (r != FDTD_OK) return r;
@@ -1262,7 +1278,9 @@ fdtd_status fdtd_set_eps_host(fdtd_sim* s, const float* eps_host) {
   if (!s->ws || !(s->flags & FDTD_WS_HOST_IO)) return fail(s, FDTD_ERR_STATE, "needs a workspace with FDTD_WS_HOST_IO");
   float* own = reinterpret_cast<float*>(s->ws + s->L.eps_own);
   CUDA_TRY(s, cudaMemcpyAsync(own, eps_host, (size_t)s->d.N * 4, cudaMemcpyHostToDevice, s->stream));
-  return fdtd_set_eps(s, own);
+  const fdtd_status r = fdtd_set_eps(s, own);
+  s->eps_owned = r == FDTD_OK;   // eps now lives inside the workspace: fdtd_set_workspace must not keep this pointer
+  return r;
 }
 
 fdtd_status fdtd_forward_host(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k, float* mon_host) {
@@ -1369,18 +1387,23 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       }
     }
   };
-  cudaEvent_t e0, e1;
-  CUDA_TRY(s, cudaEventCreate(&e0));
-  CUDA_TRY(s, cudaEventCreate(&e1));
-  for (int r = 0; r < warm; ++r) once();
-  CUDA_TRY(s, cudaEventRecord(e0, s->stream));
-  for (int r = 0; r < reps; ++r) once();
-  CUDA_TRY(s, cudaEventRecord(e1, s->stream));
-  CUDA_TRY(s, cudaEventSynchronize(e1));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
   float ms = 0;
-  CUDA_TRY(s, cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
+  cudaError_t ce = cudaEventCreate(&e0);
+  if (ce == cudaSuccess) ce = cudaEventCreate(&e1);
+  if (ce == cudaSuccess) {
+    for (int r = 0; r < warm; ++r) once();
+    ce = cudaEventRecord(e0, s->stream);
+  }
+  if (ce == cudaSuccess) {
+    for (int r = 0; r < reps; ++r) once();
+    ce = cudaEventRecord(e1, s->stream);
+  }
+  if (ce == cudaSuccess) ce = cudaEventSynchronize(e1);
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  if (ce != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "fdtd_profile_kernel: %s", cudaGetErrorString(ce));
   CUDA_TRY(s, cudaGetLastError());
   *ms_out = (double)ms / reps;
   s->forward_done = s->state_final = false;

@@ -8,10 +8,19 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    txt = open(os.path.join(ROOT, "include", "fdtd.h")).read()
-    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(fdtd_[a-z_0-9]+)\s*\(", txt)))
+def _declared(headers=("fdtd.h", "fdtd_bench.h")):
+    names = set()
+    for h in headers:
+        txt = open(os.path.join(ROOT, "include", h)).read()
+        txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+        names |= set(re.findall(r"\b(fdtd_[a-z_0-9]+)\s*\(", txt))
+    return sorted(names)
+
+
+def test_bench_instrumentation_is_not_in_the_product_header():
+    product = _declared(("fdtd.h",))
+    assert "fdtd_profile_kernel" not in product and "fdtd_launch_count" not in product
+    assert set(_declared(("fdtd_bench.h",))) == {"fdtd_profile_kernel", "fdtd_launch_count"}
 
 
 def test_header_declares_the_four_north_star_calls():
