@@ -82,16 +82,89 @@ def whole_job_value(cells, nsteps, steps, world, total_ms):
     return float(cells) * nsteps * steps * world / (total_ms * 1e-3) / 1e6
 
 
-# DRAM bytes per launch of a kernel group (read + write, summed over the group's kernels) from the committed ncu --set full
-# captures (profiles/r01d_c2.md, r01e_c3_c2.md, r01c_full.md): what roofline.traffic reports beside the algorithmic bytes.  ncu flushes the caches
-# between launches, so on C2 (working set of the order of the L2) arrays that stay in L2 do not appear as writes.
-NCU_TRAFFIC = {
-    ("C2", "fwd_e"): 88.2e6, ("C2", "fwd_h"): 76.7e6, ("C2", "inv_h"): 32.2e6, ("C2", "adj_h"): 76.6e6,
-    ("C2", "grad_inv_e"): 44.3e6, ("C2", "adj_e"): 88.4e6,
-    ("C3", "fwd_e"): 364.7e6, ("C3", "fwd_h"): 314.7e6, ("C3", "inv_h"): 175.6e6, ("C3", "adj_h"): 335.2e6,
-    ("C3", "grad_inv_e"): 231.8e6, ("C3", "adj_e"): 382.7e6,
-    ("C4", "fwd_fused"): 6112.8e6, ("C4", "fwd_fused_slabs"): 3242.1e6,
+# DRAM bytes per launch of a kernel group (dram__bytes_read.sum + dram__bytes_write.sum, summed over the group's kernels) from
+# `ncu --set full` captures of THIS build: profiles/ncu_traffic.json, written by `python bench.py --ncu-import <raw.csv> ...`
+# from the raw page of a capture and stamped with a hash of the kernel sources.  A stamp that does not match the sources on disk
+# means the capture is stale: the traffic is then reported as null (with the reason), never silently reused.
+NCU_JSON = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+KERNEL_SOURCES = ["fdtd_api.cu", "fdtd_dev.cuh", "fdtd_stencil.cuh", "fdtd_store.cuh", "fdtd_fused.cuh"]
+# kernel group -> the kernels whose launches make up one "launch" of the group (names as ncu prints them, prefix match)
+GROUP_KERNELS = {
+    "fwd_e": ["k_row<0>", "k_lean_curlm<4, 0>", "k_lean_curlm<1, 0>", "k_gen_e"],
+    "fwd_h": ["k_row<1>", "k_lean_h", "k_gen_h"],
+    "inv_h": ["k_inv_h"],
+    "adj_h": ["k_row<2>", "k_lean_curlm<4, 1>", "k_lean_curlm<1, 1>", "k_gen_adj_h"],
+    "grad_inv_e": ["k_inv_e<", "k_grad("],
+    "adj_e": ["k_row<3>", "k_lean_adj_e", "k_gen_adj_e"],
+    "record": ["k_record"],
+    "inject_h": ["k_inject"],
+    "inject_e": ["k_inject"],
+    "fwd_fused": ["k_fused_he"],
+    "fwd_fused_slabs": ["k_gen_h", "k_gen_e"],
 }
+
+
+def kernel_source_hash():
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2603_24027_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def load_ncu_traffic(workload):
+    """{group: bytes per launch} for the workload, or ({}, reason) when there is no capture of this build."""
+    if not os.path.exists(NCU_JSON):
+        return {}, "no profiles/ncu_traffic.json"
+    with open(NCU_JSON) as f:
+        d = json.load(f)
+    e = d.get(workload)
+    if not e:
+        return {}, f"no ncu capture of {workload} in profiles/ncu_traffic.json"
+    if e.get("kernel_source_hash") != kernel_source_hash():
+        return {}, (f"ncu capture of {workload} is stale: taken from kernel sources {e.get('kernel_source_hash')}, "
+                    f"the sources on disk are {kernel_source_hash()}")
+    return e["groups"], e.get("source", "profiles/ncu_traffic.json")
+
+
+def ncu_import(args):
+    """bench.py --ncu-import raw.csv --workload W --ncu-note '...': read `ncu -i rep --page raw --csv` output of a capture
+    made by `ncu --set full ... python bench.py --workload W --profile-only ...` (every group launched once, in
+    Sim.KERNELS order) and store DRAM bytes per group launch in profiles/ncu_traffic.json."""
+    import csv
+    rows = list(csv.reader(open(args.ncu_import)))
+    hdr = rows[0]
+    ci = {n: hdr.index(n) for n in ("Kernel Name", "dram__bytes_read.sum", "dram__bytes_write.sum", "gpu__time_duration.sum")}
+    units = rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+
+    def by(r, n):
+        return float(r[ci[n]]) * scale[units[ci[n]]]
+    launches = [(r[ci["Kernel Name"]], by(r, "dram__bytes_read.sum"), by(r, "dram__bytes_write.sum"),
+                 float(r[ci["gpu__time_duration.sum"]])) for r in rows[2:]]
+    from paper_2603_24027_b200 import fdtd
+    groups, detail, pos = {}, {}, 0
+    for name in fdtd.Sim.KERNELS:
+        pref = GROUP_KERNELS[name]
+        got = []
+        while pos < len(launches) and any(launches[pos][0].replace("void ", "").replace("fdtd::", "").startswith(p) for p in pref) \
+                and len(got) < (2 if name not in ("inv_h", "inject_h", "inject_e", "fwd_fused") else 1):
+            got.append(launches[pos])
+            pos += 1
+        if not got:
+            continue
+        groups[name] = sum(g[1] + g[2] for g in got)
+        detail[name] = [{"kernel": g[0][:60], "read": g[1], "write": g[2], "us": g[3]} for g in got]
+    d = {}
+    if os.path.exists(NCU_JSON):
+        with open(NCU_JSON) as f:
+            d = json.load(f)
+    d[args.workload] = {"kernel_source_hash": kernel_source_hash(), "source": args.ncu_note or os.path.basename(args.ncu_import),
+                        "groups": groups, "launches": detail}
+    with open(NCU_JSON, "w") as f:
+        json.dump(d, f, indent=1)
+    print(json.dumps({"workload": args.workload, "groups": groups, "unmatched_launches": len(launches) - pos}))
 
 
 class ClockSampler:
@@ -140,6 +213,21 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def profile_kernels(sim, fdtd, w, flags, flush, reps, fused):
+    """Each kernel group timed alone on the library's stream (fdtd_profile_kernel): {name: {us, algo_bytes}}.  Needs a completed
+    forward run of at least 4*k steps (record / inject read the store)."""
+    out = {}
+    for kid, name in enumerate(fdtd.Sim.KERNELS):
+        if kid >= 9 and not fused:
+            continue
+        if 6 <= kid <= 8:
+            sim.forward(min(w.nsteps, 4 * w.k), w.sources, w.store_dtype, w.k, flags=flags)
+        flush.fill_(1)
+        ms, by = sim.profile_kernel(kid, warm=3 if reps > 1 else 0, reps=reps)
+        out[name] = {"us": ms * 1e3, "algo_bytes": by}
+    return out
+
+
 def run_gpu(args, rank, world):
     import torch
     import torch.distributed as dist
@@ -160,24 +248,23 @@ def run_gpu(args, rank, world):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     extra = {}
 
+    if args.profile_only:
+        # one launch of every kernel group, in Sim.KERNELS order, for an `ncu --set full` capture (see --ncu-import)
+        sim.forward(min(w.nsteps, 64), w.sources, w.store_dtype, w.k, flags=flags)
+        fused = sim.uses_fused(w.nsteps)
+        torch.cuda.synchronize()
+        torch.cuda.profiler.start()
+        k = profile_kernels(sim, fdtd, w, flags, flush, 1, fused)
+        torch.cuda.profiler.stop()
+        print(json.dumps({"profile_only": True, "workload": args.workload, "kernels": k, "kernel_source_hash": kernel_source_hash()}))
+        return
+
     def loss_cotangent_dev(mon):
         # harness-level objective on the small monitor tensor (SURVEY layer L4), on the device for the device-timed leg
         L, d = W.loss_and_cotangent(w, mon.cpu().numpy(), extra)
-        return L, torch.from_numpy(d.astype(np.float32)).to(dev)
+        return L, torch.from_numpy(d.astype(np.float32, copy=False)).to(dev)
 
-    # one untimed pass fixes the objective's constants (C3's target amplitude) and the cotangent, so that the timed
-    # device leg contains only library work
-    mon = sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
-    if w.loss == "pulse_shape":
-        A = np.asarray(w.extra["A"], dtype=np.float64).reshape(mon.shape[2:])
-        extra.update(w.extra)
-        extra["target_amp"] = 0.5 * float(np.max(np.abs(np.tensordot(mon[:, 0].cpu().numpy().astype(np.float64), A, axes=3))))
-    L0, dmon = loss_cotangent_dev(mon)
-    grad = sim.reverse(None, dmon, W.LINEAR)
-    sim.sync()
-    assert torch.isfinite(grad).all().item(), "gradient is not finite"
-    if not args.nsteps:
-        assert grad.abs().max().item() > 0, "gradient is zero on the full-length workload"
+    state = {"dmon": None, "L0": None, "grad": None}
 
     def barrier():
         torch.cuda.synchronize()
@@ -185,33 +272,51 @@ def run_gpu(args, rank, world):
             dist.barrier()
             torch.cuda.synchronize()
 
-    def one_step(timed):
+    def one_step():
         flush.fill_(1)                                # L2 flush between steps (not timed)
         e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
         torch.cuda.synchronize()
         e[0].record()
-        sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
+        mon = sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
         e[1].record()
-        sim.reverse(None, dmon, W.LINEAR)
+        if state["dmon"] is None:
+            # first (warm-up) pass: fix the objective's constants (C3's target amplitude) and the loss cotangent once, so that
+            # every later pass — all timed ones — contains only library work between the events
+            if w.loss == "pulse_shape":
+                A = np.asarray(w.extra["A"], dtype=np.float64).reshape(mon.shape[2:])
+                extra.update(w.extra)
+                extra["target_amp"] = 0.5 * float(np.max(np.abs(np.tensordot(mon[:, 0].cpu().numpy().astype(np.float64), A, axes=3))))
+            state["L0"], state["dmon"] = loss_cotangent_dev(mon)
+            e[1].record()
+        grad = sim.reverse(None, state["dmon"], W.LINEAR)
         e[2].record()
         torch.cuda.synchronize()
+        if state["grad"] is None:
+            state["grad"] = grad.clone()
         return e[0].elapsed_time(e[1]), e[1].elapsed_time(e[2])
 
     for _ in range(args.warmup):
-        one_step(False)
+        one_step()
+    grad = state["grad"]
+    assert torch.isfinite(grad).all().item(), "gradient is not finite"
+    if not args.nsteps:
+        assert grad.abs().max().item() > 0, "gradient is zero on the full-length workload"
     barrier()
     sampler = ClockSampler(local, args.clock_sample_ms) if rank == 0 else None
     l0 = sim.launch_count()
     t0 = time.time()
     tf, tr = [], []
     for _ in range(args.steps):
-        a, b = one_step(True)
+        a, b = one_step()
         tf.append(a)
         tr.append(b)
     barrier()
     t1 = time.time()
     launches = sim.launch_count() - l0
     clocks = sampler.stop(t0, t1) if sampler else None
+    store_bytes = int(sim.store_bytes())
+    nrec = sim.num_slots() - 1
+    slot_vals = int(sim.slot_values())
     tot_ms = float(np.sum(tf) + np.sum(tr))
     tot_ms, f_ms, r_ms = reduce_max([tot_ms, float(np.sum(tf)), float(np.sum(tr))], world, dev)
     value = whole_job_value(w.cells, w.nsteps, args.steps, world, tot_ms)
@@ -222,6 +327,7 @@ def run_gpu(args, rank, world):
     dmon_host = torch.empty(w.monitor_shape(), dtype=torch.float32).pin_memory()
     lo, hi = w.design
     grad_host = torch.empty([hi[a] - lo[a] for a in range(3)], dtype=torch.float32).pin_memory()
+    state["dmon"] = None                                 # the device cotangent is not needed any more (7.9 GB on C4)
 
     def e2e_step():
         sim.set_eps_host(eps_host)
@@ -230,9 +336,11 @@ def run_gpu(args, rank, world):
         dmon_host.copy_(torch.from_numpy(np.ascontiguousarray(d, dtype=np.float32)))
         sim.reverse_host(dmon_host, W.LINEAR, grad_host)
         return L
-    e2e_step()
+    # the device-timed passes above have warmed the GPU; a pass of the host-buffer path first only where it is cheap
+    ne2e = max(1, min(args.steps, 3)) if tot_ms / args.steps < 5e3 else 1
+    if tot_ms / args.steps < 5e3:
+        e2e_step()
     barrier()
-    ne2e = max(1, min(args.steps, 3))
     te = time.perf_counter()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
@@ -255,40 +363,46 @@ def run_gpu(args, rank, world):
             dist.destroy_process_group()
         return
 
-    # ---- per-kernel roofline (rank 0): each stencil kernel timed alone, back to back, CUDA events on its stream ----
+    # ---- per-kernel roofline (rank 0): each kernel group timed alone, back to back, CUDA events on its stream ----
     peak, peak_src = load_peaks()
-    sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
-    nrec = sim.num_slots() - 1
+    sim.forward(min(w.nsteps, 64), w.sources, w.store_dtype, w.k, flags=flags)
     fused = sim.uses_fused(w.nsteps)   # large grids: H half-step of step m and E half-step of step m+1 in one marching kernel
     counts = {"fwd_e": 1 if fused else w.nsteps, "fwd_h": 1 if fused else w.nsteps, "inv_h": w.nsteps, "adj_h": w.nsteps,
               "grad_inv_e": w.nsteps, "adj_e": w.nsteps, "record": nrec + 1, "inject_h": w.nsteps, "inject_e": w.nsteps,
               "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1}
-    kernels = {}
-    for kid, name in enumerate(fdtd.Sim.KERNELS):
-        if kid >= 9 and not fused:
-            continue
-        if 6 <= kid <= 8:
-            sim.forward(min(w.nsteps, 4 * w.k), w.sources, w.store_dtype, w.k, flags=flags)
-        flush.fill_(1)
-        ms, by = sim.profile_kernel(kid, warm=3, reps=20)
-        kernels[name] = {"us": ms * 1e3, "algo_bytes": by, "gbs": by / (ms * 1e-3) / 1e9, "launches_per_step": counts[name]}
-    tot = sum(v["us"] * v["launches_per_step"] for v in kernels.values())
-    for v in kernels.values():
-        v["share"] = v["us"] * v["launches_per_step"] / tot
-        v["frac"] = v["gbs"] / peak
+    kernels = profile_kernels(sim, fdtd, w, flags, flush, 20, fused)
+    traffic, traffic_src = load_ncu_traffic(args.workload if not (args.store or args.k or args.tangential) else "-")
+    tot = sum(v["us"] * counts[n] for n, v in kernels.items())
+    for n, v in kernels.items():
+        v["launches_per_step"] = counts[n]
+        v["share"] = v["us"] * counts[n] / tot
+        # algorithmic bytes (SURVEY 8(d) / DESIGN.md "Roofline") over the measured time: an EFFECTIVE bandwidth
+        v["effective_gbs"] = v["algo_bytes"] / (v["us"] * 1e-6) / 1e9
+        v["frac"] = v["effective_gbs"] / peak
+        # DRAM bytes of the same launch from the ncu capture of this build over the same measured time
+        v["dram_bytes"] = traffic.get(n)
+        v["dram_gbs"] = traffic[n] / (v["us"] * 1e-6) / 1e9 if n in traffic else None
+        v["dram_frac"] = v["dram_gbs"] / peak if n in traffic else None
     dom = max(kernels, key=lambda n: kernels[n]["share"])
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dom]["gbs"] / peak, "traffic": NCU_TRAFFIC.get((args.workload, dom)), "peak_source": peak_src,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch (all kernels of the group), ncu --set full, "
-                                  "profiles/r01d_c2.md, r01e_c3_c2.md, r01c_full.md" if (args.workload, dom) in NCU_TRAFFIC else None,
-                "how": "kernel group timed alone (its lean and general kernel side by side, as in the step): 20 back-to-back launches "
-                       "between CUDA events on the library's stream after 3 warm-up launches; achieved = algorithmic bytes per "
-                       "launch (DESIGN.md Roofline) / mean launch time",
-                "launch_us": kernels[dom]["us"], "algo_bytes": kernels[dom]["algo_bytes"]}
+    kd = kernels[dom]
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kd["effective_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kd["frac"], "traffic": kd["dram_bytes"], "peak_source": peak_src,
+                "traffic_source": ("dram__bytes_read.sum + dram__bytes_write.sum per launch (all kernels of the group), ncu --set full, "
+                                   + str(traffic_src)) if kd["dram_bytes"] is not None else f"null: {traffic_src}",
+                "dram_frac": kd["dram_frac"],
+                "how": "dominant kernel group (largest share of the step) timed alone, its kernels side by side as in the step: 20 "
+                       "back-to-back launches between CUDA events on the library's stream after 3 warm-up launches, L2 flushed before "
+                       "the series; achieved = ALGORITHMIC bytes per launch (DESIGN.md Roofline; SURVEY 8(d)) / mean launch time; "
+                       "dram_frac = ncu DRAM bytes of the same launch / the same time / peak",
+                "launch_us": kd["us"], "algo_bytes": kd["algo_bytes"]}
+    if dom == "adj_e":
+        # SURVEY 8(d)'s table counts the adjoint of the E half-step at 36 B per cell; the kernel also reads ce (S/eps): 40 B
+        survey = kd["algo_bytes"] - 4.0 * w.cells
+        roofline["survey_bytes"] = survey
+        roofline["frac_survey_bytes"] = survey / (kd["us"] * 1e-6) / 1e9 / peak
     # whole-pass effective bandwidth: algorithmic bytes of all stencil launches of one step / measured time
     fwd_names = ("fwd_e", "fwd_h", "fwd_fused", "fwd_fused_slabs")
-    algo_fwd = sum(kernels[n]["algo_bytes"] * kernels[n]["launches_per_step"] for n in fwd_names if n in kernels) \
-        + kernels["record"]["algo_bytes"] * (nrec + 1)
+    algo_fwd = sum(kernels[n]["algo_bytes"] * counts[n] for n in fwd_names if n in kernels) + kernels["record"]["algo_bytes"] * (nrec + 1)
     algo_rev = sum(kernels[n]["algo_bytes"] for n in ("inv_h", "adj_h", "grad_inv_e", "adj_e", "inject_h", "inject_e")) * w.nsteps
     fwd_gbs = algo_fwd / (f_ms / args.steps * 1e-3) / 1e9
     # the same forward time against the bytes of the two-kernel form (76 B per cell): comparable across paths
@@ -299,8 +413,11 @@ def run_gpu(args, rank, world):
     # ---- CPU baseline: the oracle as it stands on a bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if world == 1 and not args.no_cpu and not args.tangential:
+        del sim, flush
+        torch.cuda.empty_cache()
         cpu = cpu_baseline(args.workload, args.cpu_steps)
 
+    ws_mb = 13 * w.cells * 4 / 1e6
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": tot_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -309,21 +426,25 @@ def run_gpu(args, rank, world):
                                f"{W.DTYPE_NAMES[w.store_dtype]} store, k={w.k}, linear interpolation, loss={w.loss}",
                    "grid": list(w.shape), "pml": w.pml, "nsteps": w.nsteps, "store_dtype": W.DTYPE_NAMES[w.store_dtype], "k": w.k,
                    "store_components": "tangential (12 slices per slot)" if args.tangential else "all six per face (36 slices per slot)",
-                   "l2": "256 MB write between timed steps flushes L2; inside a step the working set "
-                         f"({13 * w.cells * 4 / 1e6:.0f} MB of fields) is what the workload itself keeps resident",
+                   "l2": (f"inputs larger than L2: every time step streams its working set ({ws_mb:.0f} MB of fields in the reverse run, "
+                          f"{7 * w.cells * 4 / 1e6:.0f} MB forward) from HBM; a 256 MB write also flushes L2 between timed steps")
+                         if 7 * w.cells * 4 > 1.5 * 126e6 else
+                         (f"256 MB write between timed steps flushes L2; inside a step the working set ({ws_mb:.0f} MB of fields) is of "
+                          "the order of the 126 MB L2, so per-kernel fractions are effective bandwidths, not DRAM traffic"),
                    "replicas": world, "parallelism": "replicas only (the path runs on one GPU)"},
         "forward_mcells_per_s": whole_job_value(w.cells, w.nsteps, args.steps, world, f_ms),
         "reverse_mcells_per_s": whole_job_value(w.cells, w.nsteps, args.steps, world, r_ms),
         "forward_ms": f_ms / args.steps, "reverse_ms": r_ms / args.steps,
-        "store_bytes": sim_store_bytes(sim, w, flags), "store_bytes_per_step": sim_store_bytes(sim, w, flags) / w.nsteps,
-        "store_bytes_f32_k1": (w.nsteps + 1) * sim.slot_values() * (3 if args.tangential else 1) * 4,   # all six components
+        "store_bytes": store_bytes, "store_bytes_per_step": store_bytes / w.nsteps,
+        "store_bytes_f32_k1": (w.nsteps + 1) * slot_vals * (3 if args.tangential else 1) * 4,   # all six components
         "effective_gbs": {"forward": fwd_gbs, "reverse": rev_gbs, "forward_frac_of_peak": fwd_gbs / peak,
                           "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused),
                           "forward_two_kernel_equivalent": fwd2_gbs, "forward_two_kernel_equivalent_frac": fwd2_gbs / peak,
                           # also against the nominal HBM3e figure (8000 GB/s)
-                          "forward_frac_of_nominal_8000": fwd_gbs / 8000.0, "reverse_frac_of_nominal_8000": rev_gbs / 8000.0},
+                          "forward_frac_of_nominal_8000": fwd_gbs / 8000.0, "reverse_frac_of_nominal_8000": rev_gbs / 8000.0,
+                          "note": "algorithmic bytes (SURVEY 8(d)) / measured time: effective bandwidths, not DRAM counters"},
         "roofline": roofline, "kernels": kernels, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
-        "loss": L0, "grad_abs_max": float(grad.abs().max().item()),
+        "loss": state["L0"], "grad_abs_max": float(grad.abs().max().item()),
     }
     if cpu is not None:
         out["cpu_baseline"] = cpu
@@ -332,43 +453,59 @@ def run_gpu(args, rank, world):
         dist.destroy_process_group()
 
 
-def sim_store_bytes(sim, w, flags):
-    if not sim.store_bytes():
-        sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
-    return int(sim.store_bytes())
+class OracleRunner:
+    """The CPU oracle (f32), as it stands, on the first `nsteps` time steps of workload w.  Built once (its arrays are
+    allocated at construction); every pass resets it to state 0 and runs forward + reverse."""
+
+    def __init__(self, w, nsteps):
+        import dataclasses
+        from oracle import fdtd_oracle as orc
+        self.orc = orc
+        srcs = [dataclasses.replace(s, wave=s.wave[:nsteps]) for s in w.sources]
+        self.ws = dataclasses.replace(w, nsteps=nsteps, sources=srcs)
+        self.s = orc.OracleSim(32, self.ws.eps, self.ws.pml, W.S)
+        self.s.set_design(*self.ws.design)
+        self.s.set_monitor(*self.ws.monitor)
+        for q in srcs:
+            self.s.add_source(q.comp, q.lo, q.hi, q.amp, q.wave)
+
+    def one_pass(self):
+        """(forward seconds, reverse seconds, threads)"""
+        ws, s = self.ws, self.s
+        s.reset()
+        t0 = time.perf_counter()
+        s.forward(ws.nsteps, ws.store_dtype, ws.k)
+        tf = time.perf_counter() - t0
+        ex = dict(ws.extra)
+        ex["target_amp"] = 1.0
+        L, d = W.loss_and_cotangent(ws, s.monitor_record(), ex)
+        t1 = time.perf_counter()
+        s.reverse(None, d, self.orc.LINEAR)
+        tr = time.perf_counter() - t1
+        return tf, tr, self.orc.get_threads()
 
 
-def oracle_pass(w, nsteps):
-    """One forward + reverse of the CPU oracle (f32) on the first nsteps of workload w.  Returns (seconds, cores)."""
-    import dataclasses
-    from oracle import fdtd_oracle as orc
-    srcs = [dataclasses.replace(s, wave=s.wave[:nsteps]) for s in w.sources]
-    ws = dataclasses.replace(w, nsteps=nsteps, sources=srcs)
-    s = orc.OracleSim(32, ws.eps, ws.pml, W.S)
-    s.set_design(*ws.design)
-    s.set_monitor(*ws.monitor)
-    for q in srcs:
-        s.add_source(q.comp, q.lo, q.hi, q.amp, q.wave)
-    t0 = time.perf_counter()
-    s.forward(nsteps, ws.store_dtype, ws.k)
-    tf = time.perf_counter() - t0
-    ex = dict(ws.extra)
-    ex["target_amp"] = 1.0
-    L, d = W.loss_and_cotangent(ws, s.monitor_record(), ex)
-    t1 = time.perf_counter()
-    s.reverse(None, d, orc.LINEAR)
-    tr = time.perf_counter() - t1
-    return tf, tr, orc.get_threads()
+def sample_description(w, nsteps, per_step=False):
+    first = min(getattr(s.wave, "size", 0) and int(np.argmax(np.abs(s.wave) > 1e-3 * np.abs(s.wave).max())) for s in w.sources) + 1
+    quiet = (f"; the source is still below 1e-3 of its peak until step {first}, so the sampled steps run on (near-)zero fields"
+             if first > nsteps else "")
+    return (f"{w.name} grid, first {nsteps} of {w.nsteps} time steps" + (" per bench step" if per_step else "") +
+            f", forward + reverse, float32 oracle, {W.DTYPE_NAMES[w.store_dtype]} k={w.k}{quiet}")
+
+
+def default_sample_steps(w, seconds):
+    """Time steps of the workload that the oracle gets through in about `seconds` (its measured ~40 Mcell-updates/s forward +
+    reverse on 16 cores), at least 2 (one stored slot interval needs two states), at most 60."""
+    return int(max(2, min(60, seconds * 40e6 / w.cells)))
 
 
 def cpu_baseline(workload, nsteps):
     w = make_workload(workload, None)
-    nsteps = min(nsteps, w.nsteps)
-    tf, tr, cores = oracle_pass(w, nsteps)
+    nsteps = min(nsteps or default_sample_steps(w, 15.0), w.nsteps)
+    tf, tr, cores = OracleRunner(w, nsteps).one_pass()
     cu = float(w.cells) * nsteps
     return {"value": cu / (tf + tr) / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{w.name} grid, first {nsteps} of {w.nsteps} steps, forward + reverse, float32 oracle, "
-                      f"{W.DTYPE_NAMES[w.store_dtype]} k={w.k}",
+            "sample": sample_description(w, nsteps),
             "forward_mcells_per_s": cu / tf / 1e6, "reverse_mcells_per_s": cu / tr / 1e6, "seconds": tf + tr}
 
 
@@ -377,17 +514,17 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     w = make_workload(args.workload, None)
-    sample = min(args.ref_steps, w.nsteps)
+    sample = min(args.ref_steps or default_sample_steps(w, 6.0), w.nsteps)
+    runner = OracleRunner(w, sample)
     for _ in range(args.warmup):
-        oracle_pass(w, sample)
+        runner.one_pass()
     t = 0.0
     cores = 0
     for _ in range(args.steps):
-        tf, tr, cores = oracle_pass(w, sample)
+        tf, tr, cores = runner.one_pass()
         t += tf + tr
     value = float(w.cells) * sample * args.steps / t / 1e6
-    desc = (f"{w.name} grid, first {sample} of {w.nsteps} steps per bench step, forward + reverse, float32 oracle, "
-            f"{W.DTYPE_NAMES[w.store_dtype]} k={w.k}")
+    desc = sample_description(w, sample, per_step=True)
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -406,10 +543,14 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4"],
+                    help="C4 (512^3, 10 000 steps, bf16 k=4: the largest single-GPU configuration, HBM-bound) is the default")
     ap.add_argument("--nsteps", type=int, default=0, help="override the workload's number of time steps")
-    ap.add_argument("--cpu-steps", type=int, default=60, help="time steps of the cpu_baseline sample")
-    ap.add_argument("--ref-steps", type=int, default=20, help="time steps per bench step of --impl reference")
+    ap.add_argument("--cpu-steps", type=int, default=0, help="time steps of the cpu_baseline sample (0: about 15 s of oracle work)")
+    ap.add_argument("--ref-steps", type=int, default=0, help="time steps per bench step of --impl reference (0: about 6 s of oracle work)")
+    ap.add_argument("--profile-only", action="store_true", help="launch every kernel group once (for an ncu --set full capture) and exit")
+    ap.add_argument("--ncu-import", default="", help="raw-page CSV of such a capture: store its DRAM bytes in profiles/ncu_traffic.json")
+    ap.add_argument("--ncu-note", default="", help="provenance string stored with --ncu-import")
     ap.add_argument("--store", default="", choices=[""] + sorted(STORE_BY_NAME), help="override the workload's store dtype")
     ap.add_argument("--k", type=int, default=0, help="override the workload's temporal subsampling factor")
     ap.add_argument("--tangential", action="store_true",
@@ -420,7 +561,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
-    if args.impl == "reference":
+    if args.ncu_import:
+        ncu_import(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_gpu(args, rank, world)

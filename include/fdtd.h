@@ -159,6 +159,10 @@ fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
  * in the fused reverse run: they are summed before being subtracted).  With the fused reverse run the fields left after
  * fdtd_reverse are state 0 on the interior only. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
+/* Row kernels: the plain cells and the z-slab cells of the same rows in one launch, so that whole rows
+ * are streamed.  mode -1 (default) = on grids that stream from HBM (forward working set > 1.5 x L2), 0 = never, 1 = whenever
+ * the vector path applies (nz % 4 == 0, pml_width % 4 == 0).  Bit-identical results in every mode.  Before fdtd_set_workspace. */
+fdtd_status fdtd_set_rows(fdtd_sim*, int mode);
 /* 1 if fdtd_forward(nsteps) would take the fused path with the current settings (after fdtd_set_workspace), else 0. */
 int fdtd_uses_fused(const fdtd_sim*, int nsteps);
 

@@ -23,6 +23,14 @@ fdtd_status fdtd_profile_kernel(fdtd_sim*, int kernel_id, int warm, int reps, do
 /* Number of kernels this library has launched on behalf of the handle since create (bench.py's gpu_launches). */
 unsigned long long fdtd_launch_count(const fdtd_sim*);
 
+/* Debugging aid standing in for compute-sanitizer (closed on the GPU pool this library is developed on).  With FDTD_WS_GUARD in
+ * the flags of fdtd_workspace_bytes / fdtd_set_workspace every sub-array of the workspace is followed by a 4 KiB guard band and
+ * the whole workspace starts as 0xFF bytes: a kernel that WRITES out of bounds dirties a guard band (counted here), a kernel that
+ * READS a guard band or a sub-array nobody initialised picks up a NaN that reaches the fields or the gradient (caught by the
+ * parity tests).  Returns the number of guard bytes that lost the pattern, -1 without a guarded workspace.  Synchronises. */
+#define FDTD_WS_GUARD 4u
+long long fdtd_debug_guard_check(fdtd_sim*);
+
 #ifdef __cplusplus
 }
 #endif

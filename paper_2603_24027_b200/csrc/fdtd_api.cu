@@ -35,7 +35,10 @@ struct Layout {
   size_t store_cap;
   int slots_cap;
   size_t total;
+  std::vector<std::pair<size_t, size_t>> guards;   // FDTD_WS_GUARD: (offset, bytes) of the guard band behind every sub-array
 };
+constexpr size_t kGuardBytes = 4096;
+constexpr unsigned kWsGuard = 4u;   // FDTD_WS_GUARD (include/fdtd_bench.h)
 
 }  // namespace
 
@@ -43,6 +46,8 @@ namespace {
 struct Split {          // one half-step over an x range: lean region + complement boxes
   Region reg{};
   bool has_lean = false;
+  bool rows = false;    // the lean launch is a ROW kernel that also covers the z-slab cells of its rows (no class-Z boxes)
+  int nlo = 0, nhi = 0; // its z-slab groups per row below / above the lean z range
   BoxList boxes{};
   int x0 = 0, x1 = 0;
 };
@@ -88,6 +93,8 @@ struct fdtd_sim {
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 16;           // planes per block of the fused marching kernels
+  bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
+  bool use_rows = true;    // vector path: row kernels (lean cells + the z-slab cells of the same rows in one launch)
   int zalign = 0;          // z alignment (cells) of the lean regions, chosen at create: 32 (128-byte lines) on grids that stream
                            // from HBM, 16 on grids that live in L2 (more cells for the slower general kernels otherwise)
   int store_mode = 0;      // 0: six components per face (R6); 1: tangential only (fdtd_set_store_mode)
@@ -172,7 +179,13 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   Layout L{};
   size_t o = 0;
   const size_t N = (size_t)s->n[0] * s->n[1] * s->n[2];
-  auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + std::max<size_t>(bytes, 4)); return r; };
+  const bool guard = (flags & kWsGuard) != 0;
+  auto take = [&](size_t bytes) {
+    size_t r = o;
+    o = align_up(o + std::max<size_t>(bytes, 4));
+    if (guard) { L.guards.emplace_back(o, kGuardBytes); o += kGuardBytes; }
+    return r;
+  };
   L.ce = take(N * 4);
   for (int c = 0; c < 3; ++c) L.E[c] = take(N * 4);
   for (int c = 0; c < 3; ++c) L.H[c] = take(N * 4);
@@ -307,11 +320,14 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
     }
     if (a == 2) {
       // z range of the lean region: whole groups of V cells, and (zalign > V) whole 128-byte lines, so that neither the lean
-      // nor the z-slab kernels fetch half-used lines (a row of the lean region then starts and ends on a line boundary)
-      const int za = (which < 4 && s->zalign > V && n % s->zalign == 0) ? s->zalign : V;
+      // nor the z-slab kernels fetch half-used lines (a row of the lean region then starts and ends on a line boundary).
+      // Row kernels stream whole rows anyway: groups of V cells only.
+      const bool rows = which < 4 && V == 4 && s->use_rows;
+      const int za = (which < 4 && !rows && s->zalign > V && n % s->zalign == 0) ? s->zalign : V;
       int lo2 = (lo + za - 1) / za * za, hi2 = hi / za * za;
       if (hi2 - lo2 < za) { lo2 = (lo + V - 1) / V * V; hi2 = hi / V * V; }
       lo = lo2; hi = hi2;
+      if (std::getenv("FDTD_DEBUG_FULLROW") && which < 4) { lo = 0; hi = n; }   // TIMING EXPERIMENT ONLY: wrong results
     }
     full.lo[a] = lo; full.hi[a] = hi;
   }
@@ -347,6 +363,13 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
   add(CLS_X, full.hi[0], nx, 0, ny, 0, nz);
   add(CLS_Y, full.lo[0], full.hi[0], 0, full.lo[1], 0, nz);
   add(CLS_Y, full.lo[0], full.hi[0], full.hi[1], ny, 0, nz);
+  if (which < 4 && V == 4 && s->use_rows && sp.has_lean && x0 <= full.lo[0] && x1 >= full.hi[0]) {
+    // the row kernel takes the z-slab cells of the lean x-y range itself
+    sp.rows = true;
+    sp.nlo = full.lo[2] / 4;
+    sp.nhi = (nz - full.hi[2]) / 4;
+    return sp;
+  }
   add(CLS_Z, full.lo[0], full.hi[0], full.lo[1], full.hi[1], 0, full.lo[2]);
   add(CLS_Z, full.lo[0], full.hi[0], full.lo[1], full.hi[1], full.hi[2], nz);
   return sp;
@@ -394,11 +417,25 @@ void join(fdtd_sim* s, int branches) {
   }
 }
 
-void launch_lean(fdtd_sim* s, int which, const Split& sp) {
+void launch_lean(fdtd_sim* s, int which, const Split& sp, int pb = 0) {
   if (!sp.has_lean) return;
   const dim3 b(32, TY);
   const dim3 g = grid_lean(s, sp.reg);
   const Region& r = sp.reg;
+  if (sp.rows) {
+    RowArgs ra;
+    ra.reg = r; ra.nlo = sp.nlo; ra.nhi = sp.nhi;
+    ra.ztiles = (int)g.x;
+    ra.ns = (ROW_RS * (sp.nlo + sp.nhi) + 32 * TY - 1) / (32 * TY);
+    const dim3 gr((unsigned)((ROW_RS / TY) * ra.ztiles + ra.ns), (unsigned)((r.hi[1] - r.lo[1] + ROW_RS - 1) / ROW_RS), g.z);
+    switch (which) {
+      case 0: LAUNCH(s, k_row<0>, gr, b, s->d, ra, pb); break;
+      case 1: LAUNCH(s, k_row<1>, gr, b, s->d, ra, pb); break;
+      case 2: LAUNCH(s, k_row<2>, gr, b, s->d, ra, pb); break;
+      default: LAUNCH(s, k_row<3>, gr, b, s->d, ra, pb);
+    }
+    return;
+  }
   if (s->V == 4) {
     switch (which) {
       case 0: LAUNCH(s, (k_lean_curlm<4, false>), g, b, s->d, r); break;
@@ -450,10 +487,10 @@ void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp, const FieldIO* 
   }
 }
 // The four split half-steps: lean kernel on the plain cells + general kernel on the rest (disjoint writes).
-void launch_lean(fdtd_sim* s, int which) { launch_lean(s, which, s->split[which]); }
+void launch_lean(fdtd_sim* s, int which, int pb = 0) { launch_lean(s, which, s->split[which], pb); }
 void launch_gen(fdtd_sim* s, int which, int pb) { launch_gen(s, which, pb, s->split[which]); }
 void launch_split(fdtd_sim* s, int which, int pb) {
-  launch_lean(s, which);
+  launch_lean(s, which, pb);
   launch_gen(s, which, pb);
 }
 void launch_inv_h(fdtd_sim* s) {
@@ -586,12 +623,12 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
     if (s->parallel) { cudaEventRecord(s->ev_mid, s->aux[0]); cudaStreamWaitEvent(s->stream, s->ev_mid, 0); }
   }
   launch_gen(s, 2, pb);
-  on(s, 0); launch_lean(s, 2);
+  on(s, 0); launch_lean(s, 2, pb);
   on(s, 2); launch_inv_h(s); launch_sources(s, m_base, step_dev, -1.0f);
   on(s, 3); launch_inject(s, m_base, step_dev, 1, interp);
   join(s, 4);
   fork(s, 4);
-  on(s, 0); launch_lean(s, 3);
+  on(s, 0); launch_lean(s, 3, pb);
   on(s, 1); launch_gen(s, 3, pb);
   on(s, 2); launch_inv_e(s); launch_grad(s);
   on(s, 3); launch_inject(s, m_base, step_dev, 0, interp);
@@ -682,7 +719,7 @@ void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const floa
     if (s->parallel) { cudaEventRecord(s->ev_mid, s->aux[0]); cudaStreamWaitEvent(s->stream, s->ev_mid, 0); }
   }
   launch_gen(s, 2, pb);
-  on(s, 0); launch_lean(s, 2);
+  on(s, 0); launch_lean(s, 2, pb);
   on(s, 2);
   launch_inject(s, m_base, step_dev, 1, interp, cur, oth);
   launch_fused(s, true, cur, oth);
@@ -690,7 +727,7 @@ void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const floa
   join(s, 3);
   set_cur(s, oth);
   fork(s, 4);
-  on(s, 0); launch_lean(s, 3);
+  on(s, 0); launch_lean(s, 3, pb);
   on(s, 1); launch_gen(s, 3, pb);
   on(s, 2); launch_grad(s);
   on(s, 3);
@@ -1024,11 +1061,16 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
     cudaGetLastError();
     const double fwd_bytes = 7.0 * 4.0 * (double)nx * ny * nz;
     s->zalign = (l2 > 0 && fwd_bytes > 1.5 * (double)l2) ? 32 : 16;
+    // Row kernels (fdtd_stencil.cuh: lean cells and the z-slab cells of the same rows in one launch) pay where the arrays stream
+    // from HBM (whole DRAM pages while they are open).  On a grid that lives in L2 (C2) the split with its own z-slab boxes is
+    // as fast or faster: forward H 13.4 us against 14.6, adjoint of E 17.9 against 18.2 (round 2, B200).
+    s->use_rows = s->rows_auto = l2 <= 0 || fwd_bytes > 1.5 * (double)l2;
   }
   if (const char* e = std::getenv("FDTD_ZALIGN")) {   // debug knob: only multiples of 4 that are >= V keep the float4 accesses aligned
     const int v = atoi(e);
     if (v >= s->V && v % 4 == 0) s->zalign = v;
   }
+  if (const char* e = std::getenv("FDTD_ROWS")) s->use_rows = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
@@ -1098,6 +1140,9 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   }
   s->ws = static_cast<char*>(ws_dev);
   s->ws_bytes = bytes; s->L = L; s->flags = flags;
+  // debugging aid (fdtd_bench.h): every byte of the workspace starts as 0xFF — guard bands keep that pattern unless a kernel writes
+  // out of bounds, and a float read from a guard band or from a sub-array nobody initialised is a NaN that reaches the results
+  if (flags & kWsGuard) CUDA_TRY(s, cudaMemsetAsync(ws_dev, 0xFF, L.total, s->stream));
   s->max_nsteps = nsteps; s->max_k = k; s->max_dtype = (int)dt;
   Dev& d = s->d;
   d = Dev{};
@@ -1209,6 +1254,13 @@ fdtd_status fdtd_set_store_mode(fdtd_sim* s, int mode) {
   if (!s || mode < 0 || mode > 1) return FDTD_ERR_INVALID_ARG;
   if (s->ws) return fail(s, FDTD_ERR_STATE, "fdtd_set_store_mode must precede fdtd_set_workspace");
   s->store_mode = mode;
+  return FDTD_OK;
+}
+
+fdtd_status fdtd_set_rows(fdtd_sim* s, int mode) {
+  if (!s || mode < -1 || mode > 1) return FDTD_ERR_INVALID_ARG;
+  if (s->ws) return fail(s, FDTD_ERR_STATE, "fdtd_set_rows must precede fdtd_set_workspace");
+  s->use_rows = mode < 0 ? s->rows_auto : mode == 1;
   return FDTD_OK;
 }
 
@@ -1351,11 +1403,11 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* cons
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
-  if (!s || id < 0 || id > 10 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s || id < 0 || id > 18 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
   if (id >= 6 && id <= 8 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
-  if (id >= 9 && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
+  if (id >= 9 && id <= 10 && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
   s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
   // a split half-step is timed in the launch configuration of the real step: lean and general kernel side by side
@@ -1380,6 +1432,8 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
       case 8: launch_inject(s, mrev, nullptr, 0, 0); break;
       case 9: launch_fused(s, false, s->cb, s->cb ^ 1); break;
+      case 11: case 12: case 13: case 14: launch_lean(s, id - 11); break;     // lean kernel of split half-step id - 11, alone
+      case 15: case 16: case 17: case 18: launch_gen(s, id - 15, 0); break;   // general kernel of split half-step id - 15, alone
       default: {
         const int cur = s->cb, oth = cur ^ 1;
         { const FieldIO io = io_of(s, cur, cur, oth, 1); launch_gen(s, 1, 0, s->split[5], &io); }
@@ -1437,6 +1491,16 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
         v = 52 * c;
         break;
       }
+      case 11: case 12: case 13: case 14: case 15: case 16: case 17: case 18: {
+        const int which = (id - 11) % 4;
+        const Region& r = s->split[which].reg;
+        double in = 1;
+        for (int a = 0; a < 3; ++a) in *= std::max(0, r.hi[a] - r.lo[a]);
+        if (!s->split[which].has_lean) in = 0;
+        const double per = (which == 0 || which == 3) ? 40 : 36;
+        v = id <= 14 ? per * in : per * (N - in) + 16 * slab;
+        break;
+      }
       default: {  // slab kernels of the fused path: H half-step on the complement of split 5, E half-step on that of split 4
         double in5 = 1, in4 = 1;
         for (int a = 0; a < 3; ++a) {
@@ -1449,6 +1513,19 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
     *bytes_out = v;
   }
   return FDTD_OK;
+}
+
+long long fdtd_debug_guard_check(fdtd_sim* s) {
+  if (!s || !s->ws || !(s->flags & kWsGuard)) return -1;
+  unsigned long long* cnt = reinterpret_cast<unsigned long long*>(s->ws + s->L.scratch);   // 16 bytes of scratch
+  unsigned long long zero = 0, bad = 0;
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return -1;
+  if (cudaMemcpy(cnt, &zero, 8, cudaMemcpyHostToDevice) != cudaSuccess) return -1;
+  for (const auto& g : s->L.guards)
+    k_guard_count<<<4, 256, 0, s->stream>>>(reinterpret_cast<const unsigned char*>(s->ws + g.first), g.second, cnt);
+  if (cudaStreamSynchronize(s->stream) != cudaSuccess) return -1;
+  if (cudaMemcpy(&bad, cnt, 8, cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+  return (long long)bad;
 }
 
 fdtd_status fdtd_sync(fdtd_sim* s) {

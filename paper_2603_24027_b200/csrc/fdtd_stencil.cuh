@@ -798,9 +798,7 @@ __device__ __forceinline__ bool lean_decode(const Region& r, int& i, int& j, int
 // ADJ = false: forward E half-step   E_c  = fma(ce, curl^-(H)_c,  E_c)      (row A1)
 // ADJ = true : adjoint of H half-step lE_c = fma(-S, curl^-(lH)_c, lE_c)     (row R4)
 template <int V, bool ADJ>
-__global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
-  int i, j, k0;
-  if (!lean_decode<V>(r, i, j, k0)) return;
+__device__ __forceinline__ void lean_curlm_body(const Dev& d, const int i, const int j, const int k0) {
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const float* const* in = ADJ ? d.lH : d.H;
@@ -829,9 +827,7 @@ __global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ 
 
 // forward H half-step on plain cells:  H_c = fma(-S, curl^+(E)_c, H_c)   (row A2)
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
-  int i, j, k0;
-  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
+__device__ __forceinline__ void lean_h_body(const Dev& d, const int i, const int j, const int k0) {
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
@@ -855,9 +851,7 @@ __global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev 
 
 // adjoint of the E half-step on plain cells:  lH_h = lH_h + curl^+(ce*lE)_h   (row R4)
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
-  int i, j, k0;
-  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
+__device__ __forceinline__ void lean_adj_e_body(const Dev& d, const int i, const int j, const int k0) {
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * d.n[1] + j) * d.n[2] + k0;
   const VF<V> ce = ldv_ce<V>(d, d.ce + q), ce_xp = ldv_ce<V>(d, d.ce + q + sx), ce_yp = ldv_ce<V>(d, d.ce + q + sy);
@@ -888,6 +882,91 @@ __global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ 
   stv<V>(d.lH[0] + q, lhx);
   stv<V>(d.lH[1] + q, lhy);
   stv<V>(d.lH[2] + q, lhz);
+}
+
+// the lean kernels proper (scalar path V = 1, and the per-kernel timings of fdtd_profile_kernel)
+template <int V, bool ADJ>
+__global__ void __launch_bounds__(32 * TY) k_lean_curlm(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V>(r, i, j, k0)) return;
+  lean_curlm_body<V, ADJ>(d, i, j, k0);
+}
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_lean_h(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
+  lean_h_body<V>(d, i, j, k0);
+}
+template <int V>
+__global__ void __launch_bounds__(32 * TY) k_lean_adj_e(const __grid_constant__ Dev d, const __grid_constant__ Region r) {
+  int i, j, k0;
+  if (!lean_decode<V, SWEEP_FLIP>(r, i, j, k0)) return;
+  lean_adj_e_body<V>(d, i, j, k0);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// ROW kernels (vector path): the lean cells and the z-slab cells of the same rows in ONE launch, so that every row of the
+// lean x-y range is streamed whole and DRAM pages are used in full while they are open.  A lean region that covers 256 of a
+// row's 512 bytes, next to a z-slab kernel that fetches the two 128-byte ends at a 512-byte stride somewhere else in the grid
+// (C3), ran at 0.70-0.79 of the measured copy bandwidth; with whole rows the lean half-steps alone measured 0.94-1.0 (round 2,
+// FDTD_DEBUG_FULLROW timing experiment: C3 forward E 76.3 -> 60.3 us, adjoint of E 82.6 -> 61.3 us; C4 forward E 927 -> 827 us).
+// Grid: x = blocks of one SUPER-TILE of ROW_RS rows: first its lean blocks (row tile of TY rows x z tile of 128 cells, exactly
+// the lean kernels' blocks), then `ns` SLAB blocks that pack the z-slab groups of those ROW_RS rows densely into their threads
+// (item -> row, group) and run the class-Z general body on them (z CPML terms, low z wall, high z ghost); y = super-tile;
+// z = plane.  Blocks are dispatched x-fastest, so the slab cells of a row are in flight together with its lean cells, and no
+// lean block waits for the (3x longer) slab body of a neighbour warp.
+// WHICH: 0 forward E, 1 forward H, 2 adjoint of H, 3 adjoint of E.  Same bodies as the split kernels: bit-identical results.
+// ---------------------------------------------------------------------------------------------------------
+// Resident blocks per SM the row kernels are compiled for (128 threads each): 6 (<= 85 registers, no spills) for the E-type and
+// adjoint kernels, 8 (64 registers, a few spilled words in the slab blocks only) for the forward H kernel.  Measured on B200,
+// group time in us, bounds 5 / 6 / 7 / 8: C4 forward E 834 / 834 / 849 / 872, forward H 847 / 847 / 815 / 799, adjoint of H
+// 815 / 790 / 810 / 824, adjoint of E 918 / 862 / 912 / 890; C3 forward E 64.6 / 64.9 / 67.0 / 71.2, adjoint of E 77.1 / 71.4 / 73.2 / 72.9.
+#ifndef FDTD_ROW_MINB
+#define FDTD_ROW_MINB(WHICH) ((WHICH) == 1 ? 8 : 6)
+#endif
+constexpr int ROW_RS = 4 * TY;   // rows per super-tile
+struct RowArgs {
+  Region reg;     // lean region; z bounds are multiples of 4
+  int nlo, nhi;   // z-slab groups (of 4 cells) per row below reg.lo[2] / from reg.hi[2] up to nz
+  int ztiles;     // lean blocks along z
+  int ns;         // slab blocks per super-tile
+};
+template <int WHICH>
+__global__ void __launch_bounds__(32 * TY, FDTD_ROW_MINB(WHICH)) k_row(const __grid_constant__ Dev d, const __grid_constant__ RowArgs r, const int pb) {
+  constexpr bool FLIP = SWEEP_FLIP && (WHICH == 1 || WHICH == 3);
+  const int i = FLIP ? r.reg.hi[0] - 1 - (int)blockIdx.z : r.reg.lo[0] + (int)blockIdx.z;
+  const int jsup = r.reg.lo[1] + (int)blockIdx.y * ROW_RS;
+  const int nlean = (ROW_RS / TY) * r.ztiles;
+  if ((int)blockIdx.x < nlean) {
+    const int rt = (int)blockIdx.x / r.ztiles, zt = (int)blockIdx.x - rt * r.ztiles;
+    const int k0 = r.reg.lo[2] + (zt * 32 + (int)threadIdx.x) * 4;
+    const int j = jsup + rt * TY + (int)threadIdx.y;
+    if (k0 >= r.reg.hi[2] || j >= r.reg.hi[1]) return;
+    if (WHICH == 0) lean_curlm_body<4, false>(d, i, j, k0);
+    else if (WHICH == 1) lean_h_body<4>(d, i, j, k0);
+    else if (WHICH == 2) lean_curlm_body<4, true>(d, i, j, k0);
+    else lean_adj_e_body<4>(d, i, j, k0);
+    return;
+  }
+  const int ng = r.nlo + r.nhi;
+  const int rows = min(ROW_RS, r.reg.hi[1] - jsup);
+  const int it = ((int)blockIdx.x - nlean) * (32 * TY) + (int)threadIdx.y * 32 + (int)threadIdx.x;
+  if (it >= rows * ng) return;
+  // items are numbered group-major inside a row, rows consecutive: a warp covers whole rows' slab groups
+  const int row = it / ng, g = it - row * ng;
+  const int k0 = g < r.nlo ? 4 * g : r.reg.hi[2] + 4 * (g - r.nlo);
+  const int j = jsup + row;
+  if (WHICH == 0 || WHICH == 1) {
+    FieldIO io;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { io.E[c] = d.E[c]; io.H[c] = d.H[c]; io.out[c] = WHICH == 0 ? d.E[c] : d.H[c]; }
+    if (WHICH == 0) gen_e_body<4, false, false>(d, i, j, k0, io);
+    else gen_h_body<4, false, false>(d, i, j, k0, io);
+  } else if (WHICH == 2) {
+    gen_adj_h_body<4, false, false>(d, i, j, k0, pb);
+  } else {
+    gen_adj_e_body<4, false, false>(d, i, j, k0, pb);
+  }
 }
 
 }  // namespace fdtd

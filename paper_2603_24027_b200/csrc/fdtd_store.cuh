@@ -463,6 +463,12 @@ __global__ void k_box(const __grid_constant__ Dev d, const __grid_constant__ Box
   else (comp < 3 ? d.lE[comp] : d.lH[comp - 3])[q] += rec[off];
 }
 
+// debugging aid (fdtd_debug_guard_check): bytes of a guard band that no longer hold the 0xFF fill pattern
+__global__ void k_guard_count(const unsigned char* p, size_t n, unsigned long long* bad) {
+  unsigned c = 0;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) c += p[t] != 0xFFu;
+  if (c) atomicAdd(bad, (unsigned long long)c);
+}
 __global__ void k_tick(int* step_dev, int delta) { *step_dev += delta; }
 __global__ void k_set_int(int* p, int v) { *p = v; }
 

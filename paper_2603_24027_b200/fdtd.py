@@ -17,6 +17,7 @@ F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14
 LINEAR, CUBIC = 0, 1
 STORE_ALL, STORE_TANGENTIAL = 0, 1
 WS_REVERSE, WS_HOST_IO = 1, 2
+WS_GUARD = 4   # debugging aid (include/fdtd_bench.h): guard bands + 0xFF fill
 STATUS = {0: "FDTD_OK", 1: "FDTD_ERR_INVALID_ARG", 2: "FDTD_ERR_OOM", 3: "FDTD_ERR_CUDA", 4: "FDTD_ERR_STATE",
           5: "FDTD_ERR_UNSUPPORTED"}
 ELEM_BYTES = {F32: 4, F16: 2, BF16: 2, F8E4M3_SCALED: 1, F8E4M3_MX32: 1, F8E4M3B11FNUZ: 1, F8E5M2FNUZ: 1, F8E4M3FNUZ: 1, F8E4M3: 1,
@@ -69,6 +70,7 @@ def lib():
     L.fdtd_set_graphs.argtypes = [vp, C.c_int]
     L.fdtd_set_fused.argtypes = [vp, C.c_int, C.c_int]
     L.fdtd_uses_fused.argtypes = [vp, C.c_int]
+    L.fdtd_set_rows.argtypes = [vp, C.c_int]
     L.fdtd_set_store_mode.argtypes = [vp, C.c_int]
     L.fdtd_get_fields.argtypes = [vp, vp]
     L.fdtd_get_adjoint.argtypes = [vp, vp]
@@ -91,16 +93,18 @@ def lib():
     L.fdtd_destroy.argtypes = [vp]
     L.fdtd_launch_count.restype = C.c_ulonglong
     L.fdtd_launch_count.argtypes = [vp]
+    L.fdtd_debug_guard_check.restype = C.c_longlong
+    L.fdtd_debug_guard_check.argtypes = [vp]
     _lib = L
     return L
 
 
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
-            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_uses_fused", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
+            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_set_rows", "fdtd_uses_fused", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_slot_bytes", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
-            "fdtd_launch_count"]
+            "fdtd_launch_count", "fdtd_debug_guard_check"]
 
 
 def _torch():
@@ -121,7 +125,7 @@ def _stream_ptr(torch):
 class Sim:
     """fdtd_sim handle.  eps: float32 CUDA tensor [nx,ny,nz] (kept alive by this object)."""
 
-    def __init__(self, eps, dx, dt, pml_width, design=None, monitor=None, cpml=None, store_mode=STORE_ALL):
+    def __init__(self, eps, dx, dt, pml_width, design=None, monitor=None, cpml=None, store_mode=STORE_ALL, rows=-1):
         torch = _torch()
         self._torch = torch
         self._L = lib()
@@ -145,6 +149,8 @@ class Sim:
         self.store_mode = int(store_mode)
         if store_mode != STORE_ALL:
             self._check(self._L.fdtd_set_store_mode(self._h, int(store_mode)))
+        if rows != -1:
+            self._check(self._L.fdtd_set_rows(self._h, int(rows)))
         if design is not None:
             self.design = (tuple(design[0]), tuple(design[1]))
             self._check(self._L.fdtd_set_design(self._h, _i3(design[0]), _i3(design[1])))
@@ -348,6 +354,10 @@ class Sim:
 
     def launch_count(self):
         return int(self._L.fdtd_launch_count(self._h))
+
+    def guard_check(self):
+        """Guard bytes overwritten since fdtd_set_workspace(flags | WS_GUARD); -1 without a guarded workspace."""
+        return int(self._L.fdtd_debug_guard_check(self._h))
 
 
 # ---- stand-alone codec (bit-exactness tests on identical slices) ----

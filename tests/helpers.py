@@ -40,11 +40,11 @@ def rel_l2(a, b):
 
 
 # ---- CUDA path (imported lazily so that CPU-only test runs never touch torch.cuda) ----
-def gpu_sim(w, cpml=None, store_mode=0):
+def gpu_sim(w, cpml=None, store_mode=0, rows=-1):
     import torch
     from paper_2603_24027_b200 import fdtd
     eps = torch.from_numpy(np.ascontiguousarray(w.eps, dtype=np.float32)).cuda()
-    return fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor, cpml=cpml, store_mode=store_mode)
+    return fdtd.Sim(eps, W.DX, W.DT, w.pml, design=w.design, monitor=w.monitor, cpml=cpml, store_mode=store_mode, rows=rows)
 
 
 def gpu_gradient(w, dtype, k, interp=0, extra=None, sim=None):

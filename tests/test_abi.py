@@ -20,7 +20,7 @@ def _declared(headers=("fdtd.h", "fdtd_bench.h")):
 def test_bench_instrumentation_is_not_in_the_product_header():
     product = _declared(("fdtd.h",))
     assert "fdtd_profile_kernel" not in product and "fdtd_launch_count" not in product
-    assert set(_declared(("fdtd_bench.h",))) == {"fdtd_profile_kernel", "fdtd_launch_count"}
+    assert set(_declared(("fdtd_bench.h",))) == {"fdtd_profile_kernel", "fdtd_launch_count", "fdtd_debug_guard_check"}
 
 
 def test_header_declares_the_four_north_star_calls():
