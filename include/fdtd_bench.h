@@ -15,8 +15,10 @@ extern "C" {
 /* Measurement aid for bench.py's roofline: launch stencil kernel `kernel_id` reps times back to back on the current
  * buffers between two CUDA events (after `warm` untimed launches) and return the mean milliseconds per launch.
  * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e, 9 fused forward
- * marching kernel, 10 slab kernels of the fused forward path (FDTD_ERR_UNSUPPORTED where the grid cannot fuse).  Needs a reverse
- * workspace and a completed forward for ids >= 2.  The field contents are garbage afterwards: call fdtd_reset.
+ * marching kernel, 10 slab kernels of the fused forward path (FDTD_ERR_UNSUPPORTED where the grid cannot fuse); 11-14 the
+ * lean / row kernel of split half-step id - 11 alone, 15-18 its general (slab-box) kernel alone.  Needs a reverse workspace for
+ * ids >= 2 and a completed forward run for ids 6-8 (its store stays readable through any sequence of these calls).  The field
+ * contents are garbage afterwards: call fdtd_reset.
  * Synchronises.  algo_bytes (may be NULL) receives the algorithmic bytes one launch moves. */
 fdtd_status fdtd_profile_kernel(fdtd_sim*, int kernel_id, int warm, int reps, double* ms_per_launch, double* algo_bytes);
 

@@ -1460,7 +1460,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
   if (ce != cudaSuccess) return fail(s, FDTD_ERR_CUDA, "fdtd_profile_kernel: %s", cudaGetErrorString(ce));
   CUDA_TRY(s, cudaGetLastError());
   *ms_out = (double)ms / reps;
-  s->forward_done = s->state_final = false;
+  s->state_final = false;   // the fields are garbage now; the store of the last forward run stays readable (ids 6-8)
   if (bytes_out) {
     // algorithmic bytes per launch: f32 arrays read / written once, psi read+written in the slabs
     const double N = (double)s->d.N;
