@@ -59,9 +59,9 @@ struct fdtd_sim {
   double dx = 0, dt = 0, Sd = 0;
   cudaStream_t stream = nullptr;
   cudaStream_t cur = nullptr;          // stream the next LAUNCH goes to (fork / on / join)
-  cudaStream_t aux[3] = {nullptr, nullptr, nullptr};
+  cudaStream_t aux[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaStream_t cap = nullptr;          // origin stream of graph captures (the caller's stream may be the legacy default)
-  cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+  cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[4] = {nullptr, nullptr, nullptr, nullptr};
   bool parallel = false;               // auxiliary streams available
   std::vector<cudaGraphExec_t> dead_graphs;
   cudaGraphExec_t graph_cache[4] = {nullptr, nullptr, nullptr, nullptr};   // forward, fused forward, reverse, fused reverse
@@ -94,6 +94,7 @@ struct fdtd_sim {
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 16;           // planes per block of the fused marching kernels
   bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
+  bool use_zf = true;      // vector path: the inverse kernels inject the interior cells of the two z faces (fdtd_stencil.cuh, ZF)
   bool use_rows = true;    // vector path: row kernels (lean cells + the z-slab cells of the same rows in one launch)
   int zalign = 0;          // z alignment (cells) of the lean regions, chosen at create: 32 (128-byte lines) on grids that stream
                            // from HBM, 16 on grids that live in L2 (more cells for the slower general kernels otherwise)
@@ -493,19 +494,27 @@ void launch_split(fdtd_sim* s, int which, int pb) {
   launch_lean(s, which, pb);
   launch_gen(s, which, pb);
 }
-void launch_inv_h(fdtd_sim* s) {
+// The inverse kernels of the vector path also inject the interior cells of the two z faces (fdtd_stencil.cuh, ZF)
+bool zface_fused(const fdtd_sim* s) { return s->V == 4 && s->use_zf; }
+void launch_inv_h(fdtd_sim* s, int m_base, const int* step_dev, int interp) {
   dim3 gi;
   if (!grid_inner(s, &gi)) return;
   const dim3 b(32, TY);
-  if (s->V == 4) LAUNCH(s, k_inv_h<4>, gi, b, s->d);
-  else LAUNCH(s, k_inv_h<1>, gi, b, s->d);
+  ZInj z;
+  z.st = s->st; z.m_base = m_base; z.step_dev = step_dev; z.interp = interp;
+  if (zface_fused(s)) { FDTD_DT_SWITCH(s->dtype, LAUNCH(s, (k_inv_h<4, DT, true>), gi, b, s->d, z)) }
+  else if (s->V == 4) LAUNCH(s, (k_inv_h<4, DT_F32, false>), gi, b, s->d, z);
+  else LAUNCH(s, (k_inv_h<1, DT_F32, false>), gi, b, s->d, z);
 }
-void launch_inv_e(fdtd_sim* s) {
+void launch_inv_e(fdtd_sim* s, int m_base, const int* step_dev, int interp) {
   dim3 gi;
   if (!grid_inner(s, &gi)) return;
   const dim3 b(32, TY);
-  if (s->V == 4) LAUNCH(s, k_inv_e<4>, gi, b, s->d);
-  else LAUNCH(s, k_inv_e<1>, gi, b, s->d);
+  ZInj z;
+  z.st = s->st; z.m_base = m_base; z.step_dev = step_dev; z.interp = interp;
+  if (zface_fused(s)) { FDTD_DT_SWITCH(s->dtype, LAUNCH(s, (k_inv_e<4, DT, true>), gi, b, s->d, z)) }
+  else if (s->V == 4) LAUNCH(s, (k_inv_e<4, DT_F32, false>), gi, b, s->d, z);
+  else LAUNCH(s, (k_inv_e<1, DT_F32, false>), gi, b, s->d, z);
 }
 // design ∩ inner interior extents; false if empty
 bool grad_extents(const fdtd_sim* s, int ext[3]) {
@@ -561,14 +570,17 @@ void launch_record(fdtd_sim* s, int m_base, const int* step_dev, int half) {
 }
 // from / to: buffer that holds the shell E of state m / buffer that receives the injected values (-1 = the current one)
 void launch_inject(fdtd_sim* s, int m_base, const int* step_dev, int magnetic, int interp, int from = -1, int to = -1) {
-  const unsigned g = (unsigned)((s->st.cell_off[6] + 255) / 256);
+  // beside the two-kernel reverse primal of the vector path the z faces are injected by the inverse kernels themselves
+  const int nfaces = (from < 0 && to < 0 && zface_fused(s)) ? 4 : 6;
+  const unsigned g = (unsigned)((s->st.cell_off[nfaces] + 255) / 256);
+  if (g == 0) return;
   InjIO io;
   for (int c = 0; c < 3; ++c) {
     io.Eold[c] = from < 0 ? s->d.E[c] : s->fb[from][c];
     io.Eout[c] = to < 0 ? s->d.E[c] : s->fb[to][c];
     io.Hout[c] = to < 0 ? s->d.H[c] : s->fb[to][3 + c];
   }
-  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_inject<DT>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp, io))
+  FDTD_DT_SWITCH(s->dtype, LAUNCH(s, k_inject<DT>, g, 256, s->d, s->st, m_base, step_dev, magnetic, interp, io, nfaces))
 }
 
 // One forward step m-1 -> m (R2): E half-step (+CPML), sources, H half-step (+CPML), monitor, record.
@@ -624,15 +636,16 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
   }
   launch_gen(s, 2, pb);
   on(s, 0); launch_lean(s, 2, pb);
-  on(s, 2); launch_inv_h(s); launch_sources(s, m_base, step_dev, -1.0f);
+  on(s, 2); launch_inv_h(s, m_base, step_dev, interp); launch_sources(s, m_base, step_dev, -1.0f);
   on(s, 3); launch_inject(s, m_base, step_dev, 1, interp);
   join(s, 4);
-  fork(s, 4);
+  fork(s, 5);
   on(s, 0); launch_lean(s, 3, pb);
   on(s, 1); launch_gen(s, 3, pb);
-  on(s, 2); launch_inv_e(s); launch_grad(s);
+  on(s, 2); launch_inv_e(s, m_base, step_dev, interp);
   on(s, 3); launch_inject(s, m_base, step_dev, 0, interp);
-  join(s, 4);
+  on(s, 4); launch_grad(s);   // reads H^{m-1/2} and lambda_E (read-only in this phase), adds to inner design cells only
+  join(s, 5);
 }
 
 // ---- fused path (fdtd_fused.cuh): H half-step of step m and E half-step of step m+1 in one marching kernel ----
@@ -643,6 +656,10 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     a.Eout[c] = s->fb[to][c]; a.Hout[c] = s->fb[to][3 + c];
   }
   for (int ax = 0; ax < 3; ++ax) { a.lo[ax] = s->P + 1; a.hi[ax] = s->n[ax] - s->P - (inv ? 1 : 0); }
+  // forward: start on a whole group of 4 z cells.  The slab kernels' box lists (split 4, 5) cover z < P + 4 anyway (their lean z
+  // range is rounded to groups), and a first group with one cell masked out cost every warp of the first z tile 24 scalar stores
+  // per plane beside its 6 vector stores
+  if (!inv) a.lo[2] = (a.lo[2] + 3) / 4 * 4;
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
   a.xseg = s->xseg;
   const int zbase = a.lo[2] / 4 * 4, zlast = (a.hi[2] - 1) / 4 * 4, groups = (zlast - zbase) / 4 + 1;
@@ -712,6 +729,7 @@ void forward_fused_step(fdtd_sim* s, int m_base, const int* step_dev, bool rec, 
 void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
   const bool cot = dmon && s->has_mon;
   const int cur = s->cb, oth = cur ^ 1;
+  const bool alone = s->fuse_rev_mode == 2;   // the marching kernel gets a phase of its own
   fork(s, 3);
   on(s, 1);
   if (cot) {
@@ -722,9 +740,10 @@ void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const floa
   on(s, 0); launch_lean(s, 2, pb);
   on(s, 2);
   launch_inject(s, m_base, step_dev, 1, interp, cur, oth);
+  if (alone) join(s, 3);
   launch_fused(s, true, cur, oth);
   launch_inv_e_sources(s, m_base, step_dev, cur, oth);
-  join(s, 3);
+  if (!alone) join(s, 3);
   set_cur(s, oth);
   fork(s, 4);
   on(s, 0); launch_lean(s, 3, pb);
@@ -872,7 +891,7 @@ bool use_fused_reverse(const fdtd_sim* s) {
   // mode -1 (auto): off.  Measured on B200 (round 1, C4): bit-identical to the two-kernel reverse primal and 2.5 GB fewer
   // bytes per step, but the step is not faster (3406 vs 3395 us): beside the adjoint kernels the marching kernel runs at
   // 1.23 ms instead of the 1.03 ms of its forward twin.  Kept as an option (fdtd_set_fused mode 1).
-  return s->fuse_rev_mode == 1 && s->can_fuse;
+  return s->fuse_rev_mode >= 1 && s->can_fuse;
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
@@ -1051,7 +1070,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   s->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
   s->cur = s->stream;
   if (const char* e = std::getenv("FDTD_FUSE")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_mode = v; }
-  if (const char* e = std::getenv("FDTD_FUSE_REV")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_rev_mode = v; }
+  if (const char* e = std::getenv("FDTD_FUSE_REV")) { const int v = atoi(e); if (v >= -1 && v <= 2) s->fuse_rev_mode = v; }
   {
     // DRAM is fetched in whole 128-byte lines: a lean region that starts 64 bytes into a row (P = 16) costs the lean AND the
     // z-slab kernel a half-used line per row end (measured on C3: reads 33 % above the arrays' size, profiles/r01d_c3.md)
@@ -1071,14 +1090,19 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
     if (v >= s->V && v % 4 == 0) s->zalign = v;
   }
   if (const char* e = std::getenv("FDTD_ROWS")) s->use_rows = atoi(e) != 0;
+  // z-face injection inside the inverse kernels: the two threads per row that do it make their whole warp walk the fetch path, so
+  // it pays where a row is several warps long.  Measured (round 2, B200): C4 (4 warps per row) reverse 3176 -> 3106 us per step;
+  // C3 (1 warp per row) 226.6 -> 238.4, C2 57.2 -> 63.1: off there.
+  s->use_zf = nz - 2 * pml_width > 256;
+  if (const char* e = std::getenv("FDTD_ZF")) s->use_zf = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
-  for (int b = 0; b < 3 && ok; ++b)
+  for (int b = 0; b < 4 && ok; ++b)
     ok = cudaStreamCreateWithFlags(&s->aux[b], cudaStreamNonBlocking) == cudaSuccess &&
          cudaEventCreateWithFlags(&s->ev_join[b], cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaStreamCreateWithFlags(&s->cap, cudaStreamNonBlocking) == cudaSuccess;
-  if (!ok) { for (int b = 0; b < 3; ++b) s->aux[b] = nullptr; cudaGetLastError(); }   // graphs off, serial launches
+  if (!ok) { for (int b = 0; b < 4; ++b) s->aux[b] = nullptr; cudaGetLastError(); }   // graphs off, serial launches
   *out = s;
   return FDTD_OK;
 }
@@ -1403,11 +1427,11 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* cons
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
-  if (!s || id < 0 || id > 18 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s || id < 0 || id > 19 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
-  if (id >= 6 && id <= 8 && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
-  if (id >= 9 && id <= 10 && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
+  if (((id >= 6 && id <= 8) || id == 2 || id == 4) && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
+  if ((id == 9 || id == 10 || id == 19) && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
   s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
   // a split half-step is timed in the launch configuration of the real step: lean and general kernel side by side
@@ -1424,14 +1448,24 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
     switch (id) {
       case 0: split_pair(0); break;
       case 1: split_pair(1); break;
-      case 2: launch_inv_h(s); break;
+      case 2: launch_inv_h(s, mrev, nullptr, 0); break;
       case 3: split_pair(2); break;
-      case 4: launch_inv_e(s); launch_grad(s); break;
+      case 4: {   // inverse-E and gradient side by side, as in the step
+        const bool was = s->parallel;
+        s->parallel = s->aux[0] != nullptr;
+        fork(s, 2);
+        on(s, 1); launch_grad(s);
+        on(s, 0); launch_inv_e(s, mrev, nullptr, 0);
+        join(s, 2);
+        s->parallel = was;
+        break;
+      }
       case 5: split_pair(3); break;
       case 6: launch_record(s, s->nsteps, nullptr, 2); break;
       case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
       case 8: launch_inject(s, mrev, nullptr, 0, 0); break;
       case 9: launch_fused(s, false, s->cb, s->cb ^ 1); break;
+      case 19: launch_fused(s, true, s->cb, s->cb ^ 1); break;   // reverse marching kernel (inverse-H + inverse-E), alone
       case 11: case 12: case 13: case 14: launch_lean(s, id - 11); break;     // lean kernel of split half-step id - 11, alone
       case 15: case 16: case 17: case 18: launch_gen(s, id - 15, 0); break;   // general kernel of split half-step id - 15, alone
       default: {
@@ -1474,17 +1508,24 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       for (int a = 0; a < 3; ++a) dcells *= std::max(0, std::min(s->dhi[a], s->n[a] - s->P - 1) - std::max(s->dlo[a], s->P + 1));
     }
     const double eb = elem_bytes_host(s->dtype);
-    double shell = (double)s->st.cell_off[6];
+    // shell cells k_inject handles, and those the inverse kernels inject themselves (interior cells of the two z faces)
+    const double zin = zface_fused(s) ? 2.0 * std::max(0, s->n[0] - 2 * s->P - 2) * std::max(0, s->n[1] - 2 * s->P - 2) : 0.0;
+    const double shell = (double)s->st.cell_off[6] - zin;
+    const double zbytes = (s->store_mode == 1 ? 1.0 : 3.0) * zin * (2 * eb + 4);
     double v = 0;
     switch (id) {
       case 0: v = 40 * N + 16 * slab; break;          // E rw (24) + H (12) + ce (4); 2 psi arrays rw per slab-cell-axis
       case 1: v = 36 * N + 16 * slab; break;          // H rw (24) + E (12)
-      case 2: v = 36 * Ninner; break;
+      case 2: v = 36 * Ninner + zbytes; break;
       case 3: v = 36 * N + 16 * slab; break;          // lE rw + lH; lpsiH read (old) + written (new)
-      case 4: v = 40 * Ninner + 28 * dcells; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
+      case 4: v = 40 * Ninner + 28 * dcells + zbytes; break;   // E rw + H + ce; design: lE (12) + f64 acc rw (16)
       case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
       case 6: v = (double)s->st.slot_values * 4 + (double)slot_bytes_host(s, s->dtype); break;   // f32 gathered, slot written (block scales included)
       case 7: case 8: v = (s->store_mode == 1 ? 1.0 : 3.0) * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+      case 19: {  // reverse marching kernel: 52 B per inner-interior cell
+        v = 52 * Ninner;
+        break;
+      }
       case 9: {   // fused marching kernel: E, H read once and written once, ce read: 52 B per cell of [P+1, n-P)^3
         double c = 1;
         for (int a = 0; a < 3; ++a) c *= std::max(0, s->n[a] - 2 * s->P - 1);
@@ -1544,7 +1585,7 @@ void fdtd_destroy(fdtd_sim* s) {
   reap_graphs(s);
   for (int g = 0; g < 4; ++g)
     if (s->graph_cache[g]) cudaGraphExecDestroy(s->graph_cache[g]);
-  for (int b = 0; b < 3; ++b) {
+  for (int b = 0; b < 4; ++b) {
     if (s->aux[b]) cudaStreamDestroy(s->aux[b]);
     if (s->ev_join[b]) cudaEventDestroy(s->ev_join[b]);
   }

@@ -39,8 +39,10 @@ struct FusedArgs {
 
 template <bool INV>
 __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __grid_constant__ Dev d, const __grid_constant__ FusedArgs a) {
-  __shared__ float4 shH[2][FUSED_TR + 1][32][2];   // new Hx, Hz of the current plane, double-buffered over the march
-  __shared__ float4 shE[2][FUSED_TR + 1][32][2];   // Ex, Ez of the NEXT plane (read one march step later by the row below)
+  // [buffer][warp][component][lane]: a warp's 128-bit accesses are contiguous (lane-major, 16 bytes apart), hence free of bank
+  // conflicts; with [lane][component] (32 bytes apart) ncu counted 8-way conflicts on every shared load and store
+  __shared__ float4 shH[2][FUSED_TR + 1][2][32];   // new Hx, Hz of the current plane, double-buffered over the march
+  __shared__ float4 shE[2][FUSED_TR + 1][2][32];   // Ex, Ez of the NEXT plane (read one march step later by the row below)
   const int lane = threadIdx.x, w = threadIdx.y;
   const int ny = d.n[1], nz = d.n[2];
   const int zbase = (a.lo[2] / 4) * 4;            // first stored group of tile 0
@@ -71,7 +73,7 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __gri
     VF<4> hx = ldv<4>(a.Hin[0] + q), hy = ldv<4>(a.Hin[1] + q), hz = ldv<4>(a.Hin[2] + q);
     VF<4> ex_yp, ez_yp;
     if (yp_smem && i >= xs) {
-      const float4 t0 = shE[buf][w + 1][lane][0], t1 = shE[buf][w + 1][lane][1];
+      const float4 t0 = shE[buf][w + 1][0][lane], t1 = shE[buf][w + 1][1][lane];
       ex_yp.v[0] = t0.x; ex_yp.v[1] = t0.y; ex_yp.v[2] = t0.z; ex_yp.v[3] = t0.w;
       ez_yp.v[0] = t1.x; ez_yp.v[1] = t1.y; ez_yp.v[2] = t1.z; ez_yp.v[3] = t1.w;
     } else {
@@ -113,14 +115,14 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __gri
     }
     // ---- hand the new H to the row above (shared memory) and to the lane above (shuffle); E of the next plane to the
     //      row below for the next march step ----
-    shH[buf][w][lane][0] = make_float4(hx.v[0], hx.v[1], hx.v[2], hx.v[3]);
-    shH[buf][w][lane][1] = make_float4(hz.v[0], hz.v[1], hz.v[2], hz.v[3]);
-    shE[buf ^ 1][w][lane][0] = make_float4(exn.v[0], exn.v[1], exn.v[2], exn.v[3]);
-    shE[buf ^ 1][w][lane][1] = make_float4(ezn.v[0], ezn.v[1], ezn.v[2], ezn.v[3]);
+    shH[buf][w][0][lane] = make_float4(hx.v[0], hx.v[1], hx.v[2], hx.v[3]);
+    shH[buf][w][1][lane] = make_float4(hz.v[0], hz.v[1], hz.v[2], hz.v[3]);
+    shE[buf ^ 1][w][0][lane] = make_float4(exn.v[0], exn.v[1], exn.v[2], exn.v[3]);
+    shE[buf ^ 1][w][1][lane] = make_float4(ezn.v[0], ezn.v[1], ezn.v[2], ezn.v[3]);
     const float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
     __syncthreads();
     if (store_plane) {
-      const float4 t0 = shH[buf][w - 1][lane][0], t1 = shH[buf][w - 1][lane][1];
+      const float4 t0 = shH[buf][w - 1][0][lane], t1 = shH[buf][w - 1][1][lane];
       const float hx_ym[4] = {t0.x, t0.y, t0.z, t0.w}, hz_ym[4] = {t1.x, t1.y, t1.z, t1.w};
       VF<4> eo;
       VF<4> e1, e2;

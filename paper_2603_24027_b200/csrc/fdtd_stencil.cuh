@@ -10,6 +10,7 @@
 //    the thin z slabs still fill their warps.
 #pragma once
 #include "fdtd_dev.cuh"
+#include "fdtd_store.cuh"
 
 namespace fdtd {
 
@@ -299,9 +300,50 @@ __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int 
 // elements outside the inner interior are neither computed nor written.  Grid: x = z groups, y = rows from P+1, z = planes
 // from P+1.
 // ---------------------------------------------------------------------------------------------------------
+// Z-face injection inside the inverse kernels (ZF, vector path): the interface cells of the two z faces, (i, j, P) and
+// (i, j, n-P-1), are the elements just outside a row's inner-interior range — element 0 of its first group of 4 cells and
+// element 3 of its last one.  The thread that owns such a group fetches the dequantised, interpolated shell values (row R1)
+// itself and stores the group whole.  Done from k_inject, these cells are a scatter of 4-byte writes at a stride of one row
+// (one 32-byte DRAM sector read, modified and written per value: 1.4 M of them per half-step on 512^3), which cost the reverse
+// step 137 us of 3177 on C4 although inject moves 1 % of the step's bytes; here they ride on lines that are written anyway, and
+// the inverse kernels lose their element-wise stores at the row ends.  Interior cells of a z face belong to no other face, so
+// the ownership rule of DESIGN.md R9 is untouched; k_inject keeps the x and y faces (contiguous along z).
+struct ZInj {
+  StoreDev st;
+  int m_base;
+  const int* step_dev;
+  int interp;
+};
+// values of the three components (magnetic: H, else E) of z-face `side` at (i, j); returns a bit mask of the components stored
+template <int DT>
+__device__ __forceinline__ unsigned zface_fetch(const Dev& d, const ZInj& z, const FetchPlan& p, int side, int i, int j, bool magnetic,
+                                                float out[3]) {
+  const StoreDev& s = z.st;
+  const int f = 4 + side;
+  const long long e = (long long)(i - d.P) * s.dv[f] + (j - d.P);
+  const long long fs = (long long)s.du[f] * s.dv[f];
+  const long long nb = s.blkc_off[f + 1] - s.blkc_off[f], b0 = s.blk_off[f] + (e >> 5);
+  unsigned mask = 0;
+  if (s.mode == 1) {   // tangential store: H (x, y) on the low face, E (x, y) on the high face
+    if (side != (magnetic ? 0 : 1)) return 0;
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc) {
+      out[cc] = fetch_value<DT>(s, p, f * 6 + (magnetic ? 3 + cc : cc), s.val_off[f] + cc * fs + e, b0 + cc * nb);
+      mask |= 1u << cc;
+    }
+    return mask;
+  }
+#pragma unroll
+  for (int cc = 0; cc < 3; ++cc) {
+    const int comp = magnetic ? 3 + cc : cc;
+    out[cc] = fetch_value<DT>(s, p, f * 6 + comp, s.val_off[f] + comp * fs + e, b0 + comp * nb);
+  }
+  return 7u;
+}
+
 // inverse of the H half-step:  H^{m-1/2} = H^{m+1/2} + S * curl^+(E^m)
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d) {
+template <int V, int DT, bool ZF>
+__global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d, const __grid_constant__ ZInj z) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const int klo = P + 1, khi = nz - P - 1;
   const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
@@ -311,6 +353,14 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const float S = d.S;
+  const bool part_lo = k0 < klo, part_hi = k0 + V > khi;
+  float zlo[3], zhi[3];
+  unsigned mlo = 0, mhi = 0;
+  if (ZF && (part_lo || part_hi)) {   // shell values first: their loads overlap with everything below
+    const FetchPlan p = make_plan(cur_step(z.m_base, z.step_dev) - 1, z.st.nsteps, z.st.k, z.st.nslots, z.interp);
+    if (part_lo) mlo = zface_fetch<DT>(d, z, p, 0, i, j, true, zlo);
+    if (part_hi) mhi = zface_fetch<DT>(d, z, p, 1, i, j, true, zhi);
+  }
   const VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   const VF<V> ey_xp = ldv<V>(d.E[1] + q + sx), ez_xp = ldv<V>(d.E[2] + q + sx);
   const VF<V> ex_yp = ldv<V>(d.E[0] + q + sy), ez_yp = ldv<V>(d.E[2] + q + sy);
@@ -330,8 +380,25 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
     hy.v[v] = fmaf(S, (ex_zq - ex.v[v]) - (ez_xp.v[v] - ez.v[v]), hy.v[v]);
     hz.v[v] = fmaf(S, (ey_xp.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
   }
+  if (ZF) {
+    // the shell elements take the injected values (components the store does not hold keep what the arrays hold)
+    if (part_lo) {
+      if (mlo & 1u) hx.v[0] = zlo[0];
+      if (mlo & 2u) hy.v[0] = zlo[1];
+      if (mlo & 4u) hz.v[0] = zlo[2];
+    }
+    if (part_hi) {
+      if (mhi & 1u) hx.v[V - 1] = zhi[0];
+      if (mhi & 2u) hy.v[V - 1] = zhi[1];
+      if (mhi & 4u) hz.v[V - 1] = zhi[2];
+    }
+    stv<V>(d.H[0] + q, hx);
+    stv<V>(d.H[1] + q, hy);
+    stv<V>(d.H[2] + q, hz);
+    return;
+  }
   // a group that straddles the shell must not touch the shell cells: inject H runs concurrently with this kernel
-  if (k0 >= klo && k0 + V <= khi) {
+  if (!part_lo && !part_hi) {
     stv<V>(d.H[0] + q, hx);
     stv<V>(d.H[1] + q, hy);
     stv<V>(d.H[2] + q, hz);
@@ -346,9 +413,24 @@ __global__ void __launch_bounds__(32 * TY) k_inv_h(const __grid_constant__ Dev d
   }
 }
 
+// shell-cell gradient term in its dE form (R9 step 4), shared with k_inject's arithmetic:
+//   acc += sum_c lE_c * ((E_old - E_new)_c / ce)   on design ∩ shell
+__device__ __forceinline__ void shell_grad(const Dev& d, int i, int j, int k, idx_t qc, const float eold[3], const float enew[3], float cev) {
+  if (!(d.has_design && i >= d.dlo[0] && i < d.dhi[0] && j >= d.dlo[1] && j < d.dhi[1] && k >= d.dlo[2] && k < d.dhi[2])) return;
+  const double ce = (double)cev;
+  double sacc = 0.0;
+#pragma unroll
+  for (int cc = 0; cc < 3; ++cc) {
+    const float dE = eold[cc] - enew[cc];
+    sacc += (double)d.lE[cc][qc] * ((double)dE / ce);
+  }
+  const long long ei = ((long long)(i - d.dlo[0]) * (d.dhi[1] - d.dlo[1]) + (j - d.dlo[1])) * (d.dhi[2] - d.dlo[2]) + (k - d.dlo[2]);
+  d.acc[ei] += sacc;
+}
+
 // inverse of the E half-step (row R2):  E^{m-1} = E^m - ce * curl^-(H^{m-1/2})   on the inner interior
-template <int V>
-__global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d) {
+template <int V, int DT, bool ZF>
+__global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d, const __grid_constant__ ZInj z) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const int klo = P + 1, khi = nz - P - 1;
   const int k0 = (klo / V) * V + (blockIdx.x * 32 + threadIdx.x) * V;
@@ -357,12 +439,21 @@ __global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d
   if (k0 >= khi || j >= ny - P - 1 || i >= nx - P - 1) return;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
+  const bool part_lo = k0 < klo, part_hi = k0 + V > khi;
+  float zlo[3], zhi[3];
+  unsigned mlo = 0, mhi = 0;
+  if (ZF && (part_lo || part_hi)) {
+    const FetchPlan p = make_plan(cur_step(z.m_base, z.step_dev) - 1, z.st.nsteps, z.st.k, z.st.nslots, z.interp);
+    if (part_lo) mlo = zface_fetch<DT>(d, z, p, 0, i, j, false, zlo);
+    if (part_hi) mhi = zface_fetch<DT>(d, z, p, 1, i, j, false, zhi);
+  }
   const VF<V> hx = ldv<V>(d.H[0] + q), hy = ldv<V>(d.H[1] + q), hz = ldv<V>(d.H[2] + q);
   const VF<V> hy_xm = ldv<V>(d.H[1] + q - sx), hz_xm = ldv<V>(d.H[2] + q - sx);
   const VF<V> hx_ym = ldv<V>(d.H[0] + q - sy), hz_ym = ldv<V>(d.H[2] + q - sy);
   const float hx_z0 = d.H[0][q - 1], hy_z0 = d.H[1][q - 1];   // k0 >= 1: the inner interior starts at P + 1
   VF<V> ex = ldv<V>(d.E[0] + q), ey = ldv<V>(d.E[1] + q), ez = ldv<V>(d.E[2] + q);
   const VF<V> ce = ldv_ce<V>(d, d.ce + q);
+  const float eold_lo[3] = {ex.v[0], ey.v[0], ez.v[0]}, eold_hi[3] = {ex.v[V - 1], ey.v[V - 1], ez.v[V - 1]};
 #pragma unroll
   for (int v = 0; v < V; ++v) {
     const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
@@ -374,7 +465,31 @@ __global__ void __launch_bounds__(32 * TY) k_inv_e(const __grid_constant__ Dev d
     ey.v[v] = fmaf(-ce.v[v], cy, ey.v[v]);
     ez.v[v] = fmaf(-ce.v[v], cz, ez.v[v]);
   }
-  if (k0 >= klo && k0 + V <= khi) {   // see k_inv_h: inject E runs concurrently on the shell cells
+  if (ZF) {
+    // Shell elements: E_new = the injected value (a component the store does not hold keeps E_old: tangential store, where the
+    // design box cannot touch the shell); the gradient term of design ∩ shell uses E_old, exactly as k_inject does.
+    if (part_lo) {
+      float en[3] = {eold_lo[0], eold_lo[1], eold_lo[2]};
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+        if (mlo >> cc & 1u) en[cc] = zlo[cc];
+      if (mlo == 7u) shell_grad(d, i, j, k0, q, eold_lo, en, ce.v[0]);
+      ex.v[0] = en[0]; ey.v[0] = en[1]; ez.v[0] = en[2];
+    }
+    if (part_hi) {
+      float en[3] = {eold_hi[0], eold_hi[1], eold_hi[2]};
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+        if (mhi >> cc & 1u) en[cc] = zhi[cc];
+      if (mhi == 7u) shell_grad(d, i, j, k0 + V - 1, q + (V - 1), eold_hi, en, ce.v[V - 1]);
+      ex.v[V - 1] = en[0]; ey.v[V - 1] = en[1]; ez.v[V - 1] = en[2];
+    }
+    stv<V>(d.E[0] + q, ex);
+    stv<V>(d.E[1] + q, ey);
+    stv<V>(d.E[2] + q, ez);
+    return;
+  }
+  if (!part_lo && !part_hi) {   // see k_inv_h: inject E runs concurrently on the shell cells
     stv<V>(d.E[0] + q, ex);
     stv<V>(d.E[1] + q, ey);
     stv<V>(d.E[2] + q, ez);

@@ -343,9 +343,11 @@ struct InjIO {
 template <int DT>
 __global__ void __launch_bounds__(256) k_inject(const __grid_constant__ Dev d, const __grid_constant__ StoreDev s,
                                                 int m_base, const int* step_dev, int magnetic, int interp,
-                                                const __grid_constant__ InjIO io) {
+                                                const __grid_constant__ InjIO io, int nfaces) {
+  // nfaces = 6, or 4 where the inverse kernels inject the interior cells of the two z faces themselves (fdtd_stencil.cuh, ZF);
+  // the z faces' edge cells belong to an x or y face anyway
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= s.cell_off[6]) return;
+  if (t >= s.cell_off[nfaces]) return;
   const int nstate = cur_step(m_base, step_dev) - 1;
   const int f = find_face(s.cell_off, t);
   const long long e = t - s.cell_off[f];

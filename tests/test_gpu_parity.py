@@ -640,6 +640,35 @@ def test_row_kernels_match_split_kernels_and_oracle(which, graphs):
         assert np.array_equal(res[0][key], res[1][key]), key
 
 
+@pytest.mark.parametrize("which,dtype,k,interp,store_mode", [("c1", W.F32, 1, W.LINEAR, 0), ("c1", W.F8E4M3_SCALED, 8, W.CUBIC, 0),
+                                                             ("mid", W.BF16, 4, W.LINEAR, 0), ("wide", W.F8E4M3_MX32, 3, W.CUBIC, 0),
+                                                             ("mid", W.F16, 4, W.LINEAR, 1)])
+def test_zface_injection_in_the_inverse_kernels_matches_k_inject(monkeypatch, which, dtype, k, interp, store_mode):
+    """Vector path, rows several warps long (the library's own choice on 512^3; forced here with FDTD_ZF=1): the inverse kernels
+    inject the interior cells of the two z faces themselves (and take their shell gradient term); FDTD_ZF=0 leaves all six faces
+    to k_inject.  Same bits either way: gradient, reconstructed state 0, adjoint fields."""
+    w = _rows_workload(which)
+    if store_mode:
+        w = _inner_design(w)
+    o = oracle_gradient(w, 32, dtype, k, interp, store_mode=store_mode)
+    res = {}
+    for zf in ("0", "1"):
+        monkeypatch.setenv("FDTD_ZF", zf)
+        s = gpu_sim(w, store_mode=store_mode)
+        res[zf] = gpu_gradient(w, dtype, k, interp, sim=s)
+        res[zf]["adj"] = s.adjoint().cpu().numpy()
+    monkeypatch.delenv("FDTD_ZF")
+    f_err, g_err = _report(f"z-face injection {which} dtype={dtype} k={k} mode={store_mode}", res["1"], o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    P = w.pml
+    interior = (slice(None),) + tuple(slice(P + (1 if store_mode else 0), n - P - (1 if store_mode else 0)) for n in w.shape)
+    for key in ("final", "mon", "grad", "adj"):
+        assert np.array_equal(res["0"][key], res["1"][key]), key
+    assert np.array_equal(res["0"]["state0"][interior], res["1"]["state0"][interior])
+    peak = np.abs(o["final"]).max()
+    assert np.abs((res["1"]["state0"] - o["state0"])[interior]).max() <= 1e-5 * peak
+
+
 # ---------------------------------------------------------------------------------------------------------
 # Own memory checks (compute-sanitizer is closed on this GPU pool): guard bands behind every sub-array of the workspace and a
 # 0xFF (NaN) fill.  An out-of-bounds write dirties a guard band; an out-of-bounds or uninitialised read puts a NaN into the
