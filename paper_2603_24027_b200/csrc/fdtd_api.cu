@@ -29,7 +29,7 @@ constexpr double kC0 = 299792458.0;
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-  size_t ce, E[3], H[3], E2[3], H2[3], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
+  size_t ce, E[3], H[3], E2[3], H2[3], pHz2[2], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
   size_t lE[3], lH[3], lpsiE[2][3][2], lpsiH[2][3][2], acc;
   size_t eps_own, mon_stage, grad_stage, amp_stage;
   size_t store_cap;
@@ -89,11 +89,14 @@ struct fdtd_sim {
   // E/H buffer pair(s): fb[b][0..2] = E, fb[b][3..5] = H of buffer b; d.E / d.H always point at the current one (cb)
   float* fb[2][6] = {{nullptr}};
   int cb = 0;
+  float* pz[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // psi_H of the z axis per buffer: [b][0] H_x term, [b][1] H_y term
+  bool fuse_z = false;     // the fused forward path uses the whole-row marching kernel (k_fused_fz): no class-Z slab boxes
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
-  int xseg = 16;           // planes per block of the fused marching kernels
+  int xseg = 0;            // planes per block of the fused marching kernels (0: chosen by fused_xseg)
   bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
+  bool use_fz = true;      // fused forward path: whole-row marching kernel (k_fused_fz) instead of k_fused_he + class-Z slab boxes
   bool use_zf = true;      // vector path: the inverse kernels inject the interior cells of the two z faces (fdtd_stencil.cuh, ZF)
   bool use_rows = true;    // vector path: row kernels (lean cells + the z-slab cells of the same rows in one launch)
   int zalign = 0;          // z alignment (cells) of the lean regions, chosen at create: 32 (128-byte lines) on grids that stream
@@ -193,6 +196,7 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   if (s->V == 4 && s->P >= 4) {   // ping-pong partners of E and H for the fused marching kernels
     for (int c = 0; c < 3; ++c) L.E2[c] = take(N * 4);
     for (int c = 0; c < 3; ++c) L.H2[c] = take(N * 4);
+    for (int t = 0; t < 2; ++t) L.pHz2[t] = take((size_t)psi_elems(s, 2) * 4);   // partners of psi_H of the z axis (k_fused_fz)
   }
   for (int c = 0; c < 3; ++c)
     for (int t = 0; t < 2; ++t) L.psiE[c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
@@ -319,7 +323,8 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
       case 4: lo = P + 1; hi = n - P; break;                          // fused-path E: layer P joins the slab boxes
       default: lo = P + 1; hi = n - P - 1; break;                     // fused-path H: layers P and n-P-1 join them
     }
-    if (a == 2) {
+    if (a == 2 && which >= 4 && s->fuse_z) { lo = 0; hi = n; }   // whole-row marching kernel: z-slab cells ride on their rows
+    else if (a == 2) {
       // z range of the lean region: whole groups of V cells, and (zalign > V) whole 128-byte lines, so that neither the lean
       // nor the z-slab kernels fetch half-used lines (a row of the lean region then starts and ends on a line boundary).
       // Row kernels stream whole rows anyway: groups of V cells only.
@@ -392,6 +397,7 @@ bool grid_inner(const fdtd_sim* s, dim3* g) {
 void set_cur(fdtd_sim* s, int b) {
   s->cb = b;
   for (int c = 0; c < 3; ++c) { s->d.E[c] = s->fb[b][c]; s->d.H[c] = s->fb[b][3 + c]; }
+  if (s->pz[b][0]) { s->d.psiH[0][1] = s->pz[b][0]; s->d.psiH[1][0] = s->pz[b][1]; }   // ping-ponged with the fields
 }
 
 #define LAUNCH(s, kern, grid, block, ...)            \
@@ -456,6 +462,7 @@ void launch_lean(fdtd_sim* s, int which, const Split& sp, int pb = 0) {
 FieldIO io_inplace(const fdtd_sim* s, int which) {   // which: 0 = E half-step, 1 = H half-step
   FieldIO io;
   for (int c = 0; c < 3; ++c) { io.E[c] = s->d.E[c]; io.H[c] = s->d.H[c]; io.out[c] = which == 0 ? s->d.E[c] : s->d.H[c]; }
+  io_psi_inplace(io, s->d);
   return io;
 }
 void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp, const FieldIO* iop = nullptr) {
@@ -649,6 +656,19 @@ void reverse_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmo
 }
 
 // ---- fused path (fdtd_fused.cuh): H half-step of step m and E half-step of step m+1 in one marching kernel ----
+long long fused_tiles(const fdtd_sim* s, int xseg) {
+  long long tiles = s->fuse_z ? (s->n[2] / 4 + 31) / 32 : ((s->n[2] - 2 * s->P) / 4 + FUSED_ZG - 1) / FUSED_ZG;
+  tiles *= (s->n[1] - 2 * s->P + FUSED_TR - 1) / FUSED_TR;
+  tiles *= (s->n[0] - 2 * s->P + xseg - 1) / xseg;
+  return tiles;
+}
+// planes a block of the marching kernels walks: 32 where that still leaves four waves of tiles (3 blocks per SM), else 16.
+// Measured on B200 (round 2, whole-row kernel): C4 forward per 400 steps at 8 / 16 / 24 / 32 / 64 planes 605.9 / 592.7 / 586.5 /
+// 586.5 / 585.8 ms; C3 per 2000 steps at 4 / 8 / 12 / 16 planes 242.7 / 232.8 / 245.9 / 223.5 ms.
+int fused_xseg(const fdtd_sim* s) {
+  if (s->xseg > 0) return s->xseg;
+  return fused_tiles(s, 32) >= 4 * 3 * 148 ? 32 : 16;
+}
 void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   FusedArgs a;
   for (int c = 0; c < 3; ++c) {
@@ -661,7 +681,22 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   // per plane beside its 6 vector stores
   if (!inv) a.lo[2] = (a.lo[2] + 3) / 4 * 4;
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
-  a.xseg = s->xseg;
+  a.xseg = fused_xseg(s);
+  if (!inv && s->fuse_z) {   // whole rows, z CPML terms in the edge lanes (k_fused_fz)
+    FusedZArgs z;
+    for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
+    for (int t = 0; t < 2; ++t) { z.pHz_in[t] = s->pz[from][t]; z.pHz_out[t] = s->pz[to][t]; }
+    z.pEz[0] = s->d.psiE[0][1]; z.pEz[1] = s->d.psiE[1][0];
+    for (int ax = 0; ax < 2; ++ax) { z.lo[ax] = a.lo[ax]; z.hi[ax] = a.hi[ax]; }
+    z.xseg = a.xseg;
+    const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
+                  (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
+    static bool attr_set = false;   // more than 48 KB of shared memory per block: opt in once
+    if (!attr_set) { cudaFuncSetAttribute(k_fused_fz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedZSmem)); attr_set = true; }
+    k_fused_fz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedZSmem), s->cur>>>(s->d, z);
+    ++s->launches;
+    return;
+  }
   const int zbase = a.lo[2] / 4 * 4, zlast = (a.hi[2] - 1) / 4 * 4, groups = (zlast - zbase) / 4 + 1;
   const dim3 g((unsigned)((groups + FUSED_ZG - 1) / FUSED_ZG), (unsigned)((a.hi[1] - a.lo[1] + FUSED_TR - 1) / FUSED_TR),
                (unsigned)((a.hi[0] - a.lo[0] + a.xseg - 1) / a.xseg));
@@ -689,6 +724,13 @@ void launch_inv_e_sources(fdtd_sim* s, int m_base, const int* step_dev, int from
 FieldIO io_of(const fdtd_sim* s, int eb, int hb, int ob, int out_is_h) {
   FieldIO io;
   for (int c = 0; c < 3; ++c) { io.E[c] = s->fb[eb][c]; io.H[c] = s->fb[hb][3 + c]; io.out[c] = s->fb[ob][out_is_h ? 3 + c : c]; }
+  // psi_H of the z axis: in place, except in the whole-row fused path, where the H half-step (out_is_h) goes from the current
+  // buffer's psi to the other buffer's (pz[b][0..1], ping-ponged with the fields)
+  if (s->fuse_z && out_is_h) {
+    for (int t = 0; t < 2; ++t) { io.pHz_in[t] = s->pz[hb][t]; io.pHz_out[t] = s->pz[ob][t]; }
+  } else {
+    io_psi_inplace(io, s->d);
+  }
   return io;
 }
 // Fused forward step m (fdtd_fused.cuh): from (E^m incl. sources, H^{m-1/2}) in the current buffer to (E^{m+1}, H^{m+1/2}) in
@@ -805,6 +847,8 @@ fdtd_status zero_state(fdtd_sim* s) {
   set_cur(s, 0);
   for (int c = 0; c < 6; ++c)
     if (s->fb[1][c]) CUDA_TRY(s, cudaMemsetAsync(s->fb[1][c], 0, N * 4, s->stream));
+  for (int t = 0; t < 2; ++t)
+    if (s->pz[1][t] && psi_elems(s, 2)) CUDA_TRY(s, cudaMemsetAsync(s->pz[1][t], 0, (size_t)psi_elems(s, 2) * 4, s->stream));
   for (int c = 0; c < 3; ++c) {
     CUDA_TRY(s, cudaMemsetAsync(s->d.E[c], 0, N * 4, s->stream));
     CUDA_TRY(s, cudaMemsetAsync(s->d.H[c], 0, N * 4, s->stream));
@@ -879,12 +923,12 @@ fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int 
 bool use_fused(const fdtd_sim* s, int nsteps) {
   if (!s->can_fuse || nsteps < 2 || s->fuse_mode == 0) return false;
   if (s->fuse_mode == 1) return true;
-  // mode -1 (auto): only where the marching kernel has several waves of tiles (3 blocks per SM).  Measured on B200 (round 1):
-  // C4 (512^3, 7200 tiles) forward 1910 -> 1727 us per step; C3 (392 tiles) 159 -> 161; C2 (169 tiles at xseg 8) 35 -> 44.
-  long long tiles = ((s->n[2] - 2 * s->P) / 4 + FUSED_ZG - 1) / FUSED_ZG;
-  tiles *= (s->n[1] - 2 * s->P + FUSED_TR - 1) / FUSED_TR;
-  tiles *= (s->n[0] - 2 * s->P + s->xseg - 1) / s->xseg;
-  return tiles >= 4 * 3 * 148;
+  // mode -1 (auto): where the marching kernel fills most of one wave of tiles (3 blocks per SM = 444 slots).  Round 1 (k_fused_he
+  // beside class-Z slab boxes) paid only with several waves: C4 (7200 tiles) forward 1910 -> 1727 us per step, C3 (392 tiles)
+  // 159 -> 161, C2 35 -> 44.  With the whole-row kernel (k_fused_fz, round 2): C4 1631 -> 1466 us per step against the split
+  // path with row kernels, C3 (392 tiles) 129.8 -> 111.8; C2 (91 tiles) 29.1 -> 67.3: stays split.
+  if (!s->fuse_z) return fused_tiles(s, fused_xseg(s)) >= 4 * 3 * 148;
+  return fused_tiles(s, 16) >= 2 * 148;
 }
 bool use_fused_reverse(const fdtd_sim* s) {
   if (s->fuse_rev_mode == 0) return false;
@@ -1095,6 +1139,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   // C3 (1 warp per row) 226.6 -> 238.4, C2 57.2 -> 63.1: off there.
   s->use_zf = nz - 2 * pml_width > 256;
   if (const char* e = std::getenv("FDTD_ZF")) s->use_zf = atoi(e) != 0;
+  if (const char* e = std::getenv("FDTD_FZ")) s->use_fz = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
@@ -1179,6 +1224,13 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   char* w = s->ws;
   d.ce = reinterpret_cast<float*>(w + L.ce);
   s->can_fuse = s->V == 4 && s->P >= 4;
+  {
+    // whole-row marching kernel: every tile boundary (a multiple of 128 cells) must have a plain cell right below it, because an
+    // edge lane recomputes the new H of that cell without CPML terms
+    bool ok = s->can_fuse && s->use_fz && 2 * s->P <= 4 * FUSED_ZSL;   // the staging area of the slab lanes
+    for (int kb = 128; ok && kb < s->n[2]; kb += 128) ok = kb - 1 >= s->P && kb - 1 < s->n[2] - s->P;
+    s->fuse_z = ok;
+  }
   for (int c = 0; c < 3; ++c) {
     d.E[c] = reinterpret_cast<float*>(w + L.E[c]);
     d.H[c] = reinterpret_cast<float*>(w + L.H[c]);
@@ -1190,6 +1242,8 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
       d.psiH[c][t] = reinterpret_cast<float*>(w + L.psiH[c][t]);
     }
   }
+  s->pz[0][0] = d.psiH[0][1]; s->pz[0][1] = d.psiH[1][0];
+  for (int t = 0; t < 2; ++t) s->pz[1][t] = s->can_fuse ? reinterpret_cast<float*>(w + L.pHz2[t]) : nullptr;
   size_t base = 0;
   for (int a = 0; a < 3; ++a) {
     for (int t = 0; t < 6; ++t) d.tab[a][t] = reinterpret_cast<float*>(w + L.tab) + base + (size_t)t * s->n[a];

@@ -42,7 +42,15 @@ struct FieldIO {
   const float* E[3];
   const float* H[3];
   float* out[3];
+  // psi_H of the z axis ([0]: the H_x term psiH[0][1], [1]: the H_y term psiH[1][0]): read from / written to.  The same arrays
+  // except beside the whole-row marching kernel (k_fused_fz), whose halo workers need the old values while the owners write
+  const float* pHz_in[2];
+  float* pHz_out[2];
 };
+__device__ __host__ __forceinline__ void io_psi_inplace(FieldIO& io, const Dev& d) {
+  io.pHz_in[0] = io.pHz_out[0] = d.psiH[0][1];
+  io.pHz_in[1] = io.pHz_out[1] = d.psiH[1][0];
+}
 
 // A lean kernel's region (plain Yee cells) and the list of boxes that make up its complement (slab cells and the
 // layers that touch them).  Each box has a class that says which CPML axes can occur in it (so the others compile

@@ -152,6 +152,208 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __gri
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// k_fused_fz — forward marching kernel over WHOLE rows: the plain cells of the lean x-y range and the z-slab cells at both ends of
+// their rows, with the z terms of the CPML (psi_E, psi_H of the z axis), the z = 0 wall and the ghost above z = nz - 1 done in
+// the edge lanes.  Why: beside k_fused_he the z-slab cells of those rows were slab-kernel boxes of 17 to 20 cells at each end of
+// a 2 KB row (C4) — 1.5 GB of DRAM traffic per step for 0.83 GB of arrays, at 4.4 TB/s.  Here they ride on their rows.
+//  * Every lane owns a group of 4 cells (no halo lane): a row of nz = 512 cells is exactly 4 tiles of 32 groups.  The new H just
+//    below a tile, which the E update of the tile's first cell needs, is one cell: lane 0 recomputes H_x, H_y there from the old
+//    fields with a handful of scalar loads (the host makes sure that cell is not a slab cell).
+//  * Halo rows (warp 0) and the priming plane recompute the new H of cells that other blocks own, z-slab cells included, from the
+//    OLD psi_H: psi_H of the z axis is therefore ping-ponged like E and H (pHz_in / pHz_out); psi_E is only ever touched by the
+//    owner of its cell and stays in place.
+//  * Arithmetic and its order are those of gen_h_body / gen_e_body for a class-Z box (R3): plain update, then the z term;
+//    masked nodes (E_x, E_y at z = 0) become 0 and keep their psi.  Bit-identical to the two-kernel path (tests).
+// ---------------------------------------------------------------------------------------------------------
+constexpr int FUSED_ZSL = 8;    // slab groups per row the staging area holds: 2 * pml_width / 4 <= 8 (static shared memory <= 48 KB)
+__device__ __forceinline__ void fused_cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+struct FusedZArgs {
+  const float* Ein[3];
+  const float* Hin[3];
+  float* Eout[3];
+  float* Hout[3];
+  const float* pHz_in[2];   // old psi_H of the z axis: [0] the H_x term (psiH[0][1]), [1] the H_y term (psiH[1][0])
+  float* pHz_out[2];
+  float* pEz[2];            // psi_E of the z axis, in place: [0] the E_x term (psiE[0][1]), [1] the E_y term (psiE[1][0])
+  int lo[2], hi[2];         // x and y range on which both half-steps are applied and stored; z is the whole row
+  int xseg;
+};
+
+struct FusedZSmem {
+  float4 H[2][FUSED_TR + 1][3][32];    // new H_x, H_y, H_z of the plane, double-buffered over the march
+  float4 E[2][FUSED_TR + 1][3][32];    // E_x, E_y, E_z of the NEXT plane
+  float4 P[2][4][FUSED_TR + 1][FUSED_ZSL];   // psi of the z axis, staged a plane ahead: psiHx, psiHy, psiEx, psiEy
+  float C[6][FUSED_ZSL * 4];           // CPML coefficients of the z axis for the slab cells: bH cH kH bE cE kE
+};
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __grid_constant__ Dev d, const __grid_constant__ FusedZArgs a) {
+  // Shared memory doubles as the register file's overflow: whatever a thread carries from one plane to the next (E of the next
+  // plane, its new H of the plane below) lives in the thread's OWN slots of the arrays through which the neighbouring rows read
+  // it anyway, and is read back where it is needed.  With those 24 values in registers the kernel spilled 34 words per plane and
+  // thread (72 registers at 3 blocks of 288 threads per SM).
+  extern __shared__ __align__(16) unsigned char fz_smem_raw[];
+  FusedZSmem& sm = *reinterpret_cast<FusedZSmem*>(fz_smem_raw);
+  const int lane = threadIdx.x, w = threadIdx.y;
+  const int ny = d.n[1], nz = d.n[2], P = d.P;
+  const int g = (int)blockIdx.x * 32 + lane, ngroups = nz / 4;
+  const bool own_grp = g < ngroups;
+  const int k0 = min(g, ngroups - 1) * 4;
+  const int jraw = a.lo[1] + (int)blockIdx.y * FUSED_TR + w - 1;
+  const int xs = a.lo[0] + (int)blockIdx.z * a.xseg, xe = min(xs + a.xseg, a.hi[0]);
+  const int j = min(jraw, a.hi[1] - 1);
+  const bool own = w >= 1 && jraw < a.hi[1] && own_grp;
+  const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];
+  const bool zs = P > 0 && in_slab(k0, nz, P);          // P % 4 == 0: a group lies in a z slab as a whole or not at all
+  const bool wall = k0 == 0, top = k0 + 4 >= nz;
+  const bool edge = lane == 0 && blockIdx.x > 0 && own_grp;   // the cell below this group belongs to the neighbouring tile
+  const bool zp_load = (lane == 31 || g + 1 >= ngroups) && !top;   // no lane above holds the next group
+  const idx_t sx = d.sx, sy = d.sy;
+  const float mS = -d.S;
+  idx_t q = ((idx_t)(xs - 1) * ny + j) * nz + k0;
+  const int szl = zs ? slab_s(k0, nz, P) : 0;           // position of the group inside the compact psi rows of the z axis
+  const int sl = szl / 4;                               // rank of the slab lane among the 2P/4 slab groups of a row (< FUSED_ZSL)
+  if (zs && w == 0) {
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      sm.C[0][sl * 4 + v] = __ldg(d.tab[2][3] + k0 + v); sm.C[1][sl * 4 + v] = __ldg(d.tab[2][4] + k0 + v); sm.C[2][sl * 4 + v] = __ldg(d.tab[2][5] + k0 + v);
+      sm.C[3][sl * 4 + v] = __ldg(d.tab[2][0] + k0 + v); sm.C[4][sl * 4 + v] = __ldg(d.tab[2][1] + k0 + v); sm.C[5][sl * 4 + v] = __ldg(d.tab[2][2] + k0 + v);
+    }
+  }
+  // psi of the z axis for the slab lanes, requested one plane ahead with cp.async: no registers held while the lines travel
+  auto stage_psi = [&](int plane, int st) {
+    if (zs) {
+      const idx_t qp = ((idx_t)plane * ny + j) * (2 * P) + szl;
+      fused_cp_async16(&sm.P[st][0][w][sl], a.pHz_in[0] + qp);
+      fused_cp_async16(&sm.P[st][1][w][sl], a.pHz_in[1] + qp);
+      fused_cp_async16(&sm.P[st][2][w][sl], a.pEz[0] + qp);
+      fused_cp_async16(&sm.P[st][3][w][sl], a.pEz[1] + qp);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  auto put = [](float4& dst, const VF<4>& x) { dst = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]); };
+  auto get = [](const float4& t) { VF<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r; };
+  stage_psi(xs - 1, (xs - 1) & 1);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    put(sm.E[0][w][c][lane], ldv<4>(a.Ein[c] + q));
+    sm.H[1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  __syncthreads();                                      // sm.C
+  int buf = 0;
+  for (int i = xs - 1; i < xe; ++i, q += sx, buf ^= 1) {
+    const idx_t qz = ((idx_t)i * ny + j) * (2 * P) + szl;
+    stage_psi(min(i + 1, xe - 1), (i + 1) & 1);        // (the last step re-requests its own plane into the idle stage: harmless)
+    // ---- loads: E of the next plane, H of this plane; E of this plane from the thread's own slots ----
+    const VF<4> exn = ldv<4>(a.Ein[0] + q + sx), eyn = ldv<4>(a.Ein[1] + q + sx), ezn = ldv<4>(a.Ein[2] + q + sx);
+    VF<4> hx = ldv<4>(a.Hin[0] + q), hy = ldv<4>(a.Hin[1] + q), hz = ldv<4>(a.Hin[2] + q);
+    const VF<4> ex = get(sm.E[buf][w][0][lane]), ey = get(sm.E[buf][w][1][lane]), ez = get(sm.E[buf][w][2][lane]);
+    VF<4> ex_yp, ez_yp;
+    if (yp_smem && i >= xs) {
+      ex_yp = get(sm.E[buf][w + 1][0][lane]);
+      ez_yp = get(sm.E[buf][w + 1][2][lane]);
+    } else {
+      ex_yp = ldv<4>(a.Ein[0] + q + sy);
+      ez_yp = ldv<4>(a.Ein[2] + q + sy);
+    }
+    float ex_zp = __shfl_down_sync(0xffffffffu, ex.v[0], 1), ey_zp = __shfl_down_sync(0xffffffffu, ey.v[0], 1);
+    if (zp_load) { ex_zp = a.Ein[0][q + 4]; ey_zp = a.Ein[1][q + 4]; }
+    if (top) { ex_zp = 0.0f; ey_zp = 0.0f; }          // ghost E[nz] = 0
+    // edge lanes: the new H_x, H_y of the cell below the group (a plain cell), in the arithmetic of the plain H update, from a
+    // handful of scalar loads out of lines the neighbouring tile streams anyway
+    float hx_e = 0.0f, hy_e = 0.0f;
+    if (edge) {
+      const float exm = a.Ein[0][q - 1], eym = a.Ein[1][q - 1], ezm = a.Ein[2][q - 1];
+      hx_e = fmaf(mS, (a.Ein[2][q - 1 + sy] - ezm) - (ey.v[0] - eym), a.Hin[0][q - 1]);
+      hy_e = fmaf(mS, (ex.v[0] - exm) - (a.Ein[2][q - 1 + sx] - ezm), a.Hin[1][q - 1]);
+    }
+    const bool store_plane = own && i >= xs;
+    VF<4> ce;
+    if (store_plane) ce = ldv<4>(d.ce + q);            // requested here, consumed after the barrier
+
+    // ---- H half-step (gen_h_body, class Z): plain update, then the z term of H_x (a2, sign -) and of H_y (a1, sign +) ----
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      const float ey_zq = v == 3 ? ey_zp : ey.v[v < 3 ? v + 1 : v];
+      const float ex_zq = v == 3 ? ex_zp : ex.v[v < 3 ? v + 1 : v];
+      hx.v[v] = fmaf(mS, (ez_yp.v[v] - ez.v[v]) - (ey_zq - ey.v[v]), hx.v[v]);
+      hy.v[v] = fmaf(mS, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
+      hz.v[v] = fmaf(mS, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
+    }
+    asm volatile("cp.async.wait_group 1;" ::: "memory");   // the psi groups of THIS plane have landed (requested a step ago)
+    if (zs) {
+      VF<4> pa = get(sm.P[i & 1][0][w][sl]), pb = get(sm.P[i & 1][1][w][sl]);
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float ey_zq = v == 3 ? ey_zp : ey.v[v < 3 ? v + 1 : v];
+        const float ex_zq = v == 3 ? ex_zp : ex.v[v < 3 ? v + 1 : v];
+        const float dz_ey = ey_zq - ey.v[v], dz_ex = ex_zq - ex.v[v];
+        const float bz = sm.C[0][sl * 4 + v], cz = sm.C[1][sl * 4 + v], kz = sm.C[2][sl * 4 + v];
+        const float px = fmaf(bz, pa.v[v], cz * dz_ey);
+        pa.v[v] = px;
+        hx.v[v] = fmaf(-1.0f * mS, fmaf(kz, dz_ey, px), hx.v[v]);
+        const float py = fmaf(bz, pb.v[v], cz * dz_ex);
+        pb.v[v] = py;
+        hy.v[v] = fmaf(1.0f * mS, fmaf(kz, dz_ex, py), hy.v[v]);
+      }
+      if (store_plane) { stv<4>(a.pHz_out[0] + qz, pa); stv<4>(a.pHz_out[1] + qz, pb); }
+    }
+    // the new H of the cell below the group: from the lane below, or recomputed by an edge lane
+    float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
+    if (edge) { hx_z0 = hx_e; hy_z0 = hy_e; }
+    if (wall) { hx_z0 = 0.0f; hy_z0 = 0.0f; }          // H[-1] ghost (only reaches the masked E_x, E_y at z = 0)
+    put(sm.H[buf][w][0][lane], hx); put(sm.H[buf][w][1][lane], hy); put(sm.H[buf][w][2][lane], hz);
+    put(sm.E[buf ^ 1][w][0][lane], exn); put(sm.E[buf ^ 1][w][1][lane], eyn); put(sm.E[buf ^ 1][w][2][lane], ezn);
+    __syncthreads();
+    if (store_plane) {
+      stv<4>(a.Hout[0] + q, hx); stv<4>(a.Hout[1] + q, hy); stv<4>(a.Hout[2] + q, hz);
+      // ---- E half-step (gen_e_body, class Z): plain update, then the z term of E_x (a2, sign -) and of E_y (a1, sign +).  E_x, E_y
+      //      are finished and stored before E_z is computed ----
+      VF<4> eo, e1;
+      {
+        const VF<4> hz_ym = get(sm.H[buf][w - 1][2][lane]), hz_xm = get(sm.H[buf ^ 1][w][2][lane]);
+        const VF<4> ex2 = get(sm.E[buf][w][0][lane]), ey2 = get(sm.E[buf][w][1][lane]);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+          const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+          eo.v[v] = fmaf(ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex2.v[v]);
+          e1.v[v] = fmaf(ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey2.v[v]);
+        }
+      }
+      if (zs) {
+        VF<4> pa = get(sm.P[i & 1][2][w][sl]), pb = get(sm.P[i & 1][3][w][sl]);
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          if (k0 + v == 0) continue;                    // PEC-masked nodes keep their psi
+          const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+          const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+          const float dz_hy = hy.v[v] - hy_zm, dz_hx = hx.v[v] - hx_zm;
+          const float bz = sm.C[3][sl * 4 + v], cz = sm.C[4][sl * 4 + v], kz = sm.C[5][sl * 4 + v];
+          const float px = fmaf(bz, pa.v[v], cz * dz_hy);
+          pa.v[v] = px;
+          eo.v[v] = fmaf(-1.0f * ce.v[v], fmaf(kz, dz_hy, px), eo.v[v]);
+          const float py = fmaf(bz, pb.v[v], cz * dz_hx);
+          pb.v[v] = py;
+          e1.v[v] = fmaf(1.0f * ce.v[v], fmaf(kz, dz_hx, py), e1.v[v]);
+        }
+        stv<4>(a.pEz[0] + qz, pa); stv<4>(a.pEz[1] + qz, pb);
+      }
+      if (wall) { eo.v[0] = 0.0f; e1.v[0] = 0.0f; }     // PEC-masked nodes: E_x = E_y = 0 at z = 0
+      stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1);
+      {
+        const VF<4> hx_ym = get(sm.H[buf][w - 1][0][lane]), hy_xm = get(sm.H[buf ^ 1][w][1][lane]);
+        const VF<4> ez2 = get(sm.E[buf][w][2][lane]);
+        VF<4> e2;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) e2.v[v] = fmaf(ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez2.v[v]);
+        stv<4>(a.Eout[2] + q, e2);
+      }
+    }
+  }
+}
+
 // Source cells of the reverse variant.  The canonical order (R9) subtracts the source of step m from E^m BEFORE the
 // inverse-E update, while the marching kernel's inverse-H update needs the untouched E^m; so the marching kernel ignores
 // the sources and this small kernel redoes the inverse-E update of the (few) source cells of the inner interior afterwards,

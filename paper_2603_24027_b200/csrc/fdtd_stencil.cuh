@@ -241,8 +241,8 @@ __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int 
   }
   if (zs) {
     qz = psi_index(d, 2, i, j, k0);
-    p_hx_z = ldv<V>(d.psiH[0][1] + qz);
-    p_hy_z = ldv<V>(d.psiH[1][0] + qz);
+    p_hx_z = ldv<V>(io.pHz_in[0] + qz);
+    p_hy_z = ldv<V>(io.pHz_in[1] + qz);
 #pragma unroll
     for (int v = 0; v < V; ++v) {
       bz[v] = __ldg(d.tab[2][3] + k0 + v); cz[v] = __ldg(d.tab[2][4] + k0 + v); kz[v] = __ldg(d.tab[2][5] + k0 + v);
@@ -290,8 +290,8 @@ __device__ __forceinline__ void gen_h_body(const Dev& d, const int i, const int 
     stv<V>(d.psiH[2][1] + qy, p_hz_y);
   }
   if (zs) {
-    stv<V>(d.psiH[0][1] + qz, p_hx_z);
-    stv<V>(d.psiH[1][0] + qz, p_hy_z);
+    stv<V>(io.pHz_out[0] + qz, p_hx_z);
+    stv<V>(io.pHz_out[1] + qz, p_hy_z);
   }
 }
 
@@ -1075,6 +1075,7 @@ __global__ void __launch_bounds__(32 * TY, FDTD_ROW_MINB(WHICH)) k_row(const __g
     FieldIO io;
 #pragma unroll
     for (int c = 0; c < 3; ++c) { io.E[c] = d.E[c]; io.H[c] = d.H[c]; io.out[c] = WHICH == 0 ? d.E[c] : d.H[c]; }
+    io_psi_inplace(io, d);
     if (WHICH == 0) gen_e_body<4, false, false>(d, i, j, k0, io);
     else gen_h_body<4, false, false>(d, i, j, k0, io);
   } else if (WHICH == 2) {

@@ -652,11 +652,14 @@ def test_zface_injection_in_the_inverse_kernels_matches_k_inject(monkeypatch, wh
         w = _inner_design(w)
     o = oracle_gradient(w, 32, dtype, k, interp, store_mode=store_mode)
     res = {}
+    fdtd = _fdtd()
     for zf in ("0", "1"):
         monkeypatch.setenv("FDTD_ZF", zf)
         s = gpu_sim(w, store_mode=store_mode)
+        s.set_workspace(w.nsteps, dtype, k, fdtd.WS_REVERSE | fdtd.WS_GUARD)   # guard bands + NaN fill (own memory check)
         res[zf] = gpu_gradient(w, dtype, k, interp, sim=s)
         res[zf]["adj"] = s.adjoint().cpu().numpy()
+        assert s.guard_check() == 0
     monkeypatch.delenv("FDTD_ZF")
     f_err, g_err = _report(f"z-face injection {which} dtype={dtype} k={k} mode={store_mode}", res["1"], o)
     assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
