@@ -152,12 +152,12 @@ fdtd_status fdtd_set_eps(fdtd_sim*, const float* eps_dev);
 fdtd_status fdtd_reset(fdtd_sim*);
 /* Replay runs of k steps through CUDA graphs (default 1 = on). */
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
-/* Fused marching kernels (two dependent half-steps per pass over the interior): mode -1 (default) =
- * forward run fused on large grids (>= 12 tiles per SM, e.g. 512^3), reverse primal never; 0 = never; 1 = forward AND
- * reverse primal whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per
- * block (0 keeps the current value).  Results are bit-identical in every mode (sources that overlap on one cell excepted
- * in the fused reverse run: they are summed before being subtracted).  With the fused reverse run the fields left after
- * fdtd_reverse are state 0 on the interior only. */
+/* Fused marching kernels (two dependent half-steps per pass over the rows of the lean x-y range): mode -1
+ * (default) = forward run fused where the marching kernel fills most of a wave of tiles (256x256x128 and larger), reverse primal
+ * never; 0 = never; 1 = forward AND reverse primal whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).
+ * xseg = planes marched per block (0 = chosen by the library: 32 on grids with four waves of tiles, else 16).  Results are
+ * bit-identical in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being
+ * subtracted).  With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
 /* Row kernels: the plain cells and the z-slab cells of the same rows in one launch, so that whole rows
  * are streamed.  mode -1 (default) = on grids that stream from HBM (forward working set > 1.5 x L2), 0 = never, 1 = whenever

@@ -96,6 +96,7 @@ struct fdtd_sim {
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 0;            // planes per block of the fused marching kernels (0: chosen by fused_xseg)
   bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
+  bool use_iz = true;      // fused reverse primal: k_fused_iz instead of k_fused_he<true>
   bool use_fz = true;      // fused forward path: whole-row marching kernel (k_fused_fz) instead of k_fused_he + class-Z slab boxes
   bool use_zf = true;      // vector path: the inverse kernels inject the interior cells of the two z faces (fdtd_stencil.cuh, ZF)
   bool use_rows = true;    // vector path: row kernels (lean cells + the z-slab cells of the same rows in one launch)
@@ -333,7 +334,6 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
       int lo2 = (lo + za - 1) / za * za, hi2 = hi / za * za;
       if (hi2 - lo2 < za) { lo2 = (lo + V - 1) / V * V; hi2 = hi / V * V; }
       lo = lo2; hi = hi2;
-      if (std::getenv("FDTD_DEBUG_FULLROW") && which < 4) { lo = 0; hi = n; }   // TIMING EXPERIMENT ONLY: wrong results
     }
     full.lo[a] = lo; full.hi[a] = hi;
   }
@@ -682,6 +682,20 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   if (!inv) a.lo[2] = (a.lo[2] + 3) / 4 * 4;
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
   a.xseg = fused_xseg(s);
+  if (inv && s->use_iz && s->n[2] - 2 * s->P >= 8) {   // reverse twin in the structure of the whole-row kernel (k_fused_iz)
+    FusedIArgs z;
+    for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
+    for (int ax = 0; ax < 2; ++ax) { z.lo[ax] = a.lo[ax]; z.hi[ax] = a.hi[ax]; }
+    z.zlo = s->P; z.zhi = s->n[2] - s->P;
+    z.xseg = a.xseg;
+    const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
+                  (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
+    static bool attr_set = false;
+    if (!attr_set) { cudaFuncSetAttribute(k_fused_iz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedISmem)); attr_set = true; }
+    k_fused_iz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedISmem), s->cur>>>(s->d, z);
+    ++s->launches;
+    return;
+  }
   if (!inv && s->fuse_z) {   // whole rows, z CPML terms in the edge lanes (k_fused_fz)
     FusedZArgs z;
     for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
@@ -932,9 +946,10 @@ bool use_fused(const fdtd_sim* s, int nsteps) {
 }
 bool use_fused_reverse(const fdtd_sim* s) {
   if (s->fuse_rev_mode == 0) return false;
-  // mode -1 (auto): off.  Measured on B200 (round 1, C4): bit-identical to the two-kernel reverse primal and 2.5 GB fewer
-  // bytes per step, but the step is not faster (3406 vs 3395 us): beside the adjoint kernels the marching kernel runs at
-  // 1.23 ms instead of the 1.03 ms of its forward twin.  Kept as an option (fdtd_set_fused mode 1).
+  // mode -1 (auto): off.  Bit-identical to the two-kernel reverse primal and 2.9 GB fewer bytes per step on C4, but not faster:
+  // round 1 (k_fused_he<true>) 3406 vs 3395 us per step; round 2 (k_fused_iz, 1.20 ms per launch against 0.63 + 0.67 ms for the
+  // two inverse kernels at 6.2-6.3 TB/s) 3148 vs 3094 us per step on C4, 229.9 vs 223.8 on C3.  Kept as an option
+  // (fdtd_set_fused mode 1; FDTD_FUSE_REV=2 gives the marching kernel a phase of its own: the same time).
   return s->fuse_rev_mode >= 1 && s->can_fuse;
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
@@ -1140,6 +1155,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   s->use_zf = nz - 2 * pml_width > 256;
   if (const char* e = std::getenv("FDTD_ZF")) s->use_zf = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_FZ")) s->use_fz = atoi(e) != 0;
+  if (const char* e = std::getenv("FDTD_IZ")) s->use_iz = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;

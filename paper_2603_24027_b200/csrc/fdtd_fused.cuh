@@ -354,6 +354,127 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// k_fused_iz — reverse twin of k_fused_fz: inverse-H + inverse-E of the inner interior in one marching pass, in the structure of
+// the whole-row kernel (every lane owns a group of 4 z cells, shared memory as register overflow, edge lanes for the cell below a
+// tile).  Groups cover z in [P, n - P): the two interface cells of a row are element 0 of its first group and element 3 of its
+// last one, so every group is stored whole — H shell elements are written back as inject H has put them into the output buffer
+// (they are the z neighbours of the first / last inner cell), E shell elements are placeholders that inject E overwrites in the
+// next phase.  The row below the first y tile and the plane below the first x segment are interface cells too: their H comes from
+// the output buffer.  Sources are ignored here and redone by k_inv_e_sources, as with k_fused_he<true>.
+// ---------------------------------------------------------------------------------------------------------
+struct FusedIArgs {
+  const float* Ein[3];
+  const float* Hin[3];
+  float* Eout[3];
+  float* Hout[3];
+  int lo[2], hi[2];      // inner-interior x and y range
+  int zlo, zhi;          // z range covered by whole groups: [P, n - P)
+  int xseg;
+};
+struct FusedISmem {
+  float4 H[2][FUSED_TR + 1][3][32];
+  float4 E[2][FUSED_TR + 1][3][32];
+};
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_iz(const __grid_constant__ Dev d, const __grid_constant__ FusedIArgs a) {
+  extern __shared__ __align__(16) unsigned char iz_smem_raw[];
+  FusedISmem& sm = *reinterpret_cast<FusedISmem*>(iz_smem_raw);
+  const int lane = threadIdx.x, w = threadIdx.y;
+  const int ny = d.n[1], nz = d.n[2];
+  const int g = (int)blockIdx.x * 32 + lane;
+  const int k0 = min(max(4 * g, a.zlo), a.zhi - 4);     // clamped for the lanes outside [zlo, zhi): they own nothing
+  const bool own_grp = 4 * g >= a.zlo && 4 * g < a.zhi;
+  const int jraw = a.lo[1] + (int)blockIdx.y * FUSED_TR + w - 1;
+  const int xs = a.lo[0] + (int)blockIdx.z * a.xseg, xe = min(xs + a.xseg, a.hi[0]);
+  const int j = min(jraw, a.hi[1] - 1);
+  const bool own = w >= 1 && jraw < a.hi[1] && own_grp;
+  const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];
+  const bool shell_row = jraw < a.lo[1];                // the interface row below the first y tile
+  const bool zs_lo = own_grp && k0 == a.zlo, zs_hi = own_grp && k0 + 4 == a.zhi;   // group holds an interface cell (element 0 / 3)
+  const bool edge = own_grp && (lane == 0 || 4 * (g - 1) < a.zlo) && !zs_lo;        // no lane below holds the cell below the group
+  const bool zp_load = lane == 31 || !own_grp || zs_hi;                             // no lane above holds the next group
+  const idx_t sx = d.sx, sy = d.sy;
+  const float S = d.S;
+  idx_t q = ((idx_t)(xs - 1) * ny + j) * nz + k0;
+  auto put = [](float4& dst, const VF<4>& x) { dst = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]); };
+  auto get = [](const float4& t) { VF<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r; };
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    put(sm.E[0][w][c][lane], ldv<4>(a.Ein[c] + q));
+    sm.H[1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  }
+  int buf = 0;
+  for (int i = xs - 1; i < xe; ++i, q += sx, buf ^= 1) {
+    const bool shell_plane = i < a.lo[0];               // the interface plane below the first x segment
+    const bool from_out = shell_row || shell_plane;     // this worker's H is an interface value: taken from the output buffer
+    const VF<4> exn = ldv<4>(a.Ein[0] + q + sx), eyn = ldv<4>(a.Ein[1] + q + sx), ezn = ldv<4>(a.Ein[2] + q + sx);
+    VF<4> hx, hy, hz;
+    if (from_out) { hx = ldv<4>(a.Hout[0] + q); hy = ldv<4>(a.Hout[1] + q); hz = ldv<4>(a.Hout[2] + q); }
+    else { hx = ldv<4>(a.Hin[0] + q); hy = ldv<4>(a.Hin[1] + q); hz = ldv<4>(a.Hin[2] + q); }
+    // interface cells at the row ends: H^{m-1/2} as inject H has written it (requested here, used after the H update)
+    float sh[3] = {0.0f, 0.0f, 0.0f}, sh3[3] = {0.0f, 0.0f, 0.0f};
+    if (zs_lo && !from_out) { sh[0] = a.Hout[0][q]; sh[1] = a.Hout[1][q]; sh[2] = a.Hout[2][q]; }
+    if (zs_hi && !from_out) { sh3[0] = a.Hout[0][q + 3]; sh3[1] = a.Hout[1][q + 3]; sh3[2] = a.Hout[2][q + 3]; }
+    const VF<4> ex = get(sm.E[buf][w][0][lane]), ey = get(sm.E[buf][w][1][lane]), ez = get(sm.E[buf][w][2][lane]);
+    VF<4> ex_yp, ez_yp;
+    if (yp_smem && i >= xs) {
+      ex_yp = get(sm.E[buf][w + 1][0][lane]);
+      ez_yp = get(sm.E[buf][w + 1][2][lane]);
+    } else {
+      ex_yp = ldv<4>(a.Ein[0] + q + sy);
+      ez_yp = ldv<4>(a.Ein[2] + q + sy);
+    }
+    float ex_zp = __shfl_down_sync(0xffffffffu, ex.v[0], 1), ey_zp = __shfl_down_sync(0xffffffffu, ey.v[0], 1);
+    if (zp_load) { ex_zp = a.Ein[0][q + 4]; ey_zp = a.Ein[1][q + 4]; }   // q + 4 <= n - P: inside the row
+    float hx_e = 0.0f, hy_e = 0.0f;
+    if (edge) {   // new H_x, H_y of the inner cell below the group, in the arithmetic of the inverse-H update
+      const float exm = a.Ein[0][q - 1], eym = a.Ein[1][q - 1], ezm = a.Ein[2][q - 1];
+      hx_e = fmaf(S, (a.Ein[2][q - 1 + sy] - ezm) - (ey.v[0] - eym), a.Hin[0][q - 1]);
+      hy_e = fmaf(S, (ex.v[0] - exm) - (a.Ein[2][q - 1 + sx] - ezm), a.Hin[1][q - 1]);
+    }
+    const bool store_plane = own && i >= xs;
+    VF<4> ce;
+    if (store_plane) ce = ldv<4>(d.ce + q);
+    // ---- inverse of the H half-step ----
+    if (!from_out) {
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float ey_zq = v == 3 ? ey_zp : ey.v[v < 3 ? v + 1 : v];
+        const float ex_zq = v == 3 ? ex_zp : ex.v[v < 3 ? v + 1 : v];
+        hx.v[v] = fmaf(S, (ez_yp.v[v] - ez.v[v]) - (ey_zq - ey.v[v]), hx.v[v]);
+        hy.v[v] = fmaf(S, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
+        hz.v[v] = fmaf(S, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
+      }
+      if (zs_lo) { hx.v[0] = sh[0]; hy.v[0] = sh[1]; hz.v[0] = sh[2]; }
+      if (zs_hi) { hx.v[3] = sh3[0]; hy.v[3] = sh3[1]; hz.v[3] = sh3[2]; }
+    }
+    float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
+    if (edge) { hx_z0 = hx_e; hy_z0 = hy_e; }
+    put(sm.H[buf][w][0][lane], hx); put(sm.H[buf][w][1][lane], hy); put(sm.H[buf][w][2][lane], hz);
+    put(sm.E[buf ^ 1][w][0][lane], exn); put(sm.E[buf ^ 1][w][1][lane], eyn); put(sm.E[buf ^ 1][w][2][lane], ezn);
+    __syncthreads();
+    if (store_plane) {
+      stv<4>(a.Hout[0] + q, hx); stv<4>(a.Hout[1] + q, hy); stv<4>(a.Hout[2] + q, hz);
+      // ---- inverse of the E half-step; the interface elements keep E^m as a placeholder (inject E overwrites them) ----
+      const VF<4> hx_ym = get(sm.H[buf][w - 1][0][lane]), hz_ym = get(sm.H[buf][w - 1][2][lane]);
+      const VF<4> hy_xm = get(sm.H[buf ^ 1][w][1][lane]), hz_xm = get(sm.H[buf ^ 1][w][2][lane]);
+      const VF<4> ex2 = get(sm.E[buf][w][0][lane]), ey2 = get(sm.E[buf][w][1][lane]), ez2 = get(sm.E[buf][w][2][lane]);
+      VF<4> eo, e1, e2;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+        const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+        eo.v[v] = fmaf(-ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex2.v[v]);
+        e1.v[v] = fmaf(-ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey2.v[v]);
+        e2.v[v] = fmaf(-ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez2.v[v]);
+      }
+      if (zs_lo) { eo.v[0] = ex2.v[0]; e1.v[0] = ey2.v[0]; e2.v[0] = ez2.v[0]; }
+      if (zs_hi) { eo.v[3] = ex2.v[3]; e1.v[3] = ey2.v[3]; e2.v[3] = ez2.v[3]; }
+      stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1); stv<4>(a.Eout[2] + q, e2);
+    }
+  }
+}
+
 // Source cells of the reverse variant.  The canonical order (R9) subtracts the source of step m from E^m BEFORE the
 // inverse-E update, while the marching kernel's inverse-H update needs the untouched E^m; so the marching kernel ignores
 // the sources and this small kernel redoes the inverse-E update of the (few) source cells of the inner interior afterwards,
