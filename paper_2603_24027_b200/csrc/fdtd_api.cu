@@ -690,8 +690,6 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     z.xseg = a.xseg;
     const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
                   (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
-    static bool attr_set = false;
-    if (!attr_set) { cudaFuncSetAttribute(k_fused_iz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedISmem)); attr_set = true; }
     k_fused_iz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedISmem), s->cur>>>(s->d, z);
     ++s->launches;
     return;
@@ -705,8 +703,6 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     z.xseg = a.xseg;
     const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
                   (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
-    static bool attr_set = false;   // more than 48 KB of shared memory per block: opt in once
-    if (!attr_set) { cudaFuncSetAttribute(k_fused_fz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedZSmem)); attr_set = true; }
     k_fused_fz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedZSmem), s->cur>>>(s->d, z);
     ++s->launches;
     return;
@@ -1246,6 +1242,10 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     bool ok = s->can_fuse && s->use_fz && 2 * s->P <= 4 * FUSED_ZSL;   // the staging area of the slab lanes
     for (int kb = 128; ok && kb < s->n[2]; kb += 128) ok = kb - 1 >= s->P && kb - 1 < s->n[2] - s->P;
     s->fuse_z = ok;
+    if (s->can_fuse) {   // the whole-row marching kernels use more than 48 KB of shared memory per block: opt in (not during a capture)
+      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_fz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedZSmem)));
+      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_iz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedISmem)));
+    }
   }
   for (int c = 0; c < 3; ++c) {
     d.E[c] = reinterpret_cast<float*>(w + L.E[c]);

@@ -123,7 +123,11 @@ def _stream_ptr(torch):
 
 
 class Sim:
-    """fdtd_sim handle.  eps: float32 CUDA tensor [nx,ny,nz] (kept alive by this object)."""
+    """fdtd_sim handle.  eps: float32 CUDA tensor [nx,ny,nz] (kept alive by this object).
+
+    Stream rule: the library is bound to the CUDA stream that is current when the object is created, and the tensors this
+    binding allocates per call (monitor record, gradient, source amplitudes) are ordered against that stream only.  forward,
+    reverse, fields, slot ... therefore raise FDTD_ERR_STATE when called under another torch.cuda.stream(...)."""
 
     def __init__(self, eps, dx, dt, pml_width, design=None, monitor=None, cpml=None, store_mode=STORE_ALL, rows=-1):
         torch = _torch()
@@ -134,6 +138,7 @@ class Sim:
         self.shape = tuple(eps.shape)
         self.pml = int(pml_width)
         self._h = C.c_void_p()
+        self._stream = torch.cuda.current_stream().cuda_stream
         st = self._L.fdtd_create(C.byref(self._h), *self.shape, float(dx), float(dt), int(pml_width), C.c_void_p(eps.data_ptr()),
                                  _stream_ptr(torch))
         if st != 0:
@@ -173,6 +178,11 @@ class Sim:
     def _check(self, st):
         if st != 0:
             raise FdtdError(st, self._L.fdtd_last_error(self._h).decode())
+
+    def _same_stream(self):
+        if self._torch.cuda.current_stream().cuda_stream != self._stream:
+            raise FdtdError(4, "called under another CUDA stream than the one the Sim was created on: tensors allocated by this "
+                               "call would not be ordered against the library's stream")
 
     # ---- workspace ----
     def workspace_bytes(self, nsteps, dtype, k, flags=WS_REVERSE):
@@ -231,6 +241,7 @@ class Sim:
     def forward(self, nsteps, sources, store_dtype=F32, k=1, flags=WS_REVERSE, reset=True):
         """fdtd_forward from state 0 (reset=True) or from the current state.  Returns the monitor record tensor
         [nsteps][ncomp][box] (or None)."""
+        self._same_stream()
         torch = self._torch
         self._ensure_ws(nsteps, store_dtype, k, flags)
         if reset:
@@ -247,6 +258,7 @@ class Sim:
     def reverse(self, dL_dfinal=None, dL_dmon=None, interp=LINEAR):
         """fdtd_reverse.  dL_dfinal = (lo, hi, comp_mask, tensor[ncomp][box]) or None; dL_dmon = tensor like the
         monitor record or None.  Returns grad_eps over the design box (float32 CUDA tensor) or None."""
+        self._same_stream()
         torch = self._torch
         cot = None
         if dL_dfinal is not None:
@@ -302,6 +314,7 @@ class Sim:
         return bool(self._L.fdtd_uses_fused(self._h, int(nsteps)))
 
     def fields(self):
+        self._same_stream()
         out = self._torch.empty((6,) + self.shape, dtype=self._torch.float32, device=self.eps.device)
         self._check(self._L.fdtd_get_fields(self._h, C.c_void_p(out.data_ptr())))
         return out
@@ -330,6 +343,7 @@ class Sim:
         """(raw bytes uint8 CUDA tensor copy, 36 float32 scales) of stored slot j.  F8E4M3_MX32: the bytes are the slot_values
         codes followed by the block-scale bytes."""
         torch = self._torch
+        self._same_stream()
         dp, sp = C.c_void_p(), C.c_void_p()
         self._check(self._L.fdtd_slot_ptr(self._h, int(j), C.byref(dp), C.byref(sp)))
         nbytes = self.slot_bytes(dtype)

@@ -786,6 +786,25 @@ def test_host_buffer_path_matches_device_path():
 # ---------------------------------------------------------------------------------------------------------
 # error behaviour and memory claims
 # ---------------------------------------------------------------------------------------------------------
+def test_calls_under_another_stream_are_refused():
+    """The binding allocates per-call tensors on torch's current stream; the library runs on the stream current at creation.
+    A call under another stream is refused (FDTD_ERR_STATE) instead of racing with the caching allocator."""
+    import torch
+    fdtd = _fdtd()
+    w = W.tiny(nsteps=6)
+    s = gpu_sim(w)
+    s.forward(w.nsteps, w.sources, W.F32, 1)
+    other = torch.cuda.Stream()
+    with torch.cuda.stream(other):
+        with pytest.raises(fdtd.FdtdError) as e:
+            s.forward(w.nsteps, w.sources, W.F32, 1)
+        assert e.value.status == 4
+        with pytest.raises(fdtd.FdtdError):
+            s.fields()
+    s.forward(w.nsteps, w.sources, W.F32, 1)      # fine again on the bound stream
+    assert torch.isfinite(s.fields()).all().item()
+
+
 def test_error_codes():
     import torch
     fdtd = _fdtd()
