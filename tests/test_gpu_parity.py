@@ -349,6 +349,23 @@ def test_fused_marching_path_matches_two_kernel_path(dtype, k, xseg, graphs):
             assert np.array_equal(sa.cpu().numpy(), sb.cpu().numpy()), j
 
 
+def test_fused_path_falls_back_where_the_whole_row_kernel_does_not_apply():
+    """pml_width = 20: more slab groups per row than the whole-row marching kernel stages (2P/4 > 8), so the fused forward path
+    is k_fused_he beside class-Z slab boxes, and the fused reverse primal k_fused_iz.  Bit-identical to the two-kernel path and
+    within tolerance of the oracle."""
+    w = mid_workload(shape=(64, 56, 136), P=20, nsteps=36, dtype=W.BF16, k=4)
+    o = oracle_gradient(w, 32, W.BF16, 4)
+    res = {}
+    for mode in (0, 1):
+        s = gpu_sim(w)
+        s.set_fused(mode, 7)
+        res[mode] = gpu_gradient(w, W.BF16, 4, sim=s)
+    f_err, g_err = _report("fused fall-back P=20", res[1], o)
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    for key in ("final", "mon", "grad"):
+        assert np.array_equal(res[0][key], res[1][key]), key
+
+
 def _inner_design(w):
     P = w.pml
     return dataclasses.replace(w, design=(tuple([P + 1] * 3), tuple(n - P - 1 for n in w.shape)))
