@@ -397,7 +397,10 @@ bool grid_inner(const fdtd_sim* s, dim3* g) {
 void set_cur(fdtd_sim* s, int b) {
   s->cb = b;
   for (int c = 0; c < 3; ++c) { s->d.E[c] = s->fb[b][c]; s->d.H[c] = s->fb[b][3 + c]; }
-  if (s->pz[b][0]) { s->d.psiH[0][1] = s->pz[b][0]; s->d.psiH[1][0] = s->pz[b][1]; }   // ping-ponged with the fields
+  // psi_H of the z axis is ping-ponged with the fields only where the whole-row marching kernel runs (fuse_z); everywhere else the
+  // slab kernels update it in place, in buffer 0's arrays
+  const int pb = s->fuse_z ? b : 0;
+  if (s->pz[pb][0]) { s->d.psiH[0][1] = s->pz[pb][0]; s->d.psiH[1][0] = s->pz[pb][1]; }
 }
 
 #define LAUNCH(s, kern, grid, block, ...)            \
