@@ -207,6 +207,27 @@ fdtd_status fdtd_codec_encode(fdtd_dtype dtype, const float* x_dev, size_t n, vo
 fdtd_status fdtd_codec_fetch(fdtd_dtype dtype, fdtd_interp interp, const void* const codes_dev[4],
                              const float scales[4], int num, int den, size_t n, float* out_dev, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Allocation-free variant of the slice encoder, for callers that cannot allocate device memory around the call (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Encodes a batch of nslices equally long slices,
+ * x_dev[nslices][slice_len] (float32), exactly as fdtd_codec_encode does slice by slice (R12-R14):
+ * codes_dev[nslices][slice_len * sizeof(dtype)], scales_dev[nslices] (1 unless FDTD_F8E4M3_SCALED).  The absmax reduction words
+ * that fdtd_codec_encode takes from the caller (scratch_dev) live in a file-scope `static __device__` array of the library
+ * instead: FDTD_NOALLOC_MAX_SLICES words = 16 KiB, held by every GPU that loads the library until the process exits.  The call
+ * performs no cudaMalloc / cudaFree and calls no allocating library routine; the caller still owns inputs and outputs.
+ *  - nslices > FDTD_NOALLOC_MAX_SLICES, nslices < 1, slice_len < 1 or FDTD_F8E4M3_MX32 (its slot layout carries scale bytes
+ *    behind the codes: use fdtd_codec_encode) -> FDTD_ERR_INVALID_ARG / FDTD_ERR_UNSUPPORTED, message in
+ *    fdtd_noalloc_last_error().
+ *  - The array is shared by ALL calls on a device and keeps the last call's contents: each call clears the words it uses, on
+ *    its stream, before reducing into them.  Calls that overlap on the GPU (different streams, or two host threads) race on it:
+ *    serialise them (one stream, or an event between them).
+ *  - Enqueues on cuda_stream and does not synchronise. */
+#define FDTD_NOALLOC_MAX_SLICES 4096
+fdtd_status fdtd_codec_encode_slices_noalloc(fdtd_dtype dtype, const float* x_dev, int nslices, size_t slice_len, void* codes_dev,
+                                             float* scales_dev, void* cuda_stream);
+/* Message of the last failed fdtd_codec_encode_slices_noalloc call of this host thread ("" if none). */
+const char* fdtd_noalloc_last_error(void);
+
 fdtd_status fdtd_sync(fdtd_sim*);
 const char* fdtd_last_error(const fdtd_sim*);
 void fdtd_destroy(fdtd_sim*);

@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1497,6 +1498,100 @@ fdtd_status fdtd_codec_fetch(fdtd_dtype dt, fdtd_interp interp, const void* cons
   const unsigned g = (unsigned)std::min<size_t>(std::max<size_t>((n + 255) / 256, 1), 1184);
   FDTD_DT_SWITCH((int)dt, (k_codec_fetch<DT><<<g, 256, 0, st>>>(a, mode, num, den, n, out_dev)))
   return cudaGetLastError() == cudaSuccess ? FDTD_OK : FDTD_ERR_CUDA;
+}
+
+// ---- allocation-free slice encoder (include/fdtd.h: fdtd_codec_encode_slices_noalloc) ----
+// The absmax words of the per-slice reduction live in this file-scope device array instead of caller memory.  In HOST code the
+// name below is a host-side stand-in, not a device address: its address is looked up once per device with cudaGetSymbolAddress
+// (that device current) and passed to the kernels.  Shared by every call on a device; a call clears the words it uses first.
+}  // extern "C"
+static __device__ __align__(256) unsigned g_noalloc_amax[FDTD_NOALLOC_MAX_SLICES];
+namespace {
+constexpr int kMaxDevices = 64;
+unsigned* g_noalloc_ptr[kMaxDevices] = {nullptr};
+std::mutex g_noalloc_mutex;
+thread_local std::string g_noalloc_err;
+
+fdtd_status noalloc_fail(fdtd_status code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_noalloc_err = buf;
+  return code;
+}
+
+// grid: x = blocks along a slice, y = slice.  Bit pattern of max|x| per slice, warp-reduced, one atomicMax per warp.
+__global__ void __launch_bounds__(256) k_noalloc_amax(const float* __restrict__ x, size_t slice_len, unsigned* __restrict__ amax) {
+  const float* xs = x + (size_t)blockIdx.y * slice_len;
+  unsigned m = 0;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < slice_len; t += (size_t)gridDim.x * blockDim.x)
+    m = max(m, __float_as_uint(fabsf(xs[t])));
+  m = __reduce_max_sync(0xffffffffu, m);
+  if ((threadIdx.x & 31) == 0) atomicMax(&amax[blockIdx.y], m);
+}
+template <int DT>
+__global__ void __launch_bounds__(256) k_noalloc_encode(const float* __restrict__ x, size_t slice_len, void* codes, float* scales,
+                                                        const unsigned* __restrict__ amax) {
+  typedef typename Codec<DT>::code_t code_t;
+  const size_t base = (size_t)blockIdx.y * slice_len;
+  float inv = 1.0f, sc = 1.0f;
+  if (DT == DT_E4M3S) {   // the arithmetic of k_codec_encode (R13)
+    const float a = __uint_as_float(amax[blockIdx.y]);
+    inv = a > 0.0f ? 448.0f / a : 0.0f;
+    sc = a > 0.0f ? a / 448.0f : 0.0f;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) scales[blockIdx.y] = sc;
+  for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < slice_len; t += (size_t)gridDim.x * blockDim.x)
+    reinterpret_cast<code_t*>(codes)[base + t] = Codec<DT>::enc(x[base + t], inv);
+}
+}  // namespace
+extern "C" {
+
+const char* fdtd_noalloc_last_error(void) { return g_noalloc_err.c_str(); }
+
+fdtd_status fdtd_codec_encode_slices_noalloc(fdtd_dtype dt, const float* x_dev, int nslices, size_t slice_len, void* codes_dev,
+                                             float* scales_dev, void* cuda_stream) {
+  g_noalloc_err.clear();
+  if (!x_dev || !codes_dev || !scales_dev) return noalloc_fail(FDTD_ERR_INVALID_ARG, "fdtd_codec_encode_slices_noalloc: NULL pointer");
+  if (!dtype_ok((int)dt)) return noalloc_fail(FDTD_ERR_INVALID_ARG, "fdtd_codec_encode_slices_noalloc: unknown store dtype %d", (int)dt);
+  if ((int)dt == DT_MX32)
+    return noalloc_fail(FDTD_ERR_UNSUPPORTED, "fdtd_codec_encode_slices_noalloc: FDTD_F8E4M3_MX32 keeps its scale bytes behind the codes; use fdtd_codec_encode");
+  if (nslices < 1 || slice_len < 1) return noalloc_fail(FDTD_ERR_INVALID_ARG, "fdtd_codec_encode_slices_noalloc: nslices and slice_len must be >= 1");
+  if (nslices > FDTD_NOALLOC_MAX_SLICES)
+    return noalloc_fail(FDTD_ERR_INVALID_ARG, "fdtd_codec_encode_slices_noalloc: %d slices exceed the static scratch array (FDTD_NOALLOC_MAX_SLICES = %d)",
+                        nslices, FDTD_NOALLOC_MAX_SLICES);
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess || dev < 0 || dev >= kMaxDevices)
+    return noalloc_fail(FDTD_ERR_CUDA, "fdtd_codec_encode_slices_noalloc: cudaGetDevice: %s (device %d)", cudaGetErrorString(e), dev);
+  unsigned* amax = nullptr;
+  {
+    // set-up, once per device, with that device current: the device address of the static array
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+      void* ptr = nullptr;
+      e = cudaGetSymbolAddress(&ptr, g_noalloc_amax);
+      if (e != cudaSuccess || !ptr)
+        return noalloc_fail(FDTD_ERR_CUDA, "fdtd_codec_encode_slices_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+      g_noalloc_ptr[dev] = static_cast<unsigned*>(ptr);
+    }
+    amax = g_noalloc_ptr[dev];
+  }
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+  const unsigned bx = (unsigned)std::min<size_t>(std::max<size_t>((slice_len + 255) / 256, 1), 64);
+  const dim3 g(bx, (unsigned)nslices);
+  if ((int)dt == DT_E4M3S) {
+    // the array keeps the last call's maxima: the words this call reduces into start at zero
+    e = cudaMemsetAsync(amax, 0, (size_t)nslices * sizeof(unsigned), st);
+    if (e != cudaSuccess) return noalloc_fail(FDTD_ERR_CUDA, "fdtd_codec_encode_slices_noalloc: cudaMemsetAsync: %s", cudaGetErrorString(e));
+    k_noalloc_amax<<<g, 256, 0, st>>>(x_dev, slice_len, amax);
+  }
+  FDTD_DT_SWITCH((int)dt, (k_noalloc_encode<DT><<<g, 256, 0, st>>>(x_dev, slice_len, codes_dev, scales_dev, amax)))
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return noalloc_fail(FDTD_ERR_CUDA, "fdtd_codec_encode_slices_noalloc: launch: %s", cudaGetErrorString(e));
+  return FDTD_OK;
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {

@@ -17,6 +17,7 @@ F8E4M3B11FNUZ, F8E5M2FNUZ, F8E4M3FNUZ, F8E4M3, F8E3M4 = 10, 11, 12, 13, 14
 LINEAR, CUBIC = 0, 1
 STORE_ALL, STORE_TANGENTIAL = 0, 1
 WS_REVERSE, WS_HOST_IO = 1, 2
+NOALLOC_MAX_SLICES = 4096   # FDTD_NOALLOC_MAX_SLICES (include/fdtd.h)
 WS_GUARD = 4   # debugging aid (include/fdtd_bench.h): guard bands + 0xFF fill
 STATUS = {0: "FDTD_OK", 1: "FDTD_ERR_INVALID_ARG", 2: "FDTD_ERR_OOM", 3: "FDTD_ERR_CUDA", 4: "FDTD_ERR_STATE",
           5: "FDTD_ERR_UNSUPPORTED"}
@@ -86,6 +87,9 @@ def lib():
     L.fdtd_reverse_host.argtypes = [vp, vp, C.c_int, vp]
     L.fdtd_codec_encode.argtypes = [C.c_int, vp, C.c_size_t, vp, vp, vp, vp]
     L.fdtd_codec_fetch.argtypes = [C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_float), C.c_int, C.c_int, C.c_size_t, vp, vp]
+    L.fdtd_codec_encode_slices_noalloc.argtypes = [C.c_int, vp, C.c_int, C.c_size_t, vp, vp, vp]
+    L.fdtd_noalloc_last_error.restype = C.c_char_p
+    L.fdtd_noalloc_last_error.argtypes = []
     L.fdtd_profile_kernel.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.fdtd_sync.argtypes = [vp]
     L.fdtd_last_error.restype = C.c_char_p
@@ -103,7 +107,7 @@ EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
             "fdtd_set_graphs", "fdtd_set_fused", "fdtd_set_rows", "fdtd_uses_fused", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_slot_bytes", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
-            "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
+            "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_codec_encode_slices_noalloc", "fdtd_noalloc_last_error", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count", "fdtd_debug_guard_check"]
 
 
@@ -407,3 +411,22 @@ def codec_fetch(dtype, interp, codes, scales, num, den, n=None):
     if st != 0:
         raise FdtdError(st, "fdtd_codec_fetch")
     return out
+
+
+def codec_encode_slices_noalloc(dtype, x, codes=None, scales=None):
+    """fdtd_codec_encode_slices_noalloc: x float32 CUDA tensor [nslices, slice_len]; codes (uint8 [nslices, slice_len * bytes]) and
+    scales (float32 [nslices]) are the caller's output tensors (allocated here only when not given).  The library call itself
+    allocates nothing: its reduction scratch is a static device array (at most NOALLOC_MAX_SLICES slices per call)."""
+    torch = _torch()
+    L = lib()
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.dim() == 2
+    nslices, slice_len = x.shape
+    if codes is None:
+        codes = torch.empty((nslices, slice_len * ELEM_BYTES[dtype]), dtype=torch.uint8, device=x.device)
+    if scales is None:
+        scales = torch.empty(nslices, dtype=torch.float32, device=x.device)
+    st = L.fdtd_codec_encode_slices_noalloc(int(dtype), C.c_void_p(x.data_ptr()), int(nslices), int(slice_len),
+                                            C.c_void_p(codes.data_ptr()), C.c_void_p(scales.data_ptr()), _stream_ptr(torch))
+    if st != 0:
+        raise FdtdError(st, L.fdtd_noalloc_last_error().decode())
+    return codes, scales
