@@ -1698,6 +1698,12 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
         double c = 1;
         for (int a = 0; a < 3; ++a) c *= std::max(0, s->n[a] - 2 * s->P - 1);
         v = 52 * c;
+        if (s->fuse_z) {
+          // whole-row kernel (k_fused_fz): the rows of the lean x-y range over their full length, plus, on their z-slab cells,
+          // psi_H of the z axis read and written (two arrays, ping-ponged) and psi_E read and written (two arrays): 32 B per cell
+          const double rows = (double)std::max(0, s->n[0] - 2 * s->P - 1) * std::max(0, s->n[1] - 2 * s->P - 1);
+          v = 52 * rows * s->n[2] + 32 * rows * 2 * s->P;
+        }
         break;
       }
       case 11: case 12: case 13: case 14: case 15: case 16: case 17: case 18: {
