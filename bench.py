@@ -99,7 +99,7 @@ GROUP_KERNELS = {
     "record": ["k_record"],
     "inject_h": ["k_inject"],
     "inject_e": ["k_inject"],
-    "fwd_fused": ["k_fused_he"],
+    "fwd_fused": ["k_fused_fz", "k_fused_he"],
     "fwd_fused_slabs": ["k_gen_h", "k_gen_e"],
 }
 
