@@ -167,3 +167,43 @@ def test_cpml_reflection_bound():
     peak = np.abs(ref).max()
     assert np.abs(got - ref).max() / peak < 1e-2
     assert np.abs(bare - ref).max() / peak > 0.5
+
+
+def test_cpml_profile_staggering_and_mirror_symmetry():
+    """The CPML constants are a reading (R5: the paper prints none), but WHERE the profile is sampled is fixed by the
+    Yee staggering: E-type terms sit at integer positions i, H-type terms at half-integer positions i + 1/2, and the absorber
+    starts at the interface planes x = P and x = N - P.  With kappa = 1 the tables give back the graded conductivity,
+    sigma + alpha = -ln b, so:
+      (1) against the physical depth (P - x or x - (N - P)) the E samples (integer depths) and the H samples (half-integer
+          depths) interleave on ONE strictly increasing curve sigma(depth) — a half-cell mix-up of the two tables breaks the
+          interleaving;
+      (2) the layout is mirror-symmetric about the middle of the grid: E(i) = E(N - i), H(i) = H(N - 1 - i);
+      (3) the interior (shell included) is plain Yee: b-terms irrelevant, c = 0, 1/kappa - 1 = 0."""
+    N, P = 40, 10
+    s = orc.OracleSim(64, np.ones((N, N, N)), P, W.S)
+    sf, kmax, amax, m = orc.CPML_DEFAULTS
+    assert kmax == 1.0
+    for axis in range(3):
+        bE, cE, kE, bH, cH, kH = s.tables(axis)
+        # (3)
+        assert np.all(cE[P:N - P + 1] == 0) and np.all(kE == 0) and np.all(kH == 0)
+        assert np.all(cH[P:N - P] == 0)
+        assert np.all(cE[:P] != 0) and np.all(cE[N - P + 1:] != 0) and np.all(cH[:P] != 0) and np.all(cH[N - P:] != 0)
+        # (2)
+        i = np.arange(1, N)
+        assert np.allclose(bE[i], bE[N - i], rtol=0, atol=1e-15) and np.allclose(cE[i], cE[N - i], rtol=0, atol=1e-15)
+        i = np.arange(0, N)
+        assert np.allclose(bH[i], bH[N - 1 - i], rtol=0, atol=1e-15) and np.allclose(cH[i], cH[N - 1 - i], rtol=0, atol=1e-15)
+        # (1) low slab: depth of E node i is P - i (i = 0 .. P-1), of H node i is P - i - 1/2
+        depth = np.concatenate([P - np.arange(P), P - np.arange(P) - 0.5])
+        loss = np.concatenate([-np.log(bE[:P]), -np.log(bH[:P])])          # sigma + alpha at that depth
+        alpha = amax * (1.0 - depth / P)
+        sigma = loss - alpha
+        order = np.argsort(depth)
+        d_sorted, s_sorted = depth[order], sigma[order]
+        assert np.all(np.diff(d_sorted) == 0.5)                               # 0.5, 1.0, 1.5, ... P: E and H alternate
+        assert np.all(np.diff(s_sorted) > 0)
+        # one power law through all 2P samples: sigma = sigma_max * (depth / P)^m with a single sigma_max
+        smax = s_sorted / (d_sorted / P) ** m
+        assert np.allclose(smax, smax[-1], rtol=1e-10)
+        assert abs(smax[-1] - sf * (m + 1) * W.S) <= 1e-7 * smax[-1]            # W.S is rounded to f32 inside the oracle
