@@ -99,7 +99,9 @@ GROUP_KERNELS = {
     "record": ["k_record"],
     "inject_h": ["k_inject"],
     "inject_e": ["k_inject"],
-    "fwd_fused": ["k_fused_fz", "k_fused_he"],
+    "fwd_fused": ["k_fused_fp", "k_fused_he"],
+    "rev_fused": ["k_fused_ip", "k_fused_he"],
+    "grad": ["k_grad("],
     "fwd_fused_slabs": ["k_gen_h", "k_gen_e"],
 }
 
@@ -144,13 +146,13 @@ def ncu_import(args):
     tscale = {"ns": 1e-3, "us": 1.0, "ms": 1e3, "s": 1e6}[units[ci["gpu__time_duration.sum"]]]
     launches = [(r[ci["Kernel Name"]], by(r, "dram__bytes_read.sum"), by(r, "dram__bytes_write.sum"),
                  float(r[ci["gpu__time_duration.sum"]]) * tscale) for r in rows[2:] if "fdtd::" in r[ci["Kernel Name"]]]
-    from paper_2603_24027_b200 import fdtd
     groups, detail, pos = {}, {}, 0
-    for name in fdtd.Sim.KERNELS:
+    present = " ".join(l[0] for l in launches)
+    for name in active_groups(None, "k_fused_fp" in present or "k_fused_he" in present, "k_fused_ip" in present):
         pref = GROUP_KERNELS[name]
         got = []
         while pos < len(launches) and any(launches[pos][0].replace("void ", "").replace("fdtd::", "").startswith(p) for p in pref) \
-                and len(got) < (2 if name not in ("inv_h", "inject_h", "inject_e", "fwd_fused") else 1):
+                and len(got) < (2 if name not in ("inv_h", "inject_h", "inject_e", "fwd_fused", "rev_fused", "grad") else 1):
             got.append(launches[pos])
             pos += 1
         if not got:
@@ -214,15 +216,24 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def profile_kernels(sim, fdtd, w, flags, flush, reps, fused):
+def active_groups(fdtd, fused, fused_rev):
+    """Names of the kernel groups that the run launches (fdtd.Sim.KERNEL_IDS), in profiling order.  fwd_e / fwd_h stay in the list
+    on the fused forward path too (its first and last half-step, and the two-kernel-equivalent figure)."""
+    names = ["fwd_e", "fwd_h"]
+    names += ["rev_fused", "grad"] if fused_rev else ["inv_h", "grad_inv_e"]
+    names += ["adj_h", "adj_e", "record", "inject_h", "inject_e"]
+    if fused:
+        names += ["fwd_fused", "fwd_fused_slabs"]
+    return names
+
+
+def profile_kernels(sim, fdtd, w, flags, flush, reps, fused, fused_rev):
     """Each kernel group timed alone on the library's stream (fdtd_profile_kernel): {name: {us, algo_bytes}}.  Needs a completed
-    forward run of at least 4*k steps (record / inject read the store)."""
+    forward run (record / inject and the z-face injection of the inverse kernels read the store)."""
     out = {}
-    for kid, name in enumerate(fdtd.Sim.KERNELS):
-        if kid >= 9 and not fused:
-            continue
+    for name in active_groups(fdtd, fused, fused_rev):
         flush.fill_(1)
-        ms, by = sim.profile_kernel(kid, warm=3 if reps > 1 else 0, reps=reps)
+        ms, by = sim.profile_kernel(fdtd.Sim.KERNEL_IDS[name], warm=3 if reps > 1 else 0, reps=reps)
         out[name] = {"us": ms * 1e3, "algo_bytes": by}
     return out
 
@@ -253,10 +264,10 @@ def run_gpu(args, rank, world):
         import dataclasses
         w = dataclasses.replace(w, nsteps=min(w.nsteps, 64))
         sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
-        fused = sim.uses_fused(w.nsteps)
+        fused, fused_rev = sim.uses_fused(w.nsteps), sim.uses_fused_reverse()
         torch.cuda.synchronize()
         torch.cuda.profiler.start()
-        k = profile_kernels(sim, fdtd, w, flags, flush, 1, fused)
+        k = profile_kernels(sim, fdtd, w, flags, flush, 1, fused, fused_rev)
         torch.cuda.profiler.stop()
         print(json.dumps({"profile_only": True, "workload": args.workload, "kernels": k, "kernel_source_hash": kernel_source_hash()}))
         return
@@ -368,11 +379,12 @@ def run_gpu(args, rank, world):
     # ---- per-kernel roofline (rank 0): each kernel group timed alone, back to back, CUDA events on its stream ----
     peak, peak_src = load_peaks()
     sim.forward(min(w.nsteps, 64), w.sources, w.store_dtype, w.k, flags=flags)
-    fused = sim.uses_fused(w.nsteps)   # large grids: H half-step of step m and E half-step of step m+1 in one marching kernel
+    fused = sim.uses_fused(w.nsteps)   # H half-step of step m and E half-step of step m+1 in one marching kernel
+    fused_rev = sim.uses_fused_reverse()   # large grids: inverse-H and inverse-E of the reverse primal in one marching kernel
     counts = {"fwd_e": 1 if fused else w.nsteps, "fwd_h": 1 if fused else w.nsteps, "inv_h": w.nsteps, "adj_h": w.nsteps,
               "grad_inv_e": w.nsteps, "adj_e": w.nsteps, "record": nrec + 1, "inject_h": w.nsteps, "inject_e": w.nsteps,
-              "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1}
-    kernels = profile_kernels(sim, fdtd, w, flags, flush, 20, fused)
+              "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1, "rev_fused": w.nsteps, "grad": w.nsteps}
+    kernels = profile_kernels(sim, fdtd, w, flags, flush, 20, fused, fused_rev)
     traffic, traffic_src = load_ncu_traffic(args.workload if not (args.store or args.k or args.tangential) else "-")
     tot = sum(v["us"] * counts[n] for n, v in kernels.items())
     for n, v in kernels.items():
@@ -405,7 +417,8 @@ def run_gpu(args, rank, world):
     # whole-pass effective bandwidth: algorithmic bytes of all stencil launches of one step / measured time
     fwd_names = ("fwd_e", "fwd_h", "fwd_fused", "fwd_fused_slabs")
     algo_fwd = sum(kernels[n]["algo_bytes"] * counts[n] for n in fwd_names if n in kernels) + kernels["record"]["algo_bytes"] * (nrec + 1)
-    algo_rev = sum(kernels[n]["algo_bytes"] for n in ("inv_h", "adj_h", "grad_inv_e", "adj_e", "inject_h", "inject_e")) * w.nsteps
+    rev_names = ("rev_fused", "grad", "inv_h", "grad_inv_e", "adj_h", "adj_e", "inject_h", "inject_e")
+    algo_rev = sum(kernels[n]["algo_bytes"] for n in rev_names if n in kernels) * w.nsteps
     fwd_gbs = algo_fwd / (f_ms / args.steps * 1e-3) / 1e9
     # the same forward time against the bytes of the two-kernel form (76 B per cell): comparable across paths
     algo_fwd2 = (kernels["fwd_e"]["algo_bytes"] + kernels["fwd_h"]["algo_bytes"]) * w.nsteps + kernels["record"]["algo_bytes"] * (nrec + 1)
@@ -440,7 +453,7 @@ def run_gpu(args, rank, world):
         "store_bytes": store_bytes, "store_bytes_per_step": store_bytes / w.nsteps,
         "store_bytes_f32_k1": (w.nsteps + 1) * slot_vals * (3 if args.tangential else 1) * 4,   # all six components
         "effective_gbs": {"forward": fwd_gbs, "reverse": rev_gbs, "forward_frac_of_peak": fwd_gbs / peak,
-                          "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused),
+                          "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused), "reverse_fused": bool(fused_rev),
                           "forward_two_kernel_equivalent": fwd2_gbs, "forward_two_kernel_equivalent_frac": fwd2_gbs / peak,
                           # also against the nominal HBM3e figure (8000 GB/s)
                           "forward_frac_of_nominal_8000": fwd_gbs / 8000.0, "reverse_frac_of_nominal_8000": rev_gbs / 8000.0,

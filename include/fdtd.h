@@ -154,10 +154,10 @@ fdtd_status fdtd_reset(fdtd_sim*);
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
 /* Fused marching kernels (two dependent half-steps per pass over the rows of the lean x-y range): mode -1
  * (default) = forward run fused where the marching kernel fills most of a wave of tiles (256x256x128 and larger), reverse primal
- * never; 0 = never; 1 = forward AND reverse primal whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).
- * xseg = planes marched per block (0 = chosen by the library: 32 on grids with four waves of tiles, else 16).  Results are
- * bit-identical in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being
- * subtracted).  With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */
+ * fused where it has several waves (512^3); 0 = never; 1 = forward AND reverse primal whenever the grid allows (nz % 4 == 0,
+ * pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per block (0 = chosen by the library).  Results are bit-identical
+ * in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being subtracted).
+ * With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
 /* Row kernels: the plain cells and the z-slab cells of the same rows in one launch, so that whole rows
  * are streamed.  mode -1 (default) = on grids that stream from HBM (forward working set > 1.5 x L2), 0 = never, 1 = whenever
@@ -165,6 +165,8 @@ fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);
 fdtd_status fdtd_set_rows(fdtd_sim*, int mode);
 /* 1 if fdtd_forward(nsteps) would take the fused path with the current settings (after fdtd_set_workspace), else 0. */
 int fdtd_uses_fused(const fdtd_sim*, int nsteps);
+/* 1 if fdtd_reverse would rebuild the primal with the fused marching kernel (inverse-H + inverse-E in one pass), else 0. */
+int fdtd_uses_fused_reverse(const fdtd_sim*);
 
 /* Current fields: out_dev[6][nx][ny][nz].  fdtd_get_box: out_dev[ncomp][hi-lo] for the components in comp_mask. */
 fdtd_status fdtd_get_fields(fdtd_sim*, float* out_dev);

@@ -91,14 +91,14 @@ struct fdtd_sim {
   float* fb[2][6] = {{nullptr}};
   int cb = 0;
   float* pz[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // psi_H of the z axis per buffer: [b][0] H_x term, [b][1] H_y term
-  bool fuse_z = false;     // the fused forward path uses the whole-row marching kernel (k_fused_fz): no class-Z slab boxes
+  bool fuse_z = false;     // the fused forward path uses the whole-row marching kernel (k_fused_fp): no class-Z slab boxes
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 0;            // planes per block of the fused marching kernels (0: chosen by fused_xseg)
   bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
-  bool use_iz = true;      // fused reverse primal: k_fused_iz instead of k_fused_he<true>
-  bool use_fz = true;      // fused forward path: whole-row marching kernel (k_fused_fz) instead of k_fused_he + class-Z slab boxes
+  bool use_iz = true;      // fused reverse primal: k_fused_ip instead of k_fused_he<true>
+  bool use_fz = true;      // fused forward path: whole-row marching kernel (k_fused_fp) instead of k_fused_he + class-Z slab boxes
   bool use_zf = true;      // vector path: the inverse kernels inject the interior cells of the two z faces (fdtd_stencil.cuh, ZF)
   bool use_rows = true;    // vector path: row kernels (lean cells + the z-slab cells of the same rows in one launch)
   int zalign = 0;          // z alignment (cells) of the lean regions, chosen at create: 32 (128-byte lines) on grids that stream
@@ -198,7 +198,7 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   if (s->V == 4 && s->P >= 4) {   // ping-pong partners of E and H for the fused marching kernels
     for (int c = 0; c < 3; ++c) L.E2[c] = take(N * 4);
     for (int c = 0; c < 3; ++c) L.H2[c] = take(N * 4);
-    for (int t = 0; t < 2; ++t) L.pHz2[t] = take((size_t)psi_elems(s, 2) * 4);   // partners of psi_H of the z axis (k_fused_fz)
+    for (int t = 0; t < 2; ++t) L.pHz2[t] = take((size_t)psi_elems(s, 2) * 4);   // partners of psi_H of the z axis (k_fused_fp)
   }
   for (int c = 0; c < 3; ++c)
     for (int t = 0; t < 2; ++t) L.psiE[c][t] = take((size_t)psi_elems(s, (c + 1 + t) % 3) * 4);
@@ -666,11 +666,12 @@ long long fused_tiles(const fdtd_sim* s, int xseg) {
   tiles *= (s->n[0] - 2 * s->P + xseg - 1) / xseg;
   return tiles;
 }
-// planes a block of the marching kernels walks: 32 where that still leaves four waves of tiles (3 blocks per SM), else 16.
-// Measured on B200 (round 2, whole-row kernel): C4 forward per 400 steps at 8 / 16 / 24 / 32 / 64 planes 605.9 / 592.7 / 586.5 /
-// 586.5 / 585.8 ms; C3 per 2000 steps at 4 / 8 / 12 / 16 planes 242.7 / 232.8 / 245.9 / 223.5 ms.
+// planes a block of the marching kernels walks.  Whole-row kernel (two blocks per SM): 32 where that leaves at least one tile per
+// SM, else 16.  Measured on B200 (round 2, k_fused_fp): C4 forward per 400 steps at 32 / 40 / 48 planes 548.4 / 548.5 / 551.0 ms;
+// C3 per 2000 steps at 16 / 20 / 24 / 28 / 32 planes 223.2 / 225.7 / 217.2 / 208.5 / 208.6 ms (196 tiles at 32).
 int fused_xseg(const fdtd_sim* s) {
   if (s->xseg > 0) return s->xseg;
+  if (s->fuse_z) return fused_tiles(s, 32) >= 148 ? 32 : 16;
   return fused_tiles(s, 32) >= 4 * 3 * 148 ? 32 : 16;
 }
 void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
@@ -686,7 +687,7 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   if (!inv) a.lo[2] = (a.lo[2] + 3) / 4 * 4;
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
   a.xseg = fused_xseg(s);
-  if (inv && s->use_iz && s->n[2] - 2 * s->P >= 8) {   // reverse twin in the structure of the whole-row kernel (k_fused_iz)
+  if (inv && s->use_iz && s->n[2] - 2 * s->P >= 8) {   // reverse twin in the structure of the whole-row kernel (k_fused_ip)
     FusedIArgs z;
     for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
     for (int ax = 0; ax < 2; ++ax) { z.lo[ax] = a.lo[ax]; z.hi[ax] = a.hi[ax]; }
@@ -694,11 +695,11 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     z.xseg = a.xseg;
     const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
                   (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
-    k_fused_iz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedISmem), s->cur>>>(s->d, z);
+    k_fused_ip<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedQSmem), s->cur>>>(s->d, z);
     ++s->launches;
     return;
   }
-  if (!inv && s->fuse_z) {   // whole rows, z CPML terms in the edge lanes (k_fused_fz)
+  if (!inv && s->fuse_z) {   // whole rows, z CPML terms in the edge lanes (k_fused_fp)
     FusedZArgs z;
     for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
     for (int t = 0; t < 2; ++t) { z.pHz_in[t] = s->pz[from][t]; z.pHz_out[t] = s->pz[to][t]; }
@@ -707,7 +708,7 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
     z.xseg = a.xseg;
     const dim3 gz((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((z.hi[1] - z.lo[1] + FUSED_TR - 1) / FUSED_TR),
                   (unsigned)((z.hi[0] - z.lo[0] + z.xseg - 1) / z.xseg));
-    k_fused_fz<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedZSmem), s->cur>>>(s->d, z);
+    k_fused_fp<<<gz, dim3(32, FUSED_TR + 1), sizeof(FusedPSmem), s->cur>>>(s->d, z);
     ++s->launches;
     return;
   }
@@ -939,18 +940,20 @@ bool use_fused(const fdtd_sim* s, int nsteps) {
   if (s->fuse_mode == 1) return true;
   // mode -1 (auto): where the marching kernel fills most of one wave of tiles (3 blocks per SM = 444 slots).  Round 1 (k_fused_he
   // beside class-Z slab boxes) paid only with several waves: C4 (7200 tiles) forward 1910 -> 1727 us per step, C3 (392 tiles)
-  // 159 -> 161, C2 35 -> 44.  With the whole-row kernel (k_fused_fz, round 2): C4 1631 -> 1466 us per step against the split
+  // 159 -> 161, C2 35 -> 44.  With the whole-row kernel (k_fused_fp, round 2): C4 1631 -> 1466 us per step against the split
   // path with row kernels, C3 (392 tiles) 129.8 -> 111.8; C2 (91 tiles) 29.1 -> 67.3: stays split.
   if (!s->fuse_z) return fused_tiles(s, fused_xseg(s)) >= 4 * 3 * 148;
   return fused_tiles(s, 16) >= 2 * 148;
 }
 bool use_fused_reverse(const fdtd_sim* s) {
-  if (s->fuse_rev_mode == 0) return false;
-  // mode -1 (auto): off.  Bit-identical to the two-kernel reverse primal and 2.9 GB fewer bytes per step on C4, but not faster:
-  // round 1 (k_fused_he<true>) 3406 vs 3395 us per step; round 2 (k_fused_iz, 1.20 ms per launch against 0.63 + 0.67 ms for the
-  // two inverse kernels at 6.2-6.3 TB/s) 3148 vs 3094 us per step on C4, 229.9 vs 223.8 on C3.  Kept as an option
-  // (fdtd_set_fused mode 1; FDTD_FUSE_REV=2 gives the marching kernel a phase of its own: the same time).
-  return s->fuse_rev_mode >= 1 && s->can_fuse;
+  if (s->fuse_rev_mode == 0 || !s->can_fuse) return false;
+  if (s->fuse_rev_mode >= 1) return true;
+  // mode -1 (auto): where the whole-row structure applies and the marching kernel has several waves of tiles (two blocks per SM).
+  // Bit-identical to the two-kernel reverse primal; 3.1 GB fewer bytes per step on C4.  Measured on B200: round 1 (k_fused_he<true>,
+  // 1.23 ms per launch) 3406 vs 3395 us per step on C4: off; round 2 with direct loads (1.20 ms) 3148 vs 3094: off; round 2 with
+  // the cp.async-pipelined kernel (k_fused_ip, 0.98 ms against 0.63 + 0.67 ms for the two inverse kernels): C4 2924 vs 3090 us per
+  // step: on; C3 (196 tiles) 234.8 vs 223.7: off.
+  return s->use_iz && s->n[2] - 2 * s->P >= 8 && fused_tiles(s, 32) >= 4 * 2 * 148;
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
@@ -1247,8 +1250,8 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     for (int kb = 128; ok && kb < s->n[2]; kb += 128) ok = kb - 1 >= s->P && kb - 1 < s->n[2] - s->P;
     s->fuse_z = ok;
     if (s->can_fuse) {   // the whole-row marching kernels use more than 48 KB of shared memory per block: opt in (not during a capture)
-      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_fz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedZSmem)));
-      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_iz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedISmem)));
+      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedPSmem)));
+      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_ip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedQSmem)));
     }
   }
   for (int c = 0; c < 3; ++c) {
@@ -1362,6 +1365,7 @@ fdtd_status fdtd_set_rows(fdtd_sim* s, int mode) {
   return FDTD_OK;
 }
 
+int fdtd_uses_fused_reverse(const fdtd_sim* s) { return (s && s->ws && use_fused_reverse(s)) ? 1 : 0; }
 int fdtd_uses_fused(const fdtd_sim* s, int nsteps) { return (s && s->ws && use_fused(s, nsteps)) ? 1 : 0; }
 
 fdtd_status fdtd_forward(fdtd_sim* s, int nsteps, const fdtd_source* src, int nsrc, fdtd_dtype dt, int k) {
@@ -1595,7 +1599,7 @@ fdtd_status fdtd_codec_encode_slices_noalloc(fdtd_dtype dt, const float* x_dev, 
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
-  if (!s || id < 0 || id > 19 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s || id < 0 || id > 20 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
   if (((id >= 6 && id <= 8) || id == 2 || id == 4) && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
@@ -1630,8 +1634,11 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       }
       case 5: split_pair(3); break;
       case 6: launch_record(s, s->nsteps, nullptr, 2); break;
-      case 7: launch_inject(s, mrev, nullptr, 1, 0); break;
-      case 8: launch_inject(s, mrev, nullptr, 0, 0); break;
+      case 7: case 8:   // as the active reverse path launches it: in place (4 or 6 faces) or between the two buffers (6 faces)
+        if (use_fused_reverse(s)) launch_inject(s, mrev, nullptr, id == 7 ? 1 : 0, 0, s->cb, s->cb ^ 1);
+        else launch_inject(s, mrev, nullptr, id == 7 ? 1 : 0, 0);
+        break;
+      case 20: launch_grad(s); break;
       case 9: launch_fused(s, false, s->cb, s->cb ^ 1); break;
       case 19: launch_fused(s, true, s->cb, s->cb ^ 1); break;   // reverse marching kernel (inverse-H + inverse-E), alone
       case 11: case 12: case 13: case 14: launch_lean(s, id - 11); break;     // lean kernel of split half-step id - 11, alone
@@ -1677,7 +1684,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
     }
     const double eb = elem_bytes_host(s->dtype);
     // shell cells k_inject handles, and those the inverse kernels inject themselves (interior cells of the two z faces)
-    const double zin = zface_fused(s) ? 2.0 * std::max(0, s->n[0] - 2 * s->P - 2) * std::max(0, s->n[1] - 2 * s->P - 2) : 0.0;
+    const double zin = (zface_fused(s) && !use_fused_reverse(s)) ? 2.0 * std::max(0, s->n[0] - 2 * s->P - 2) * std::max(0, s->n[1] - 2 * s->P - 2) : 0.0;
     const double shell = (double)s->st.cell_off[6] - zin;
     const double zbytes = (s->store_mode == 1 ? 1.0 : 3.0) * zin * (2 * eb + 4);
     double v = 0;
@@ -1690,6 +1697,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 5: v = 40 * N + 16 * slab; break;          // lH rw + lE + ce
       case 6: v = (double)s->st.slot_values * 4 + (double)slot_bytes_host(s, s->dtype); break;   // f32 gathered, slot written (block scales included)
       case 7: case 8: v = (s->store_mode == 1 ? 1.0 : 3.0) * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
+      case 20: v = 40 * dcells; break;   // lE (12) + f64 accumulator rw (16) + H of the design cells (12)
       case 19: {  // reverse marching kernel: 52 B per inner-interior cell
         v = 52 * Ninner;
         break;
@@ -1699,7 +1707,7 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
         for (int a = 0; a < 3; ++a) c *= std::max(0, s->n[a] - 2 * s->P - 1);
         v = 52 * c;
         if (s->fuse_z) {
-          // whole-row kernel (k_fused_fz): the rows of the lean x-y range over their full length, plus, on their z-slab cells,
+          // whole-row kernel (k_fused_fp): the rows of the lean x-y range over their full length, plus, on their z-slab cells,
           // psi_H of the z axis read and written (two arrays, ping-ponged) and psi_E read and written (two arrays): 32 B per cell
           const double rows = (double)std::max(0, s->n[0] - 2 * s->P - 1) * std::max(0, s->n[1] - 2 * s->P - 1);
           v = 52 * rows * s->n[2] + 32 * rows * 2 * s->P;

@@ -153,7 +153,7 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_he(const __gri
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// k_fused_fz — forward marching kernel over WHOLE rows: the plain cells of the lean x-y range and the z-slab cells at both ends of
+// Forward marching kernel over WHOLE rows (k_fused_fp below): the plain cells of the lean x-y range and the z-slab cells at both ends of
 // their rows, with the z terms of the CPML (psi_E, psi_H of the z axis), the z = 0 wall and the ghost above z = nz - 1 done in
 // the edge lanes.  Why: beside k_fused_he the z-slab cells of those rows were slab-kernel boxes of 17 to 20 cells at each end of
 // a 2 KB row (C4) — 1.5 GB of DRAM traffic per step for 0.83 GB of arrays, at 4.4 TB/s.  Here they ride on their rows.
@@ -182,19 +182,34 @@ struct FusedZArgs {
   int xseg;
 };
 
-struct FusedZSmem {
-  float4 H[2][FUSED_TR + 1][3][32];    // new H_x, H_y, H_z of the plane, double-buffered over the march
-  float4 E[2][FUSED_TR + 1][3][32];    // E_x, E_y, E_z of the NEXT plane
-  float4 P[2][4][FUSED_TR + 1][FUSED_ZSL];   // psi of the z axis, staged a plane ahead: psiHx, psiHy, psiEx, psiEy
-  float C[6][FUSED_ZSL * 4];           // CPML coefficients of the z axis for the slab cells: bH cH kH bE cE kE
+// ---------------------------------------------------------------------------------------------------------
+// k_fused_fp — the whole-row forward marching kernel described above, with every global load of the march staged through shared
+// memory by cp.async, one plane ahead (E two planes ahead): the loads of plane i+1 travel while plane i is computed, and they
+// hold no registers while they do.  Its predecessor (k_fused_fz, round 2, removed) issued the loads of a plane at the top of its
+// march step and consumed them a few instructions later, in front of a block-wide barrier; ncu: 5.4 TB/s of DRAM traffic against
+// 7.0 for k_row, long-scoreboard and barrier stalls, 41 % occupancy, and no register left (72 at 3 blocks of 288 threads) to
+// prefetch into — shared memory served as the register file's overflow there.  1186 -> 1009 us per launch on C4 (0.96 of the
+// measured copy bandwidth in algorithmic bytes).
+//  * Stages: E of plane p in stage p % 3 (plane i, i+1 in use, i+2 arriving), old H and psi of plane p in stage p % 2, new H of
+//    plane p in stage p % 2.  Everything a thread or its neighbours read of plane i has landed before the barrier of step i-1.
+//  * The halo accesses ride on the same pipeline: the row above the top warp is an extra row slot filled by the top warp; the
+//    group below a tile (edge lanes) and the group above it (last lane) are extra float4 slots.
+//  * 112 KB of shared memory per block, two blocks per SM (93 registers: nothing spills, E of the plane stays in registers across
+//    the barrier).  ce is prefetched one plane ahead into registers.
+// ---------------------------------------------------------------------------------------------------------
+struct FusedPSmem {
+  float4 E[3][FUSED_TR + 2][3][32];     // row slot w = the warp's row; slot TR + 1 = the row above the top warp's
+  float4 Hin[2][FUSED_TR + 1][3][32];
+  float4 Hn[2][FUSED_TR + 1][3][32];
+  float4 Elo[3][FUSED_TR + 2][3];       // E of the group below the tile's first group (edge lanes)
+  float4 Hlo[2][FUSED_TR + 1][2];       // old H_x, H_y of that group
+  float4 Ehi[3][FUSED_TR + 1][2];       // E_x, E_y of the group above the warp's last group
+  float4 P[2][4][FUSED_TR + 1][FUSED_ZSL];
+  float C[6][FUSED_ZSL * 4];
 };
-__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __grid_constant__ Dev d, const __grid_constant__ FusedZArgs a) {
-  // Shared memory doubles as the register file's overflow: whatever a thread carries from one plane to the next (E of the next
-  // plane, its new H of the plane below) lives in the thread's OWN slots of the arrays through which the neighbouring rows read
-  // it anyway, and is read back where it is needed.  With those 24 values in registers the kernel spilled 34 words per plane and
-  // thread (72 registers at 3 blocks of 288 threads per SM).
-  extern __shared__ __align__(16) unsigned char fz_smem_raw[];
-  FusedZSmem& sm = *reinterpret_cast<FusedZSmem*>(fz_smem_raw);
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 2) k_fused_fp(const __grid_constant__ Dev d, const __grid_constant__ FusedZArgs a) {
+  extern __shared__ __align__(16) unsigned char fp_smem_raw[];
+  FusedPSmem& sm = *reinterpret_cast<FusedPSmem*>(fp_smem_raw);
   const int lane = threadIdx.x, w = threadIdx.y;
   const int ny = d.n[1], nz = d.n[2], P = d.P;
   const int g = (int)blockIdx.x * 32 + lane, ngroups = nz / 4;
@@ -202,18 +217,19 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
   const int k0 = min(g, ngroups - 1) * 4;
   const int jraw = a.lo[1] + (int)blockIdx.y * FUSED_TR + w - 1;
   const int xs = a.lo[0] + (int)blockIdx.z * a.xseg, xe = min(xs + a.xseg, a.hi[0]);
-  const int j = min(jraw, a.hi[1] - 1);
+  // rows beyond the region clamp to the first row above it (inside the grid; they are loaded for their neighbour below, never stored)
+  const int j = min(jraw, a.hi[1]), j2 = min(jraw + 1, a.hi[1]);
   const bool own = w >= 1 && jraw < a.hi[1] && own_grp;
-  const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];
-  const bool zs = P > 0 && in_slab(k0, nz, P);          // P % 4 == 0: a group lies in a z slab as a whole or not at all
+  const bool zs = P > 0 && in_slab(k0, nz, P);
   const bool wall = k0 == 0, top = k0 + 4 >= nz;
-  const bool edge = lane == 0 && blockIdx.x > 0 && own_grp;   // the cell below this group belongs to the neighbouring tile
-  const bool zp_load = (lane == 31 || g + 1 >= ngroups) && !top;   // no lane above holds the next group
-  const idx_t sx = d.sx, sy = d.sy;
+  const bool edge = lane == 0 && blockIdx.x > 0 && own_grp;
+  const bool zp_lane = (lane == 31 || g + 1 >= ngroups) && !top;
+  const bool topw = w == FUSED_TR;
+  const idx_t sx = d.sx;
   const float mS = -d.S;
-  idx_t q = ((idx_t)(xs - 1) * ny + j) * nz + k0;
-  const int szl = zs ? slab_s(k0, nz, P) : 0;           // position of the group inside the compact psi rows of the z axis
-  const int sl = szl / 4;                               // rank of the slab lane among the 2P/4 slab groups of a row (< FUSED_ZSL)
+  const int szl = zs ? slab_s(k0, nz, P) : 0;
+  const int sl = szl / 4;
+  const idx_t rowoff = (idx_t)j * nz + k0, rowoff2 = (idx_t)j2 * nz + k0;
   if (zs && w == 0) {
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
@@ -221,57 +237,78 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
       sm.C[3][sl * 4 + v] = __ldg(d.tab[2][0] + k0 + v); sm.C[4][sl * 4 + v] = __ldg(d.tab[2][1] + k0 + v); sm.C[5][sl * 4 + v] = __ldg(d.tab[2][2] + k0 + v);
     }
   }
-  // psi of the z axis for the slab lanes, requested one plane ahead with cp.async: no registers held while the lines travel
-  auto stage_psi = [&](int plane, int st) {
+  auto issueE = [&](int p) {            // E of plane p
+    const int st = p % 3;
+    const idx_t q = (idx_t)p * sx + rowoff;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.E[st][w][c][lane], a.Ein[c] + q);
+    if (topw) {
+      const idx_t q2 = (idx_t)p * sx + rowoff2;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.E[st][FUSED_TR + 1][c][lane], a.Ein[c] + q2);
+      if (edge) fused_cp_async16(&sm.Elo[st][FUSED_TR + 1][2], a.Ein[2] + q2 - 4);
+    }
+    if (edge) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.Elo[st][w][c], a.Ein[c] + q - 4);
+    }
+    if (zp_lane) {
+      fused_cp_async16(&sm.Ehi[st][w][0], a.Ein[0] + q + 4);
+      fused_cp_async16(&sm.Ehi[st][w][1], a.Ein[1] + q + 4);
+    }
+  };
+  auto issueH = [&](int p) {            // old H and psi of plane p
+    const int st = p & 1;
+    const idx_t q = (idx_t)p * sx + rowoff;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.Hin[st][w][c][lane], a.Hin[c] + q);
+    if (edge) {
+      fused_cp_async16(&sm.Hlo[st][w][0], a.Hin[0] + q - 4);
+      fused_cp_async16(&sm.Hlo[st][w][1], a.Hin[1] + q - 4);
+    }
     if (zs) {
-      const idx_t qp = ((idx_t)plane * ny + j) * (2 * P) + szl;
+      const idx_t qp = ((idx_t)p * ny + j) * (2 * P) + szl;
       fused_cp_async16(&sm.P[st][0][w][sl], a.pHz_in[0] + qp);
       fused_cp_async16(&sm.P[st][1][w][sl], a.pHz_in[1] + qp);
       fused_cp_async16(&sm.P[st][2][w][sl], a.pEz[0] + qp);
       fused_cp_async16(&sm.P[st][3][w][sl], a.pEz[1] + qp);
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
   };
   auto put = [](float4& dst, const VF<4>& x) { dst = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]); };
   auto get = [](const float4& t) { VF<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r; };
-  stage_psi(xs - 1, (xs - 1) & 1);
+  issueE(xs - 1);
+  issueE(xs);
+  issueH(xs - 1);
+  asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    put(sm.E[0][w][c][lane], ldv<4>(a.Ein[c] + q));
-    sm.H[1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-  }
-  __syncthreads();                                      // sm.C
-  int buf = 0;
-  for (int i = xs - 1; i < xe; ++i, q += sx, buf ^= 1) {
+  for (int c = 0; c < 3; ++c) sm.Hn[xs & 1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);   // "new H of plane xs - 2": never used in a stored value
+  VF<4> ce_n = zerov<4>();
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();                                      // the priming planes and sm.C are visible to every warp
+  for (int i = xs - 1; i < xe; ++i) {
+    const idx_t q = (idx_t)i * sx + rowoff;
     const idx_t qz = ((idx_t)i * ny + j) * (2 * P) + szl;
-    stage_psi(min(i + 1, xe - 1), (i + 1) & 1);        // (the last step re-requests its own plane into the idle stage: harmless)
-    // ---- loads: E of the next plane, H of this plane; E of this plane from the thread's own slots ----
-    const VF<4> exn = ldv<4>(a.Ein[0] + q + sx), eyn = ldv<4>(a.Ein[1] + q + sx), ezn = ldv<4>(a.Ein[2] + q + sx);
-    VF<4> hx = ldv<4>(a.Hin[0] + q), hy = ldv<4>(a.Hin[1] + q), hz = ldv<4>(a.Hin[2] + q);
-    const VF<4> ex = get(sm.E[buf][w][0][lane]), ey = get(sm.E[buf][w][1][lane]), ez = get(sm.E[buf][w][2][lane]);
-    VF<4> ex_yp, ez_yp;
-    if (yp_smem && i >= xs) {
-      ex_yp = get(sm.E[buf][w + 1][0][lane]);
-      ez_yp = get(sm.E[buf][w + 1][2][lane]);
-    } else {
-      ex_yp = ldv<4>(a.Ein[0] + q + sy);
-      ez_yp = ldv<4>(a.Ein[2] + q + sy);
-    }
+    if (i + 2 <= xe) issueE(i + 2);
+    if (i + 1 < xe) issueH(i + 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const VF<4> ce = ce_n;
+    if (own && i + 1 < xe) ce_n = ldv<4>(d.ce + q + sx);    // ce of the next plane: a whole march step to arrive
+    asm volatile("cp.async.wait_group 1;" ::: "memory");    // all but the newest group: E(i+1), old H(i), psi(i) have landed
+    const int se = i % 3, sn = (i + 1) % 3, sh = i & 1;
+    const VF<4> ex = get(sm.E[se][w][0][lane]), ey = get(sm.E[se][w][1][lane]), ez = get(sm.E[se][w][2][lane]);
+    const VF<4> eyn = get(sm.E[sn][w][1][lane]), ezn = get(sm.E[sn][w][2][lane]);
+    VF<4> hx = get(sm.Hin[sh][w][0][lane]), hy = get(sm.Hin[sh][w][1][lane]), hz = get(sm.Hin[sh][w][2][lane]);
+    const VF<4> ex_yp = get(sm.E[se][w + 1][0][lane]), ez_yp = get(sm.E[se][w + 1][2][lane]);
     float ex_zp = __shfl_down_sync(0xffffffffu, ex.v[0], 1), ey_zp = __shfl_down_sync(0xffffffffu, ey.v[0], 1);
-    if (zp_load) { ex_zp = a.Ein[0][q + 4]; ey_zp = a.Ein[1][q + 4]; }
+    if (zp_lane) { ex_zp = sm.Ehi[se][w][0].x; ey_zp = sm.Ehi[se][w][1].x; }
     if (top) { ex_zp = 0.0f; ey_zp = 0.0f; }          // ghost E[nz] = 0
-    // edge lanes: the new H_x, H_y of the cell below the group (a plain cell), in the arithmetic of the plain H update, from a
-    // handful of scalar loads out of lines the neighbouring tile streams anyway
     float hx_e = 0.0f, hy_e = 0.0f;
-    if (edge) {
-      const float exm = a.Ein[0][q - 1], eym = a.Ein[1][q - 1], ezm = a.Ein[2][q - 1];
-      hx_e = fmaf(mS, (a.Ein[2][q - 1 + sy] - ezm) - (ey.v[0] - eym), a.Hin[0][q - 1]);
-      hy_e = fmaf(mS, (ex.v[0] - exm) - (a.Ein[2][q - 1 + sx] - ezm), a.Hin[1][q - 1]);
+    if (edge) {   // new H_x, H_y of the (plain) cell below the group, in the arithmetic of the plain H update
+      const float exm = sm.Elo[se][w][0].w, eym = sm.Elo[se][w][1].w, ezm = sm.Elo[se][w][2].w;
+      hx_e = fmaf(mS, (sm.Elo[se][w + 1][2].w - ezm) - (ey.v[0] - eym), sm.Hlo[sh][w][0].w);
+      hy_e = fmaf(mS, (ex.v[0] - exm) - (sm.Elo[sn][w][2].w - ezm), sm.Hlo[sh][w][1].w);
     }
     const bool store_plane = own && i >= xs;
-    VF<4> ce;
-    if (store_plane) ce = ldv<4>(d.ce + q);            // requested here, consumed after the barrier
-
     // ---- H half-step (gen_h_body, class Z): plain update, then the z term of H_x (a2, sign -) and of H_y (a1, sign +) ----
 #pragma unroll
     for (int v = 0; v < 4; ++v) {
@@ -281,9 +318,8 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
       hy.v[v] = fmaf(mS, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
       hz.v[v] = fmaf(mS, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
     }
-    asm volatile("cp.async.wait_group 1;" ::: "memory");   // the psi groups of THIS plane have landed (requested a step ago)
     if (zs) {
-      VF<4> pa = get(sm.P[i & 1][0][w][sl]), pb = get(sm.P[i & 1][1][w][sl]);
+      VF<4> pa = get(sm.P[sh][0][w][sl]), pb = get(sm.P[sh][1][w][sl]);
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         const float ey_zq = v == 3 ? ey_zp : ey.v[v < 3 ? v + 1 : v];
@@ -299,31 +335,27 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
       }
       if (store_plane) { stv<4>(a.pHz_out[0] + qz, pa); stv<4>(a.pHz_out[1] + qz, pb); }
     }
-    // the new H of the cell below the group: from the lane below, or recomputed by an edge lane
     float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
     if (edge) { hx_z0 = hx_e; hy_z0 = hy_e; }
-    if (wall) { hx_z0 = 0.0f; hy_z0 = 0.0f; }          // H[-1] ghost (only reaches the masked E_x, E_y at z = 0)
-    put(sm.H[buf][w][0][lane], hx); put(sm.H[buf][w][1][lane], hy); put(sm.H[buf][w][2][lane], hz);
-    put(sm.E[buf ^ 1][w][0][lane], exn); put(sm.E[buf ^ 1][w][1][lane], eyn); put(sm.E[buf ^ 1][w][2][lane], ezn);
+    if (wall) { hx_z0 = 0.0f; hy_z0 = 0.0f; }
+    put(sm.Hn[sh][w][0][lane], hx); put(sm.Hn[sh][w][1][lane], hy); put(sm.Hn[sh][w][2][lane], hz);
     __syncthreads();
     if (store_plane) {
       stv<4>(a.Hout[0] + q, hx); stv<4>(a.Hout[1] + q, hy); stv<4>(a.Hout[2] + q, hz);
-      // ---- E half-step (gen_e_body, class Z): plain update, then the z term of E_x (a2, sign -) and of E_y (a1, sign +).  E_x, E_y
-      //      are finished and stored before E_z is computed ----
-      VF<4> eo, e1;
-      {
-        const VF<4> hz_ym = get(sm.H[buf][w - 1][2][lane]), hz_xm = get(sm.H[buf ^ 1][w][2][lane]);
-        const VF<4> ex2 = get(sm.E[buf][w][0][lane]), ey2 = get(sm.E[buf][w][1][lane]);
+      // ---- E half-step (gen_e_body, class Z): plain update, then the z term of E_x (a2, sign -) and of E_y (a1, sign +) ----
+      const VF<4> hx_ym = get(sm.Hn[sh][w - 1][0][lane]), hz_ym = get(sm.Hn[sh][w - 1][2][lane]);
+      const VF<4> hy_xm = get(sm.Hn[sh ^ 1][w][1][lane]), hz_xm = get(sm.Hn[sh ^ 1][w][2][lane]);
+      VF<4> eo, e1, e2;
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
-          const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
-          eo.v[v] = fmaf(ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex2.v[v]);
-          e1.v[v] = fmaf(ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey2.v[v]);
-        }
+      for (int v = 0; v < 4; ++v) {
+        const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
+        const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
+        eo.v[v] = fmaf(ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex.v[v]);
+        e1.v[v] = fmaf(ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey.v[v]);
+        e2.v[v] = fmaf(ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez.v[v]);
       }
       if (zs) {
-        VF<4> pa = get(sm.P[i & 1][2][w][sl]), pb = get(sm.P[i & 1][3][w][sl]);
+        VF<4> pa = get(sm.P[sh][2][w][sl]), pb = get(sm.P[sh][3][w][sl]);
 #pragma unroll
         for (int v = 0; v < 4; ++v) {
           if (k0 + v == 0) continue;                    // PEC-masked nodes keep their psi
@@ -341,21 +373,13 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_fz(const __gri
         stv<4>(a.pEz[0] + qz, pa); stv<4>(a.pEz[1] + qz, pb);
       }
       if (wall) { eo.v[0] = 0.0f; e1.v[0] = 0.0f; }     // PEC-masked nodes: E_x = E_y = 0 at z = 0
-      stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1);
-      {
-        const VF<4> hx_ym = get(sm.H[buf][w - 1][0][lane]), hy_xm = get(sm.H[buf ^ 1][w][1][lane]);
-        const VF<4> ez2 = get(sm.E[buf][w][2][lane]);
-        VF<4> e2;
-#pragma unroll
-        for (int v = 0; v < 4; ++v) e2.v[v] = fmaf(ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez2.v[v]);
-        stv<4>(a.Eout[2] + q, e2);
-      }
+      stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1); stv<4>(a.Eout[2] + q, e2);
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// k_fused_iz — reverse twin of k_fused_fz: inverse-H + inverse-E of the inner interior in one marching pass, in the structure of
+// Reverse twin of the whole-row kernel (k_fused_ip below): inverse-H + inverse-E of the inner interior in one marching pass, in the structure of
 // the whole-row kernel (every lane owns a group of 4 z cells, shared memory as register overflow, edge lanes for the cell below a
 // tile).  Groups cover z in [P, n - P): the two interface cells of a row are element 0 of its first group and element 3 of its
 // last one, so every group is stored whole — H shell elements are written back as inject H has put them into the output buffer
@@ -372,69 +396,116 @@ struct FusedIArgs {
   int zlo, zhi;          // z range covered by whole groups: [P, n - P)
   int xseg;
 };
-struct FusedISmem {
-  float4 H[2][FUSED_TR + 1][3][32];
-  float4 E[2][FUSED_TR + 1][3][32];
+// ---------------------------------------------------------------------------------------------------------
+// k_fused_ip — the reverse twin described above, in the pipelined form of k_fused_fp: the loads of the march are staged through
+// shared memory by cp.async, a plane ahead.  The interface H of the row below the first y tile and of the plane below the first x
+// segment (put into the output buffer by inject H, earlier on the same stream) is staged from that buffer into the same slots; the
+// interface elements at the two ends of a row are prefetched a plane ahead into registers.  Its predecessor with direct loads
+// (k_fused_iz, removed) took 1202 us per launch on C4, this one 980 us (5.8 TB/s): the first fused reverse primal that beats the
+// two inverse kernels on 512^3 (reverse run 3090 -> 2924 us per step).
+// ---------------------------------------------------------------------------------------------------------
+struct FusedQSmem {
+  float4 E[3][FUSED_TR + 2][3][32];
+  float4 Hin[2][FUSED_TR + 1][3][32];
+  float4 Hn[2][FUSED_TR + 1][3][32];
+  float4 Elo[3][FUSED_TR + 2][3];
+  float4 Hlo[2][FUSED_TR + 1][2];
+  float4 Ehi[3][FUSED_TR + 1][2];
 };
-__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_iz(const __grid_constant__ Dev d, const __grid_constant__ FusedIArgs a) {
-  extern __shared__ __align__(16) unsigned char iz_smem_raw[];
-  FusedISmem& sm = *reinterpret_cast<FusedISmem*>(iz_smem_raw);
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 2) k_fused_ip(const __grid_constant__ Dev d, const __grid_constant__ FusedIArgs a) {
+  extern __shared__ __align__(16) unsigned char ip_smem_raw[];
+  FusedQSmem& sm = *reinterpret_cast<FusedQSmem*>(ip_smem_raw);
   const int lane = threadIdx.x, w = threadIdx.y;
-  const int ny = d.n[1], nz = d.n[2];
+  const int nz = d.n[2];
   const int g = (int)blockIdx.x * 32 + lane;
-  const int k0 = min(max(4 * g, a.zlo), a.zhi - 4);     // clamped for the lanes outside [zlo, zhi): they own nothing
+  const int k0 = min(max(4 * g, a.zlo), a.zhi - 4);
   const bool own_grp = 4 * g >= a.zlo && 4 * g < a.zhi;
   const int jraw = a.lo[1] + (int)blockIdx.y * FUSED_TR + w - 1;
   const int xs = a.lo[0] + (int)blockIdx.z * a.xseg, xe = min(xs + a.xseg, a.hi[0]);
-  const int j = min(jraw, a.hi[1] - 1);
+  const int j = min(jraw, a.hi[1]), j2 = min(jraw + 1, a.hi[1]);   // hi[1] = n - P - 1: the interface row above the region, in the grid
   const bool own = w >= 1 && jraw < a.hi[1] && own_grp;
-  const bool yp_smem = w < FUSED_TR && jraw + 1 < a.hi[1];
-  const bool shell_row = jraw < a.lo[1];                // the interface row below the first y tile
-  const bool zs_lo = own_grp && k0 == a.zlo, zs_hi = own_grp && k0 + 4 == a.zhi;   // group holds an interface cell (element 0 / 3)
-  const bool edge = own_grp && (lane == 0 || 4 * (g - 1) < a.zlo) && !zs_lo;        // no lane below holds the cell below the group
-  const bool zp_load = lane == 31 || !own_grp || zs_hi;                             // no lane above holds the next group
-  const idx_t sx = d.sx, sy = d.sy;
+  const bool shell_row = jraw < a.lo[1];
+  const bool zs_lo = own_grp && k0 == a.zlo, zs_hi = own_grp && k0 + 4 == a.zhi;
+  const bool edge = own_grp && lane == 0 && !zs_lo;
+  const bool zp_lane = lane == 31 || !own_grp || zs_hi;
+  const bool topw = w == FUSED_TR;
+  const idx_t sx = d.sx;
   const float S = d.S;
-  idx_t q = ((idx_t)(xs - 1) * ny + j) * nz + k0;
+  const idx_t rowoff = (idx_t)j * nz + k0, rowoff2 = (idx_t)j2 * nz + k0;
+  auto issueE = [&](int p) {
+    const int st = p % 3;
+    const idx_t q = (idx_t)p * sx + rowoff;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.E[st][w][c][lane], a.Ein[c] + q);
+    if (topw) {
+      const idx_t q2 = (idx_t)p * sx + rowoff2;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.E[st][FUSED_TR + 1][c][lane], a.Ein[c] + q2);
+      if (edge) fused_cp_async16(&sm.Elo[st][FUSED_TR + 1][2], a.Ein[2] + q2 - 4);
+    }
+    if (edge) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.Elo[st][w][c], a.Ein[c] + q - 4);
+    }
+    if (zp_lane) {
+      fused_cp_async16(&sm.Ehi[st][w][0], a.Ein[0] + q + 4);
+      fused_cp_async16(&sm.Ehi[st][w][1], a.Ein[1] + q + 4);
+    }
+  };
+  auto issueH = [&](int p) {            // H^{m+1/2} of plane p; for interface rows / planes H^{m-1/2} as inject H has written it
+    const int st = p & 1;
+    const idx_t q = (idx_t)p * sx + rowoff;
+    const bool from_out = shell_row || p < a.lo[0];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.Hin[st][w][c][lane], (from_out ? a.Hout[c] : a.Hin[c]) + q);
+    if (edge) {   // the cell below an edge lane's group is an inner cell of this row: its H^{m+1/2} (recomputed below)
+      fused_cp_async16(&sm.Hlo[st][w][0], a.Hin[0] + q - 4);
+      fused_cp_async16(&sm.Hlo[st][w][1], a.Hin[1] + q - 4);
+    }
+  };
   auto put = [](float4& dst, const VF<4>& x) { dst = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]); };
   auto get = [](const float4& t) { VF<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r; };
+  issueE(xs - 1);
+  issueE(xs);
+  issueH(xs - 1);
+  asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll
-  for (int c = 0; c < 3; ++c) {
-    put(sm.E[0][w][c][lane], ldv<4>(a.Ein[c] + q));
-    sm.H[1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-  }
-  int buf = 0;
-  for (int i = xs - 1; i < xe; ++i, q += sx, buf ^= 1) {
-    const bool shell_plane = i < a.lo[0];               // the interface plane below the first x segment
-    const bool from_out = shell_row || shell_plane;     // this worker's H is an interface value: taken from the output buffer
-    const VF<4> exn = ldv<4>(a.Ein[0] + q + sx), eyn = ldv<4>(a.Ein[1] + q + sx), ezn = ldv<4>(a.Ein[2] + q + sx);
-    VF<4> hx, hy, hz;
-    if (from_out) { hx = ldv<4>(a.Hout[0] + q); hy = ldv<4>(a.Hout[1] + q); hz = ldv<4>(a.Hout[2] + q); }
-    else { hx = ldv<4>(a.Hin[0] + q); hy = ldv<4>(a.Hin[1] + q); hz = ldv<4>(a.Hin[2] + q); }
-    // interface cells at the row ends: H^{m-1/2} as inject H has written it (requested here, used after the H update)
-    float sh[3] = {0.0f, 0.0f, 0.0f}, sh3[3] = {0.0f, 0.0f, 0.0f};
-    if (zs_lo && !from_out) { sh[0] = a.Hout[0][q]; sh[1] = a.Hout[1][q]; sh[2] = a.Hout[2][q]; }
-    if (zs_hi && !from_out) { sh3[0] = a.Hout[0][q + 3]; sh3[1] = a.Hout[1][q + 3]; sh3[2] = a.Hout[2][q + 3]; }
-    const VF<4> ex = get(sm.E[buf][w][0][lane]), ey = get(sm.E[buf][w][1][lane]), ez = get(sm.E[buf][w][2][lane]);
-    VF<4> ex_yp, ez_yp;
-    if (yp_smem && i >= xs) {
-      ex_yp = get(sm.E[buf][w + 1][0][lane]);
-      ez_yp = get(sm.E[buf][w + 1][2][lane]);
-    } else {
-      ex_yp = ldv<4>(a.Ein[0] + q + sy);
-      ez_yp = ldv<4>(a.Ein[2] + q + sy);
+  for (int c = 0; c < 3; ++c) sm.Hn[xs & 1][w][c][lane] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+  VF<4> ce_n = zerov<4>();
+  float shn[3] = {0.0f, 0.0f, 0.0f};                    // interface H of the NEXT plane at this row's end (zs_lo: element 0, zs_hi: element 3)
+  const int vi = zs_lo ? 0 : 3;
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  for (int i = xs - 1; i < xe; ++i) {
+    const idx_t q = (idx_t)i * sx + rowoff;
+    const bool from_out = shell_row || i < a.lo[0];
+    if (i + 2 <= xe) issueE(i + 2);
+    if (i + 1 < xe) issueH(i + 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const VF<4> ce = ce_n;
+    const float sh[3] = {shn[0], shn[1], shn[2]};
+    if (own && i + 1 < xe) {
+      ce_n = ldv<4>(d.ce + q + sx);
+      if ((zs_lo || zs_hi) && !shell_row) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) shn[c] = a.Hout[c][q + sx + vi];
+      }
     }
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    const int se = i % 3, sn = (i + 1) % 3, sh_ = i & 1;
+    const VF<4> ex = get(sm.E[se][w][0][lane]), ey = get(sm.E[se][w][1][lane]), ez = get(sm.E[se][w][2][lane]);
+    const VF<4> eyn = get(sm.E[sn][w][1][lane]), ezn = get(sm.E[sn][w][2][lane]);
+    VF<4> hx = get(sm.Hin[sh_][w][0][lane]), hy = get(sm.Hin[sh_][w][1][lane]), hz = get(sm.Hin[sh_][w][2][lane]);
+    const VF<4> ex_yp = get(sm.E[se][w + 1][0][lane]), ez_yp = get(sm.E[se][w + 1][2][lane]);
     float ex_zp = __shfl_down_sync(0xffffffffu, ex.v[0], 1), ey_zp = __shfl_down_sync(0xffffffffu, ey.v[0], 1);
-    if (zp_load) { ex_zp = a.Ein[0][q + 4]; ey_zp = a.Ein[1][q + 4]; }   // q + 4 <= n - P: inside the row
+    if (zp_lane) { ex_zp = sm.Ehi[se][w][0].x; ey_zp = sm.Ehi[se][w][1].x; }
     float hx_e = 0.0f, hy_e = 0.0f;
-    if (edge) {   // new H_x, H_y of the inner cell below the group, in the arithmetic of the inverse-H update
-      const float exm = a.Ein[0][q - 1], eym = a.Ein[1][q - 1], ezm = a.Ein[2][q - 1];
-      hx_e = fmaf(S, (a.Ein[2][q - 1 + sy] - ezm) - (ey.v[0] - eym), a.Hin[0][q - 1]);
-      hy_e = fmaf(S, (ex.v[0] - exm) - (a.Ein[2][q - 1 + sx] - ezm), a.Hin[1][q - 1]);
+    if (edge) {
+      const float exm = sm.Elo[se][w][0].w, eym = sm.Elo[se][w][1].w, ezm = sm.Elo[se][w][2].w;
+      hx_e = fmaf(S, (sm.Elo[se][w + 1][2].w - ezm) - (ey.v[0] - eym), sm.Hlo[sh_][w][0].w);
+      hy_e = fmaf(S, (ex.v[0] - exm) - (sm.Elo[sn][w][2].w - ezm), sm.Hlo[sh_][w][1].w);
     }
     const bool store_plane = own && i >= xs;
-    VF<4> ce;
-    if (store_plane) ce = ldv<4>(d.ce + q);
     // ---- inverse of the H half-step ----
     if (!from_out) {
 #pragma unroll
@@ -445,31 +516,31 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 3) k_fused_iz(const __gri
         hy.v[v] = fmaf(S, (ex_zq - ex.v[v]) - (ezn.v[v] - ez.v[v]), hy.v[v]);
         hz.v[v] = fmaf(S, (eyn.v[v] - ey.v[v]) - (ex_yp.v[v] - ex.v[v]), hz.v[v]);
       }
-      if (zs_lo) { hx.v[0] = sh[0]; hy.v[0] = sh[1]; hz.v[0] = sh[2]; }
-      if (zs_hi) { hx.v[3] = sh3[0]; hy.v[3] = sh3[1]; hz.v[3] = sh3[2]; }
+      if (store_plane && (zs_lo || zs_hi)) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+          if (v == vi) { hx.v[v] = sh[0]; hy.v[v] = sh[1]; hz.v[v] = sh[2]; }
+      }
     }
     float hx_z0 = __shfl_up_sync(0xffffffffu, hx.v[3], 1), hy_z0 = __shfl_up_sync(0xffffffffu, hy.v[3], 1);
     if (edge) { hx_z0 = hx_e; hy_z0 = hy_e; }
-    put(sm.H[buf][w][0][lane], hx); put(sm.H[buf][w][1][lane], hy); put(sm.H[buf][w][2][lane], hz);
-    put(sm.E[buf ^ 1][w][0][lane], exn); put(sm.E[buf ^ 1][w][1][lane], eyn); put(sm.E[buf ^ 1][w][2][lane], ezn);
+    put(sm.Hn[sh_][w][0][lane], hx); put(sm.Hn[sh_][w][1][lane], hy); put(sm.Hn[sh_][w][2][lane], hz);
     __syncthreads();
     if (store_plane) {
       stv<4>(a.Hout[0] + q, hx); stv<4>(a.Hout[1] + q, hy); stv<4>(a.Hout[2] + q, hz);
-      // ---- inverse of the E half-step; the interface elements keep E^m as a placeholder (inject E overwrites them) ----
-      const VF<4> hx_ym = get(sm.H[buf][w - 1][0][lane]), hz_ym = get(sm.H[buf][w - 1][2][lane]);
-      const VF<4> hy_xm = get(sm.H[buf ^ 1][w][1][lane]), hz_xm = get(sm.H[buf ^ 1][w][2][lane]);
-      const VF<4> ex2 = get(sm.E[buf][w][0][lane]), ey2 = get(sm.E[buf][w][1][lane]), ez2 = get(sm.E[buf][w][2][lane]);
+      const VF<4> hx_ym = get(sm.Hn[sh_][w - 1][0][lane]), hz_ym = get(sm.Hn[sh_][w - 1][2][lane]);
+      const VF<4> hy_xm = get(sm.Hn[sh_ ^ 1][w][1][lane]), hz_xm = get(sm.Hn[sh_ ^ 1][w][2][lane]);
       VF<4> eo, e1, e2;
 #pragma unroll
       for (int v = 0; v < 4; ++v) {
         const float hy_zm = v == 0 ? hy_z0 : hy.v[v > 0 ? v - 1 : 0];
         const float hx_zm = v == 0 ? hx_z0 : hx.v[v > 0 ? v - 1 : 0];
-        eo.v[v] = fmaf(-ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex2.v[v]);
-        e1.v[v] = fmaf(-ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey2.v[v]);
-        e2.v[v] = fmaf(-ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez2.v[v]);
+        eo.v[v] = fmaf(-ce.v[v], (hz.v[v] - hz_ym.v[v]) - (hy.v[v] - hy_zm), ex.v[v]);
+        e1.v[v] = fmaf(-ce.v[v], (hx.v[v] - hx_zm) - (hz.v[v] - hz_xm.v[v]), ey.v[v]);
+        e2.v[v] = fmaf(-ce.v[v], (hy.v[v] - hy_xm.v[v]) - (hx.v[v] - hx_ym.v[v]), ez.v[v]);
       }
-      if (zs_lo) { eo.v[0] = ex2.v[0]; e1.v[0] = ey2.v[0]; e2.v[0] = ez2.v[0]; }
-      if (zs_hi) { eo.v[3] = ex2.v[3]; e1.v[3] = ey2.v[3]; e2.v[3] = ez2.v[3]; }
+      if (zs_lo) { eo.v[0] = ex.v[0]; e1.v[0] = ey.v[0]; e2.v[0] = ez.v[0]; }   // interface elements: placeholders, inject E overwrites them
+      if (zs_hi) { eo.v[3] = ex.v[3]; e1.v[3] = ey.v[3]; e2.v[3] = ez.v[3]; }
       stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1); stv<4>(a.Eout[2] + q, e2);
     }
   }
