@@ -31,7 +31,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
   size_t ce, E[3], H[3], E2[3], H2[3], pHz2[2], psiE[3][2], psiH[3][2], tab, step, scratch, srcdesc, waves, store, scales, amax;
-  size_t lE[3], lH[3], lpsiE[2][3][2], lpsiH[2][3][2], acc;
+  size_t lE[3], lH[3], lE2[3], lH2[3], lpsiE[2][3][2], lpsiH[2][3][2], acc;
   size_t eps_own, mon_stage, grad_stage, amp_stage;
   size_t store_cap;
   int slots_cap;
@@ -65,7 +65,7 @@ struct fdtd_sim {
   cudaEvent_t ev_fork = nullptr, ev_mid = nullptr, ev_join[4] = {nullptr, nullptr, nullptr, nullptr};
   bool parallel = false;               // auxiliary streams available
   std::vector<cudaGraphExec_t> dead_graphs;
-  cudaGraphExec_t graph_cache[4] = {nullptr, nullptr, nullptr, nullptr};   // forward, fused forward, reverse, fused reverse
+  cudaGraphExec_t graph_cache[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // forward, fused forward, reverse, fused reverse, fully fused reverse
   mutable std::string err;
   const float* eps_dev = nullptr;
   bool eps_owned = false;              // eps_dev points into the workspace (fdtd_set_eps_host)
@@ -90,7 +90,12 @@ struct fdtd_sim {
   // E/H buffer pair(s): fb[b][0..2] = E, fb[b][3..5] = H of buffer b; d.E / d.H always point at the current one (cb)
   float* fb[2][6] = {{nullptr}};
   int cb = 0;
+  float* lb[2][6] = {{nullptr}};   // lambda_E / lambda_H buffer pair(s), as fb; d.lE / d.lH point at the current one (acb)
+  int acb = 0;
+  bool fa_debug = false;           // DEBUG: fused adjoint path without its marching kernel (slab kernels on the whole grid)
+  int fuse_adj_mode = -1;          // fused adjoint (adjoint of H + adjoint of E in one marching pass): -1 auto, 0 never, 1 whenever possible
   float* pz[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // psi_H of the z axis per buffer: [b][0] H_x term, [b][1] H_y term
+  bool fuse_za = false;    // ... and the adjoint marching kernel (k_fused_ap) applies too
   bool fuse_z = false;     // the fused forward path uses the whole-row marching kernel (k_fused_fp): no class-Z slab boxes
   bool can_fuse = false;   // second buffer present (V == 4, P >= 4)
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
@@ -107,7 +112,8 @@ struct fdtd_sim {
   int V = 1;    // z cells per thread of the lean kernels (4 when nz % 4 == 0 and P % 4 == 0, else 1)
   int VG = 1;   // ... of the general kernels (2 in vector mode)
   // lean regions and complement box lists of the four split half-steps: 0 fwd E, 1 fwd H, 2 adj H, 3 adj E
-  Split split[6]{};   // + 4, 5: the slab kernels' E / H box lists of the fused forward path
+  Split split[8]{};   // + 4, 5: the slab kernels' E / H box lists of the fused forward path; 6, 7: adjoint-of-H / adjoint-of-E box
+                      // lists of the fused adjoint path
 
   // run state
   int nsteps = 0, k = 1, dtype = 0;
@@ -218,6 +224,10 @@ Layout make_layout(const fdtd_sim* s, int nsteps, int dtype, int k, unsigned fla
   if (flags & FDTD_WS_REVERSE) {
     for (int c = 0; c < 3; ++c) L.lE[c] = take(N * 4);
     for (int c = 0; c < 3; ++c) L.lH[c] = take(N * 4);
+    if (s->V == 4 && s->P >= 4) {   // ping-pong partners of lambda_E, lambda_H for the fused adjoint path
+      for (int c = 0; c < 3; ++c) L.lE2[c] = take(N * 4);
+      for (int c = 0; c < 3; ++c) L.lH2[c] = take(N * 4);
+    }
     for (int b = 0; b < 2; ++b)
       for (int c = 0; c < 3; ++c)
         for (int t = 0; t < 2; ++t) {
@@ -323,9 +333,14 @@ Split make_split(const fdtd_sim* s, int which, int x0, int x1) {
       // fused forward path: the marching kernel stores [P+1, n-P); the slab kernels cover the rest plus the plain layers
       // whose values they hand to each other (fdtd_fused.cuh, forward_fused_step)
       case 4: lo = P + 1; hi = n - P; break;                          // fused-path E: layer P joins the slab boxes
-      default: lo = P + 1; hi = n - P - 1; break;                     // fused-path H: layers P and n-P-1 join them
+      case 5: lo = P + 1; hi = n - P - 1; break;                      // fused-path H: layers P and n-P-1 join them
+      // fused adjoint path: the marching kernel stores [P+1, n-P-1) in x and y (whole rows in z); the slab kernels cover the rest,
+      // and their adjoint-of-H boxes also the layer P+1, whose new lambda_E their adjoint-of-E boxes read across the edge
+      case 6: lo = P + 2; hi = n - P - 1; break;
+      default: lo = P + 1; hi = n - P - 1; break;
     }
     if (a == 2 && which >= 4 && s->fuse_z) { lo = 0; hi = n; }   // whole-row marching kernel: z-slab cells ride on their rows
+    if (which >= 6 && s->fa_debug) { lo = 0; hi = 0; }              // DEBUG: no marching kernel, the slab kernels take the whole grid
     else if (a == 2) {
       // z range of the lean region: whole groups of V cells, and (zalign > V) whole 128-byte lines, so that neither the lean
       // nor the z-slab kernels fetch half-used lines (a row of the lean region then starts and ends on a line boundary).
@@ -404,6 +419,11 @@ void set_cur(fdtd_sim* s, int b) {
   if (s->pz[pb][0]) { s->d.psiH[0][1] = s->pz[pb][0]; s->d.psiH[1][0] = s->pz[pb][1]; }
 }
 
+void set_cur_adj(fdtd_sim* s, int b) {
+  s->acb = b;
+  for (int c = 0; c < 3; ++c) { s->d.lE[c] = s->lb[b][c]; s->d.lH[c] = s->lb[b][3 + c]; }
+}
+
 #define LAUNCH(s, kern, grid, block, ...)            \
   do {                                               \
     kern<<<grid, block, 0, (s)->cur>>>(__VA_ARGS__); \
@@ -469,32 +489,38 @@ FieldIO io_inplace(const fdtd_sim* s, int which) {   // which: 0 = E half-step, 
   io_psi_inplace(io, s->d);
   return io;
 }
-void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp, const FieldIO* iop = nullptr) {
+AdjIO adj_inplace(const fdtd_sim* s) {
+  AdjIO io;
+  for (int c = 0; c < 3; ++c) { io.lEin[c] = s->d.lE[c]; io.lH[c] = s->d.lH[c]; io.lEout[c] = s->d.lE[c]; io.lHout[c] = s->d.lH[c]; }
+  return io;
+}
+void launch_gen(fdtd_sim* s, int which, int pb, const Split& sp, const FieldIO* iop = nullptr, const AdjIO* aop = nullptr) {
   const dim3 b(32, TY);
   const BoxList& B = sp.boxes;
   const FieldIO io = iop ? *iop : io_inplace(s, which == 1 ? 1 : 0);
+  const AdjIO ao = aop ? *aop : adj_inplace(s);
   const unsigned g = (unsigned)B.off[B.nb];
   if (g == 0) return;
   if (s->VG == 4) {
     switch (which) {
       case 0: LAUNCH(s, k_gen_e<4>, g, b, s->d, B, io); break;
       case 1: LAUNCH(s, k_gen_h<4>, g, b, s->d, B, io); break;
-      case 2: LAUNCH(s, k_gen_adj_h<4>, g, b, s->d, B, pb); break;
-      default: LAUNCH(s, k_gen_adj_e<4>, g, b, s->d, B, pb);
+      case 2: LAUNCH(s, k_gen_adj_h<4>, g, b, s->d, B, pb, ao); break;
+      default: LAUNCH(s, k_gen_adj_e<4>, g, b, s->d, B, pb, ao);
     }
   } else if (s->VG == 2) {
     switch (which) {
       case 0: LAUNCH(s, k_gen_e<2>, g, b, s->d, B, io); break;
       case 1: LAUNCH(s, k_gen_h<2>, g, b, s->d, B, io); break;
-      case 2: LAUNCH(s, k_gen_adj_h<2>, g, b, s->d, B, pb); break;
-      default: LAUNCH(s, k_gen_adj_e<2>, g, b, s->d, B, pb);
+      case 2: LAUNCH(s, k_gen_adj_h<2>, g, b, s->d, B, pb, ao); break;
+      default: LAUNCH(s, k_gen_adj_e<2>, g, b, s->d, B, pb, ao);
     }
   } else {
     switch (which) {
       case 0: LAUNCH(s, k_gen_e<1>, g, b, s->d, B, io); break;
       case 1: LAUNCH(s, k_gen_h<1>, g, b, s->d, B, io); break;
-      case 2: LAUNCH(s, k_gen_adj_h<1>, g, b, s->d, B, pb); break;
-      default: LAUNCH(s, k_gen_adj_e<1>, g, b, s->d, B, pb);
+      case 2: LAUNCH(s, k_gen_adj_h<1>, g, b, s->d, B, pb, ao); break;
+      default: LAUNCH(s, k_gen_adj_e<1>, g, b, s->d, B, pb, ao);
     }
   }
 }
@@ -812,6 +838,67 @@ void reverse_fused_step(fdtd_sim* s, int m_base, const int* step_dev, const floa
   join(s, 4);
 }
 
+// ---- fully fused reverse step: fused primal (k_fused_ip) AND fused adjoint (adjoint of H + adjoint of E in one marching pass) ----
+AdjIO adj_io(const fdtd_sim* s, int from, int to, bool phase_b) {
+  AdjIO io;
+  for (int c = 0; c < 3; ++c) {
+    io.lEin[c] = phase_b ? s->lb[to][c] : s->lb[from][c];   // adjoint of E reads the NEW lambda_E
+    io.lH[c] = s->lb[from][3 + c];
+    io.lEout[c] = s->lb[to][c];
+    io.lHout[c] = s->lb[to][3 + c];
+  }
+  return io;
+}
+void launch_fused_adj(fdtd_sim* s, int from, int to, int pb);   // the adjoint marching kernel (below)
+// Phase 1: the monitor cotangent first (it changes the current lambda buffers, which everything below reads), then
+//   branch 1: slab kernels, adjoint of H on the boxes of split 6 (current -> other lambda_E), then adjoint of E on those of split 7
+//             (lambda_E other, lambda_H current -> other lambda_H); every lambda_E value the second one reads was written by the first;
+//   branch 0: inject H, the primal marching kernel, its source cells, then the adjoint marching kernel on [P+1, n-P-1)^2 x whole rows
+//             (one after the other: two marching kernels side by side starve each other, profiles/r02c_marching.md).
+// Then both buffer pairs swap.  Phase 2: gradient (new lambda_E, new H) beside inject E (shell gradient term with the new lambda_E).
+void reverse_fullfused_step(fdtd_sim* s, int m_base, const int* step_dev, const float* dmon, int interp, int pb) {
+  const bool cot = dmon && s->has_mon;
+  const int cur = s->cb, oth = cur ^ 1, acur = s->acb, aoth = acur ^ 1;
+  if (cot) launch_box(s, s->mon, const_cast<float*>(dmon), m_base, step_dev, 1);
+  fork(s, 2);
+  on(s, 1);
+  { const AdjIO io = adj_io(s, acur, aoth, false); launch_gen(s, 2, pb, s->split[6], nullptr, &io); }
+  { const AdjIO io = adj_io(s, acur, aoth, true); launch_gen(s, 3, pb, s->split[7], nullptr, &io); }
+  on(s, 0);
+  launch_inject(s, m_base, step_dev, 1, interp, cur, oth);
+  launch_fused(s, true, cur, oth);
+  launch_inv_e_sources(s, m_base, step_dev, cur, oth);
+  if (!s->fa_debug) launch_fused_adj(s, acur, aoth, pb);
+  join(s, 2);
+  set_cur(s, oth);
+  set_cur_adj(s, aoth);
+  fork(s, 2);
+  on(s, 0); launch_grad(s);
+  on(s, 1);
+  launch_sources(s, m_base, step_dev, -1.0f, 0, 1 << 30, cur);
+  launch_inject(s, m_base, step_dev, 0, interp, cur, oth);
+  join(s, 2);
+}
+void launch_fused_adj(fdtd_sim* s, int from, int to, int pb) {
+  FusedAArgs a;
+  for (int c = 0; c < 3; ++c) {
+    a.lEin[c] = s->lb[from][c]; a.lHin[c] = s->lb[from][3 + c];
+    a.lEout[c] = s->lb[to][c]; a.lHout[c] = s->lb[to][3 + c];
+  }
+  const int nb = pb ^ 1;
+  a.pH_in[0] = s->d.lpsiH[pb][0][1]; a.pH_in[1] = s->d.lpsiH[pb][1][0];
+  a.pH_out[0] = s->d.lpsiH[nb][0][1]; a.pH_out[1] = s->d.lpsiH[nb][1][0];
+  a.pE_in[0] = s->d.lpsiE[pb][0][1]; a.pE_in[1] = s->d.lpsiE[pb][1][0];
+  a.pE_out[0] = s->d.lpsiE[nb][0][1]; a.pE_out[1] = s->d.lpsiE[nb][1][0];
+  for (int ax = 0; ax < 2; ++ax) { a.lo[ax] = s->P + 1; a.hi[ax] = s->n[ax] - s->P - 1; }
+  if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1]) return;
+  a.xseg = fused_xseg(s);
+  const dim3 g((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((a.hi[1] - a.lo[1] + FUSED_TR - 1) / FUSED_TR),
+               (unsigned)((a.hi[0] - a.lo[0] + a.xseg - 1) / a.xseg));
+  k_fused_ap<<<g, dim3(32, FUSED_TR + 1), sizeof(FusedASmem), s->cur>>>(s->d, a);
+  ++s->launches;
+}
+
 // Capture `body` (which enqueues on s->stream and its auxiliaries) into a graph and launch it `times` times.  The
 // instantiated graph of each kind (slot 0 forward, 1 fused forward, 2 reverse) is kept in the handle: the next run
 // re-captures (pointers such as the monitor record may have changed) and patches the kept executable with
@@ -955,6 +1042,11 @@ bool use_fused_reverse(const fdtd_sim* s) {
   // step: on; C3 (196 tiles) 234.8 vs 223.7: off.
   return s->use_iz && s->n[2] - 2 * s->P >= 8 && fused_tiles(s, 32) >= 4 * 2 * 148;
 }
+bool use_fused_adjoint(const fdtd_sim* s) {
+  if (s->fuse_adj_mode == 0 || !use_fused_reverse(s) || !s->fuse_za || !s->lb[1][0]) return false;
+  if (s->fuse_adj_mode >= 1) return true;
+  return false;   // auto: off until measured
+}
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
   launch_record(s, 0, nullptr, 2);
@@ -1055,6 +1147,9 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   const size_t N = (size_t)s->d.N;
   s->cur = s->stream;
   if (s->dead_graphs.size() > 32) { CUDA_TRY(s, cudaStreamSynchronize(s->stream)); reap_graphs(s); }
+  set_cur_adj(s, 0);
+  for (int c = 0; c < 6; ++c)
+    if (s->lb[1][c]) CUDA_TRY(s, cudaMemsetAsync(s->lb[1][c], 0, N * 4, s->stream));
   for (int c = 0; c < 3; ++c) {
     CUDA_TRY(s, cudaMemsetAsync(s->d.lE[c], 0, N * 4, s->stream));
     CUDA_TRY(s, cudaMemsetAsync(s->d.lH[c], 0, N * 4, s->stream));
@@ -1080,6 +1175,7 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
   int pb = 0;
   int top = s->nsteps;
   const bool rf = use_fused_reverse(s);   // inverse-H + inverse-E of the primal in one marching kernel (ping-pong buffers)
+  const bool fa = use_fused_adjoint(s);   // ... and adjoint of H + adjoint of E in one marching kernel (lambda ping-pong buffers)
   {
     const int L = 16;   // even, so the psi ping-pong parity is the same at the start of every period
     const int periods = (s->use_graphs && s->aux[0]) ? s->nsteps / L : 0;
@@ -1087,9 +1183,10 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
       int* step_dev = reinterpret_cast<int*>(s->ws + s->L.step);
       LAUNCH(s, k_set_int, 1, 1, step_dev, s->nsteps);
       s->parallel = true;
-      fdtd_status g = run_graph(s, rf ? 3 : 2, periods, [&]() {
+      fdtd_status g = run_graph(s, fa ? 4 : (rf ? 3 : 2), periods, [&]() {
         for (int t = 0; t < L; ++t) {
-          if (rf) reverse_fused_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+          if (fa) reverse_fullfused_step(s, -t, step_dev, dmon, (int)interp, t & 1);
+          else if (rf) reverse_fused_step(s, -t, step_dev, dmon, (int)interp, t & 1);
           else reverse_step(s, -t, step_dev, dmon, (int)interp, t & 1);
         }
         LAUNCH(s, k_tick, 1, 1, step_dev, -L);
@@ -1101,7 +1198,8 @@ fdtd_status reverse_impl(fdtd_sim* s, const fdtd_cotangent* fin, const float* dm
     }
   }
   for (int m = top; m >= 1; --m, pb ^= 1) {
-    if (rf) reverse_fused_step(s, m, nullptr, dmon, (int)interp, pb);
+    if (fa) reverse_fullfused_step(s, m, nullptr, dmon, (int)interp, pb);
+    else if (rf) reverse_fused_step(s, m, nullptr, dmon, (int)interp, pb);
     else reverse_step(s, m, nullptr, dmon, (int)interp, pb);
   }
   if (grad_dev && s->has_design)
@@ -1159,6 +1257,8 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   if (const char* e = std::getenv("FDTD_ZF")) s->use_zf = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_FZ")) s->use_fz = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_IZ")) s->use_iz = atoi(e) != 0;
+  if (const char* e = std::getenv("FDTD_FUSE_ADJ")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_adj_mode = v; }
+  if (const char* e = std::getenv("FDTD_FA_DEBUG")) s->fa_debug = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
@@ -1249,9 +1349,13 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
     bool ok = s->can_fuse && s->use_fz && 2 * s->P <= 4 * FUSED_ZSL;   // the staging area of the slab lanes
     for (int kb = 128; ok && kb < s->n[2]; kb += 128) ok = kb - 1 >= s->P && kb - 1 < s->n[2] - s->P;
     s->fuse_z = ok;
+    // the adjoint marching kernel recomputes the cell ABOVE a tile boundary: that one has to be plain as well
+    for (int kb = 128; ok && kb < s->n[2]; kb += 128) ok = kb < s->n[2] - s->P;
+    s->fuse_za = ok;
     if (s->can_fuse) {   // the whole-row marching kernels use more than 48 KB of shared memory per block: opt in (not during a capture)
       CUDA_TRY(s, cudaFuncSetAttribute(k_fused_fp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedPSmem)));
       CUDA_TRY(s, cudaFuncSetAttribute(k_fused_ip, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedQSmem)));
+      CUDA_TRY(s, cudaFuncSetAttribute(k_fused_ap, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FusedASmem)));
     }
   }
   for (int c = 0; c < 3; ++c) {
@@ -1283,6 +1387,12 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
         }
     }
     d.acc = reinterpret_cast<double*>(w + L.acc);
+    for (int c = 0; c < 3; ++c) {
+      s->lb[0][c] = d.lE[c]; s->lb[0][3 + c] = d.lH[c];
+      s->lb[1][c] = s->can_fuse ? reinterpret_cast<float*>(w + L.lE2[c]) : nullptr;
+      s->lb[1][3 + c] = s->can_fuse ? reinterpret_cast<float*>(w + L.lH2[c]) : nullptr;
+    }
+    s->acb = 0;
   }
   d.has_design = s->has_design ? 1 : 0;
   {   // ce resident in L2 during the reverse run where it fits a third of it (fdtd_dev.cuh, ldv_ce)
@@ -1313,7 +1423,7 @@ fdtd_status fdtd_set_workspace(fdtd_sim* s, void* ws_dev, size_t bytes, int nste
   }
   s->VG = s->V;
   if (const char* e = std::getenv("FDTD_VG")) { const int v = atoi(e); if ((v == 1 || v == 2 || v == 4) && s->V == 4) s->VG = v; }
-  for (int which = 0; which < 6; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
+  for (int which = 0; which < 8; ++which) s->split[which] = make_split(s, which, 0, s->n[0]);
   build_tables(s);
   CUDA_TRY(s, cudaMemcpyAsync(w + L.tab, s->tables_host.data(), s->tables_host.size() * 4, cudaMemcpyHostToDevice, s->stream));
   CUDA_TRY(s, cudaMemsetAsync(w + L.step, 0, 16, s->stream));
@@ -1346,7 +1456,7 @@ fdtd_status fdtd_set_graphs(fdtd_sim* s, int enabled) {
 
 fdtd_status fdtd_set_fused(fdtd_sim* s, int mode, int xseg) {
   if (!s || mode < -1 || mode > 1 || xseg < 0) return FDTD_ERR_INVALID_ARG;
-  s->fuse_mode = s->fuse_rev_mode = mode;
+  s->fuse_mode = s->fuse_rev_mode = s->fuse_adj_mode = mode;
   if (xseg > 0) s->xseg = xseg;
   return FDTD_OK;
 }
@@ -1765,7 +1875,7 @@ void fdtd_destroy(fdtd_sim* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
   reap_graphs(s);
-  for (int g = 0; g < 4; ++g)
+  for (int g = 0; g < 5; ++g)
     if (s->graph_cache[g]) cudaGraphExecDestroy(s->graph_cache[g]);
   for (int b = 0; b < 4; ++b) {
     if (s->aux[b]) cudaStreamDestroy(s->aux[b]);

@@ -52,6 +52,15 @@ __device__ __host__ __forceinline__ void io_psi_inplace(FieldIO& io, const Dev& 
   io.pHz_in[1] = io.pHz_out[1] = d.psiH[1][0];
 }
 
+// Input / output arrays of an adjoint half-step: in place (out == in) in the two-kernel path, other buffer in the fused adjoint
+// path (the adjoint marching kernel recomputes halo cells from OLD values, so lambda_E / lambda_H are ping-ponged there).
+//  adjoint of H (A): reads lH, lEin; writes lEout.      adjoint of E (B): reads lEin (the NEW lambda_E), lH; writes lHout.
+struct AdjIO {
+  const float* lEin[3];
+  const float* lH[3];
+  float* lEout[3];
+  float* lHout[3];
+};
 // A lean kernel's region (plain Yee cells) and the list of boxes that make up its complement (slab cells and the
 // layers that touch them).  Each box has a class that says which CPML axes can occur in it (so the others compile
 // out) and its own lane shape: G lanes along z (groups of V cells) x RW rows per warp, G*RW <= 32.

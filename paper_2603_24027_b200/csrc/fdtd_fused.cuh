@@ -427,7 +427,10 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 2) k_fused_ip(const __gri
   const bool shell_row = jraw < a.lo[1];
   const bool zs_lo = own_grp && k0 == a.zlo, zs_hi = own_grp && k0 + 4 == a.zhi;
   const bool edge = own_grp && lane == 0 && !zs_lo;
-  const bool zp_lane = lane == 31 || !own_grp || zs_hi;
+  // the one lane per warp whose z+1 neighbour lies in the next tile.  (The row's last group, zs_hi, needs it for its interface
+  // element only, which is replaced; lanes outside [zlo, zhi) own nothing.  They must NOT share the staging slot: the slot has one
+  // writer per warp.)
+  const bool zp_lane = lane == 31 && own_grp && !zs_hi;
   const bool topw = w == FUSED_TR;
   const idx_t sx = d.sx;
   const float S = d.S;
@@ -542,6 +545,232 @@ __global__ void __launch_bounds__(32 * (FUSED_TR + 1), 2) k_fused_ip(const __gri
       if (zs_lo) { eo.v[0] = ex.v[0]; e1.v[0] = ey.v[0]; e2.v[0] = ez.v[0]; }   // interface elements: placeholders, inject E overwrites them
       if (zs_hi) { eo.v[3] = ex.v[3]; e1.v[3] = ey.v[3]; e2.v[3] = ez.v[3]; }
       stv<4>(a.Eout[0] + q, eo); stv<4>(a.Eout[1] + q, e1); stv<4>(a.Eout[2] + q, e2);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// k_fused_ap — adjoint marching kernel: the adjoint of the H half-step (A: lambda_E += -S curl^-(lambda_H), transposed psi_H terms)
+// and the adjoint of the E half-step (B: lambda_H += curl^+(ce lambda_E), transposed psi_E terms) of one reverse step in ONE pass
+// over the rows of [P+1, n-P-1)^2, whole rows in z: 52 B per cell instead of 36 + 40.  The mirror image of k_fused_fp: A reads the
+// LOW-side neighbours of the old lambda_H, B the HIGH-side neighbours of the new lambda_E, so the march runs DOWN in x, the halo
+// workers sit on the high side (the warp above the tile, the plane above the segment: they compute A from the old values and store
+// nothing — hence ping-ponged lambda_E / lambda_H), and the cell above a tile's last group is recomputed by the last lane.
+// Loads are staged through shared memory by cp.async a plane ahead, as in k_fused_fp.  The transposed z CPML runs in the lanes of
+// the z slabs in the arithmetic of gen_adj_h_body / gen_adj_e_body for a class-Z box; the W terms of the neighbouring cell travel by
+// warp shuffle (same expression, same inputs: same bits).  lambda_psi is ping-ponged by the step parity already (pb -> pb ^ 1).
+// ---------------------------------------------------------------------------------------------------------
+struct FusedAArgs {
+  const float* lEin[3];
+  const float* lHin[3];
+  float* lEout[3];
+  float* lHout[3];
+  const float* pH_in[2];    // old lambda_psi_H of the z axis: [0] the H_x term (lpsiH[pb][0][1]), [1] the H_y term (lpsiH[pb][1][0])
+  float* pH_out[2];
+  const float* pE_in[2];    // old lambda_psi_E of the z axis: [0] the E_x term (lpsiE[pb][0][1]), [1] the E_y term (lpsiE[pb][1][0])
+  float* pE_out[2];
+  int lo[2], hi[2];
+  int xseg;
+};
+struct FusedASmem {
+  float4 H[3][FUSED_TR + 2][3][32];     // old lambda_H of plane p in stage p % 3; row slot r = row (first row of the tile) - 1 + r
+  float4 E[2][FUSED_TR + 1][3][32];     // old lambda_E of plane p in stage p % 2; row slot w
+  float4 G[2][FUSED_TR + 1][3][32];     // new ce * lambda_E of plane p in stage p % 2
+  float4 P[2][4][FUSED_TR + 1][FUSED_ZSL];   // lambda_psi of the z axis: psiH x-term, psiH y-term, psiE x-term, psiE y-term
+  float4 Hlo[3][FUSED_TR + 1][2];       // lambda_H_x, lambda_H_y of the group below the tile's first group (lane 0)
+  float4 Hhi[3][FUSED_TR + 2][3];       // lambda_H of the group above the warp's last group (last lane), rows as H
+  float4 Ehi[2][FUSED_TR + 1][2];       // old lambda_E_x, lambda_E_y of that group
+  float4 Chi[2][FUSED_TR + 1];          // ce of that group
+  float C[6][FUSED_ZSL * 4];
+};
+__global__ void __launch_bounds__(32 * (FUSED_TR + 1), 2) k_fused_ap(const __grid_constant__ Dev d, const __grid_constant__ FusedAArgs a) {
+  extern __shared__ __align__(16) unsigned char ap_smem_raw[];
+  FusedASmem& sm = *reinterpret_cast<FusedASmem*>(ap_smem_raw);
+  const int lane = threadIdx.x, w = threadIdx.y;
+  const int ny = d.n[1], nz = d.n[2], P = d.P;
+  const int g = (int)blockIdx.x * 32 + lane, ngroups = nz / 4;
+  const bool own_grp = g < ngroups;
+  const int k0 = min(g, ngroups - 1) * 4;
+  const int j0 = a.lo[1] + (int)blockIdx.y * FUSED_TR;          // first row of the tile
+  const int jraw = j0 + w;
+  const int xs = a.lo[0] + (int)blockIdx.z * a.xseg, xe = min(xs + a.xseg, a.hi[0]);
+  const int j = min(jraw, a.hi[1]);                              // rows above the region clamp to the first row above it
+  const bool own = w < FUSED_TR && jraw < a.hi[1] && own_grp;
+  const bool zs = P > 0 && in_slab(k0, nz, P);
+  const bool za = zs || (k0 > 0 && P > 0 && in_slab(k0 - 1, nz, P));          // A needs W of the cell below
+  const bool zb = zs || (k0 + 4 < nz && P > 0 && in_slab(k0 + 4, nz, P));      // B needs W of the cell above
+  const bool wall = k0 == 0, top = k0 + 4 >= nz;
+  const bool lo_lane = lane == 0 && blockIdx.x > 0 && own_grp;                 // the cell below the group belongs to the tile below
+  const bool hi_lane = (lane == 31 || g + 1 >= ngroups) && !top && own_grp;    // no lane above holds the next group
+  const idx_t sx = d.sx;
+  const float S = d.S;
+  const int szl = zs ? slab_s(k0, nz, P) : 0;
+  const int sl = szl / 4;
+  const idx_t rowoff = (idx_t)j * nz + k0, rowoff_m = (idx_t)(j0 - 1) * nz + k0;
+  if (zs && w == 0) {
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      sm.C[0][sl * 4 + v] = __ldg(d.tab[2][3] + k0 + v); sm.C[1][sl * 4 + v] = __ldg(d.tab[2][4] + k0 + v); sm.C[2][sl * 4 + v] = __ldg(d.tab[2][5] + k0 + v);
+      sm.C[3][sl * 4 + v] = __ldg(d.tab[2][0] + k0 + v); sm.C[4][sl * 4 + v] = __ldg(d.tab[2][1] + k0 + v); sm.C[5][sl * 4 + v] = __ldg(d.tab[2][2] + k0 + v);
+    }
+  }
+  auto issueH = [&](int p) {            // old lambda_H of plane p (rows: own slot w + 1; warp 0 also slot 0 = the row below the tile)
+    const int st = p % 3;
+    const idx_t q = (idx_t)p * sx + rowoff;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.H[st][w + 1][c][lane], a.lHin[c] + q);
+    if (lo_lane) {
+      fused_cp_async16(&sm.Hlo[st][w][0], a.lHin[0] + q - 4);
+      fused_cp_async16(&sm.Hlo[st][w][1], a.lHin[1] + q - 4);
+    }
+    if (hi_lane) {
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.Hhi[st][w + 1][c], a.lHin[c] + q + 4);
+    }
+    if (w == 0) {
+      const idx_t qm = (idx_t)p * sx + rowoff_m;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.H[st][0][c][lane], a.lHin[c] + qm);
+      if (hi_lane) fused_cp_async16(&sm.Hhi[st][0][2], a.lHin[2] + qm + 4);
+    }
+  };
+  auto issueE = [&](int p) {            // old lambda_E, lambda_psi of plane p
+    const int st = p & 1;
+    const idx_t q = (idx_t)p * sx + rowoff;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) fused_cp_async16(&sm.E[st][w][c][lane], a.lEin[c] + q);
+    if (hi_lane) {
+      fused_cp_async16(&sm.Ehi[st][w][0], a.lEin[0] + q + 4);
+      fused_cp_async16(&sm.Ehi[st][w][1], a.lEin[1] + q + 4);
+      fused_cp_async16(&sm.Chi[st][w], d.ce + q + 4);
+    }
+    if (zs) {
+      const idx_t qp = ((idx_t)p * ny + j) * (2 * P) + szl;
+      fused_cp_async16(&sm.P[st][0][w][sl], a.pH_in[0] + qp);
+      fused_cp_async16(&sm.P[st][1][w][sl], a.pH_in[1] + qp);
+      fused_cp_async16(&sm.P[st][2][w][sl], a.pE_in[0] + qp);
+      fused_cp_async16(&sm.P[st][3][w][sl], a.pE_in[1] + qp);
+    }
+  };
+  auto put = [](float4& dst, const VF<4>& x) { dst = make_float4(x.v[0], x.v[1], x.v[2], x.v[3]); };
+  auto get = [](const float4& t) { VF<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r; };
+  issueH(xe);
+  issueH(xe - 1);
+  issueE(xe);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  VF<4> ce_n = ldv<4>(d.ce + (idx_t)xe * sx + rowoff);   // ce of the priming plane
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();
+  for (int i = xe; i >= xs; --i) {
+    const idx_t q = (idx_t)i * sx + rowoff;
+    const idx_t qz = ((idx_t)i * ny + j) * (2 * P) + szl;
+    if (i - 2 >= xs - 1) issueH(i - 2);
+    if (i - 1 >= xs) issueE(i - 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    const VF<4> ce = ce_n;
+    if (i - 1 >= xs) ce_n = ldv<4>(d.ce + q - sx);
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    const int s0 = i % 3, s1 = (i - 1) % 3, se = i & 1;
+    const bool store_plane = own && i < xe;
+    // ---- A: adjoint of the H half-step at plane i ----
+    const VF<4> lhx = get(sm.H[s0][w + 1][0][lane]), lhy = get(sm.H[s0][w + 1][1][lane]), lhz = get(sm.H[s0][w + 1][2][lane]);
+    const VF<4> lhy_xm = get(sm.H[s1][w + 1][1][lane]), lhz_xm = get(sm.H[s1][w + 1][2][lane]);
+    const VF<4> lhx_ym = get(sm.H[s0][w][0][lane]), lhz_ym = get(sm.H[s0][w][2][lane]);
+    VF<4> lex = get(sm.E[se][w][0][lane]), ley = get(sm.E[se][w][1][lane]), lez = get(sm.E[se][w][2][lane]);
+    float lhx_z0 = __shfl_up_sync(0xffffffffu, lhx.v[3], 1), lhy_z0 = __shfl_up_sync(0xffffffffu, lhy.v[3], 1);
+    if (lo_lane) { lhx_z0 = sm.Hlo[s0][w][0].w; lhy_z0 = sm.Hlo[s0][w][1].w; }
+    if (wall) { lhx_z0 = 0.0f; lhy_z0 = 0.0f; }
+#pragma unroll
+    for (int v = 0; v < 4; ++v) {
+      const float lhy_zm = v == 0 ? lhy_z0 : lhy.v[v > 0 ? v - 1 : 0];
+      const float lhx_zm = v == 0 ? lhx_z0 : lhx.v[v > 0 ? v - 1 : 0];
+      lex.v[v] = fmaf(-S, (lhz.v[v] - lhz_ym.v[v]) - (lhy.v[v] - lhy_zm), lex.v[v]);
+      ley.v[v] = fmaf(-S, (lhx.v[v] - lhx_zm) - (lhz.v[v] - lhz_xm.v[v]), ley.v[v]);
+      lez.v[v] = fmaf(-S, (lhy.v[v] - lhy_xm.v[v]) - (lhx.v[v] - lhx_ym.v[v]), lez.v[v]);
+    }
+    {   // transposed psi_H terms of the z axis: (c=0,t=1: g = +S*lH_x -> lE_y) and (c=1,t=0: g = -S*lH_y -> lE_x)
+      float w01[4] = {0.0f, 0.0f, 0.0f, 0.0f}, w10[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+      if (zs) {
+        const VF<4> o01 = get(sm.P[se][0][w][sl]), o10 = get(sm.P[se][1][w][sl]);
+        VF<4> n01, n10;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float bz = sm.C[0][sl * 4 + v], cz = sm.C[1][sl * 4 + v], kz = sm.C[2][sl * 4 + v];
+          w01[v] = cpml_adjoint_term(S * lhx.v[v], o01.v[v], bz, cz, kz, n01.v[v]);
+          w10[v] = cpml_adjoint_term(-S * lhy.v[v], o10.v[v], bz, cz, kz, n10.v[v]);
+        }
+        if (store_plane) { stv<4>(a.pH_out[0] + qz, n01); stv<4>(a.pH_out[1] + qz, n10); }
+      }
+      float w01_m = __shfl_up_sync(0xffffffffu, w01[3], 1), w10_m = __shfl_up_sync(0xffffffffu, w10[3], 1);
+      if (lane == 0) { w01_m = 0.0f; w10_m = 0.0f; }   // the cell below a tile is a plain cell without a slab neighbour (host check)
+      if (za) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float w01m = v == 0 ? w01_m : w01[v > 0 ? v - 1 : 0];
+          const float w10m = v == 0 ? w10_m : w10[v > 0 ? v - 1 : 0];
+          lex.v[v] -= (w10[v] - w10m);
+          ley.v[v] -= (w01[v] - w01m);
+        }
+      }
+    }
+    if (wall) { lex.v[0] = 0.0f; ley.v[0] = 0.0f; }   // PEC-masked nodes (z = 0)
+    if (store_plane) { stv<4>(a.lEout[0] + q, lex); stv<4>(a.lEout[1] + q, ley); stv<4>(a.lEout[2] + q, lez); }
+    // ---- G = ce * lambda_E (new) at the cell; at the cell above the warp's last group by the last lane ----
+    VF<4> gx, gy, gz;
+#pragma unroll
+    for (int v = 0; v < 4; ++v) { gx.v[v] = ce.v[v] * lex.v[v]; gy.v[v] = ce.v[v] * ley.v[v]; gz.v[v] = ce.v[v] * lez.v[v]; }
+    float gx_zp = __shfl_down_sync(0xffffffffu, gx.v[0], 1), gy_zp = __shfl_down_sync(0xffffffffu, gy.v[0], 1);
+    if (hi_lane) {   // A at (i, j, k0 + 4), a plain cell: new lambda_E_x, lambda_E_y there
+      const float hxq = sm.Hhi[s0][w + 1][0].x, hyq = sm.Hhi[s0][w + 1][1].x, hzq = sm.Hhi[s0][w + 1][2].x;
+      const float ex_q = fmaf(-S, (hzq - sm.Hhi[s0][w][2].x) - (hyq - lhy.v[3]), sm.Ehi[se][w][0].x);
+      const float ey_q = fmaf(-S, (hxq - lhx.v[3]) - (hzq - sm.Hhi[s1][w + 1][2].x), sm.Ehi[se][w][1].x);
+      const float ceq = sm.Chi[se][w].x;
+      gx_zp = ceq * ex_q;
+      gy_zp = ceq * ey_q;
+    }
+    if (top) { gx_zp = 0.0f; gy_zp = 0.0f; }
+    // transposed psi_E terms of the z axis: (c=0,t=1: g = -G_x -> lH_y) and (c=1,t=0: g = +G_y -> lH_x); W of the cell above by shuffle
+    float u01[4] = {0.0f, 0.0f, 0.0f, 0.0f}, u10[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    VF<4> m01 = zerov<4>(), m10 = zerov<4>();
+    if (zs) {
+      const VF<4> o01 = get(sm.P[se][2][w][sl]), o10 = get(sm.P[se][3][w][sl]);
+      m01 = o01; m10 = o10;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        if (k0 + v == 0) continue;                      // PEC-masked nodes: W = 0, lambda_psi kept
+        const float bz = sm.C[3][sl * 4 + v], cz = sm.C[4][sl * 4 + v], kz = sm.C[5][sl * 4 + v];
+        u01[v] = cpml_adjoint_term(-gx.v[v], o01.v[v], bz, cz, kz, m01.v[v]);
+        u10[v] = cpml_adjoint_term(gy.v[v], o10.v[v], bz, cz, kz, m10.v[v]);
+      }
+    }
+    float u01_p = __shfl_down_sync(0xffffffffu, u01[0], 1), u10_p = __shfl_down_sync(0xffffffffu, u10[0], 1);
+    if (lane == 31 || g + 1 >= ngroups) { u01_p = 0.0f; u10_p = 0.0f; }   // the cell above a tile is a plain cell (host check) or the ghost
+    put(sm.G[se][w][0][lane], gx); put(sm.G[se][w][1][lane], gy); put(sm.G[se][w][2][lane], gz);
+    __syncthreads();
+    if (store_plane) {
+      // ---- B: adjoint of the E half-step at plane i ----
+      const VF<4> gx_yp = get(sm.G[se][w + 1][0][lane]), gz_yp = get(sm.G[se][w + 1][2][lane]);
+      const VF<4> gy_xp = get(sm.G[se ^ 1][w][1][lane]), gz_xp = get(sm.G[se ^ 1][w][2][lane]);
+      VF<4> nhx, nhy, nhz;
+#pragma unroll
+      for (int v = 0; v < 4; ++v) {
+        const float gx_zq = v == 3 ? gx_zp : gx.v[v < 3 ? v + 1 : v];
+        const float gy_zq = v == 3 ? gy_zp : gy.v[v < 3 ? v + 1 : v];
+        nhx.v[v] = lhx.v[v] + ((gz_yp.v[v] - gz.v[v]) - (gy_zq - gy.v[v]));
+        nhy.v[v] = lhy.v[v] + ((gx_zq - gx.v[v]) - (gz_xp.v[v] - gz.v[v]));
+        nhz.v[v] = lhz.v[v] + ((gy_xp.v[v] - gy.v[v]) - (gx_yp.v[v] - gx.v[v]));
+      }
+      if (zb) {
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          const float u01p = v == 3 ? u01_p : u01[v < 3 ? v + 1 : v];
+          const float u10p = v == 3 ? u10_p : u10[v < 3 ? v + 1 : v];
+          nhx.v[v] -= (u10p - u10[v]);
+          nhy.v[v] -= (u01p - u01[v]);
+        }
+      }
+      if (zs) { stv<4>(a.pE_out[0] + qz, m01); stv<4>(a.pE_out[1] + qz, m10); }
+      stv<4>(a.lHout[0] + q, nhx); stv<4>(a.lHout[1] + q, nhy); stv<4>(a.lHout[2] + q, nhz);
     }
   }
 }

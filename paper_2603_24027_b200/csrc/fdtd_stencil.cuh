@@ -546,28 +546,28 @@ __global__ void __launch_bounds__(256) k_grad(const __grid_constant__ Dev d) {
 // missing lpsi reads as zero, so absent terms evaluate to W = 0 exactly.
 // ---------------------------------------------------------------------------------------------------------
 template <int V, bool HX, bool HY>
-__device__ __forceinline__ void gen_adj_h_body(const Dev& d, const int i, const int j, const int k0, int pb) {
+__device__ __forceinline__ void gen_adj_h_body(const Dev& d, const int i, const int j, const int k0, int pb, const AdjIO& io) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const float S = d.S;
   const int nb = pb ^ 1;
-  const VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
+  const VF<V> lhx = ldv<V>(io.lH[0] + q), lhy = ldv<V>(io.lH[1] + q), lhz = ldv<V>(io.lH[2] + q);
   VF<V> lhy_xm = zerov<V>(), lhz_xm = zerov<V>(), lhx_ym = zerov<V>(), lhz_ym = zerov<V>();
   if (i > 0) {
-    lhy_xm = ldv<V>(d.lH[1] + q - sx);
-    lhz_xm = ldv<V>(d.lH[2] + q - sx);
+    lhy_xm = ldv<V>(io.lH[1] + q - sx);
+    lhz_xm = ldv<V>(io.lH[2] + q - sx);
   }
   if (j > 0) {
-    lhx_ym = ldv<V>(d.lH[0] + q - sy);
-    lhz_ym = ldv<V>(d.lH[2] + q - sy);
+    lhx_ym = ldv<V>(io.lH[0] + q - sy);
+    lhz_ym = ldv<V>(io.lH[2] + q - sy);
   }
   float lhx_z0 = 0.0f, lhy_z0 = 0.0f;
   if (k0 > 0) {
-    lhx_z0 = d.lH[0][q - 1];
-    lhy_z0 = d.lH[1][q - 1];
+    lhx_z0 = io.lH[0][q - 1];
+    lhy_z0 = io.lH[1][q - 1];
   }
-  VF<V> lex = ldv<V>(d.lE[0] + q), ley = ldv<V>(d.lE[1] + q), lez = ldv<V>(d.lE[2] + q);
+  VF<V> lex = ldv<V>(io.lEin[0] + q), ley = ldv<V>(io.lEin[1] + q), lez = ldv<V>(io.lEin[2] + q);
 
   const bool xs = HX && P > 0 && in_slab(i, nx, P), xsm = HX && P > 0 && i > 0 && in_slab(i - 1, nx, P);
   const bool ys = HY && P > 0 && in_slab(j, ny, P), ysm = HY && P > 0 && j > 0 && in_slab(j - 1, ny, P);
@@ -692,9 +692,9 @@ __device__ __forceinline__ void gen_adj_h_body(const Dev& d, const int i, const 
       if (i == 0 || j == 0) lez.v[v] = 0.0f;
     }
   }
-  stv<V>(d.lE[0] + q, lex);
-  stv<V>(d.lE[1] + q, ley);
-  stv<V>(d.lE[2] + q, lez);
+  stv<V>(io.lEout[0] + q, lex);
+  stv<V>(io.lEout[1] + q, ley);
+  stv<V>(io.lEout[2] + q, lez);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -704,32 +704,32 @@ __device__ __forceinline__ void gen_adj_h_body(const Dev& d, const int i, const 
 // Same layout as gen_adj_h_body: plain part, then the z, y, x correction blocks (lH_x: z,y; lH_y: z,x; lH_z: y,x).
 // ---------------------------------------------------------------------------------------------------------
 template <int V, bool HX, bool HY>
-__device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const int j, const int k0, int pb) {
+__device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const int j, const int k0, int pb, const AdjIO& io) {
   const int nx = d.n[0], ny = d.n[1], nz = d.n[2], P = d.P;
   const idx_t sx = d.sx, sy = d.sy;
   const idx_t q = ((idx_t)i * ny + j) * nz + k0;
   const int nb = pb ^ 1;
   const VF<V> ce = ldv_ce<V>(d, d.ce + q);
-  VF<V> gx = ldv<V>(d.lE[0] + q), gy = ldv<V>(d.lE[1] + q), gz = ldv<V>(d.lE[2] + q);
+  VF<V> gx = ldv<V>(io.lEin[0] + q), gy = ldv<V>(io.lEin[1] + q), gz = ldv<V>(io.lEin[2] + q);
   VF<V> gy_xp = zerov<V>(), gz_xp = zerov<V>(), gx_yp = zerov<V>(), gz_yp = zerov<V>();
   VF<V> ce_xp = zerov<V>(), ce_yp = zerov<V>();
   float gx_zp = 0.0f, gy_zp = 0.0f, ce_zp = 0.0f;
   if (i + 1 < nx) {
     ce_xp = ldv_ce<V>(d, d.ce + q + sx);
-    gy_xp = ldv<V>(d.lE[1] + q + sx);
-    gz_xp = ldv<V>(d.lE[2] + q + sx);
+    gy_xp = ldv<V>(io.lEin[1] + q + sx);
+    gz_xp = ldv<V>(io.lEin[2] + q + sx);
   }
   if (j + 1 < ny) {
     ce_yp = ldv_ce<V>(d, d.ce + q + sy);
-    gx_yp = ldv<V>(d.lE[0] + q + sy);
-    gz_yp = ldv<V>(d.lE[2] + q + sy);
+    gx_yp = ldv<V>(io.lEin[0] + q + sy);
+    gz_yp = ldv<V>(io.lEin[2] + q + sy);
   }
   if (k0 + V < nz) {
     ce_zp = d.ce[q + V];
-    gx_zp = d.lE[0][q + V];
-    gy_zp = d.lE[1][q + V];
+    gx_zp = io.lEin[0][q + V];
+    gy_zp = io.lEin[1][q + V];
   }
-  VF<V> lhx = ldv<V>(d.lH[0] + q), lhy = ldv<V>(d.lH[1] + q), lhz = ldv<V>(d.lH[2] + q);
+  VF<V> lhx = ldv<V>(io.lH[0] + q), lhy = ldv<V>(io.lH[1] + q), lhz = ldv<V>(io.lH[2] + q);
 
   const bool xs = HX && P > 0 && in_slab(i, nx, P), xsp = HX && P > 0 && i + 1 < nx && in_slab(i + 1, nx, P);
   const bool ys = HY && P > 0 && in_slab(j, ny, P), ysp = HY && P > 0 && j + 1 < ny && in_slab(j + 1, ny, P);
@@ -862,9 +862,9 @@ __device__ __forceinline__ void gen_adj_e_body(const Dev& d, const int i, const 
       stv<V>(d.lpsiE[nb][2][0] + qx, n20);
     }
   }
-  stv<V>(d.lH[0] + q, lhx);
-  stv<V>(d.lH[1] + q, lhy);
-  stv<V>(d.lH[2] + q, lhz);
+  stv<V>(io.lHout[0] + q, lhx);
+  stv<V>(io.lHout[1] + q, lhy);
+  stv<V>(io.lHout[2] + q, lhz);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -885,16 +885,18 @@ __global__ void __launch_bounds__(32 * TY) k_gen_h(const __grid_constant__ Dev d
   FDTD_CLASS_DISPATCH(gen_h_body, d, i, j, k0, io)
 }
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_h(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb,
+                                                       const __grid_constant__ AdjIO io) {
   int b, i, j, k0;
   if (!box_decode<V>(B, b, i, j, k0)) return;
-  FDTD_CLASS_DISPATCH(gen_adj_h_body, d, i, j, k0, pb)
+  FDTD_CLASS_DISPATCH(gen_adj_h_body, d, i, j, k0, pb, io)
 }
 template <int V>
-__global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb) {
+__global__ void __launch_bounds__(32 * TY) k_gen_adj_e(const __grid_constant__ Dev d, const __grid_constant__ BoxList B, int pb,
+                                                       const __grid_constant__ AdjIO io) {
   int b, i, j, k0;
   if (!box_decode<V, SWEEP_FLIP>(B, b, i, j, k0)) return;
-  FDTD_CLASS_DISPATCH(gen_adj_e_body, d, i, j, k0, pb)
+  FDTD_CLASS_DISPATCH(gen_adj_e_body, d, i, j, k0, pb, io)
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -1078,10 +1080,12 @@ __global__ void __launch_bounds__(32 * TY, FDTD_ROW_MINB(WHICH)) k_row(const __g
     io_psi_inplace(io, d);
     if (WHICH == 0) gen_e_body<4, false, false>(d, i, j, k0, io);
     else gen_h_body<4, false, false>(d, i, j, k0, io);
-  } else if (WHICH == 2) {
-    gen_adj_h_body<4, false, false>(d, i, j, k0, pb);
   } else {
-    gen_adj_e_body<4, false, false>(d, i, j, k0, pb);
+    AdjIO io;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { io.lEin[c] = d.lE[c]; io.lH[c] = d.lH[c]; io.lEout[c] = d.lE[c]; io.lHout[c] = d.lH[c]; }
+    if (WHICH == 2) gen_adj_h_body<4, false, false>(d, i, j, k0, pb, io);
+    else gen_adj_e_body<4, false, false>(d, i, j, k0, pb, io);
   }
 }
 
