@@ -102,6 +102,8 @@ GROUP_KERNELS = {
     "fwd_fused": ["k_fused_fp", "k_fused_he"],
     "rev_fused": ["k_fused_ip", "k_fused_he"],
     "grad": ["k_grad("],
+    "adj_fused": ["k_fused_ap"],
+    "adj_fused_slabs": ["k_gen_adj_h", "k_gen_adj_e"],
     "fwd_fused_slabs": ["k_gen_h", "k_gen_e"],
 }
 
@@ -148,11 +150,11 @@ def ncu_import(args):
                  float(r[ci["gpu__time_duration.sum"]]) * tscale) for r in rows[2:] if "fdtd::" in r[ci["Kernel Name"]]]
     groups, detail, pos = {}, {}, 0
     present = " ".join(l[0] for l in launches)
-    for name in active_groups(None, "k_fused_fp" in present or "k_fused_he" in present, "k_fused_ip" in present):
+    for name in active_groups(None, "k_fused_fp" in present or "k_fused_he" in present, "k_fused_ip" in present, "k_fused_ap" in present):
         pref = GROUP_KERNELS[name]
         got = []
         while pos < len(launches) and any(launches[pos][0].replace("void ", "").replace("fdtd::", "").startswith(p) for p in pref) \
-                and len(got) < (2 if name not in ("inv_h", "inject_h", "inject_e", "fwd_fused", "rev_fused", "grad") else 1):
+                and len(got) < (2 if name not in ("inv_h", "inject_h", "inject_e", "fwd_fused", "rev_fused", "grad", "adj_fused") else 1):
             got.append(launches[pos])
             pos += 1
         if not got:
@@ -216,22 +218,23 @@ class ClockSampler:
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def active_groups(fdtd, fused, fused_rev):
+def active_groups(fdtd, fused, fused_rev, fused_adj=False):
     """Names of the kernel groups that the run launches (fdtd.Sim.KERNEL_IDS), in profiling order.  fwd_e / fwd_h stay in the list
     on the fused forward path too (its first and last half-step, and the two-kernel-equivalent figure)."""
     names = ["fwd_e", "fwd_h"]
     names += ["rev_fused", "grad"] if fused_rev else ["inv_h", "grad_inv_e"]
-    names += ["adj_h", "adj_e", "record", "inject_h", "inject_e"]
+    names += ["adj_fused", "adj_fused_slabs"] if fused_adj else ["adj_h", "adj_e"]
+    names += ["record", "inject_h", "inject_e"]
     if fused:
         names += ["fwd_fused", "fwd_fused_slabs"]
     return names
 
 
-def profile_kernels(sim, fdtd, w, flags, flush, reps, fused, fused_rev):
+def profile_kernels(sim, fdtd, w, flags, flush, reps, fused, fused_rev, fused_adj=False):
     """Each kernel group timed alone on the library's stream (fdtd_profile_kernel): {name: {us, algo_bytes}}.  Needs a completed
     forward run (record / inject and the z-face injection of the inverse kernels read the store)."""
     out = {}
-    for name in active_groups(fdtd, fused, fused_rev):
+    for name in active_groups(fdtd, fused, fused_rev, fused_adj):
         flush.fill_(1)
         ms, by = sim.profile_kernel(fdtd.Sim.KERNEL_IDS[name], warm=3 if reps > 1 else 0, reps=reps)
         out[name] = {"us": ms * 1e3, "algo_bytes": by}
@@ -264,10 +267,10 @@ def run_gpu(args, rank, world):
         import dataclasses
         w = dataclasses.replace(w, nsteps=min(w.nsteps, 64))
         sim.forward(w.nsteps, w.sources, w.store_dtype, w.k, flags=flags)
-        fused, fused_rev = sim.uses_fused(w.nsteps), sim.uses_fused_reverse()
+        fused, fused_rev, fused_adj = sim.uses_fused(w.nsteps), sim.uses_fused_reverse(), sim.uses_fused_adjoint()
         torch.cuda.synchronize()
         torch.cuda.profiler.start()
-        k = profile_kernels(sim, fdtd, w, flags, flush, 1, fused, fused_rev)
+        k = profile_kernels(sim, fdtd, w, flags, flush, 1, fused, fused_rev, fused_adj)
         torch.cuda.profiler.stop()
         print(json.dumps({"profile_only": True, "workload": args.workload, "kernels": k, "kernel_source_hash": kernel_source_hash()}))
         return
@@ -381,10 +384,12 @@ def run_gpu(args, rank, world):
     sim.forward(min(w.nsteps, 64), w.sources, w.store_dtype, w.k, flags=flags)
     fused = sim.uses_fused(w.nsteps)   # H half-step of step m and E half-step of step m+1 in one marching kernel
     fused_rev = sim.uses_fused_reverse()   # large grids: inverse-H and inverse-E of the reverse primal in one marching kernel
+    fused_adj = sim.uses_fused_adjoint()   # large grids: adjoint of H and adjoint of E in one marching kernel
     counts = {"fwd_e": 1 if fused else w.nsteps, "fwd_h": 1 if fused else w.nsteps, "inv_h": w.nsteps, "adj_h": w.nsteps,
               "grad_inv_e": w.nsteps, "adj_e": w.nsteps, "record": nrec + 1, "inject_h": w.nsteps, "inject_e": w.nsteps,
-              "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1, "rev_fused": w.nsteps, "grad": w.nsteps}
-    kernels = profile_kernels(sim, fdtd, w, flags, flush, 20, fused, fused_rev)
+              "fwd_fused": w.nsteps - 1, "fwd_fused_slabs": w.nsteps - 1, "rev_fused": w.nsteps, "grad": w.nsteps,
+              "adj_fused": w.nsteps, "adj_fused_slabs": w.nsteps}
+    kernels = profile_kernels(sim, fdtd, w, flags, flush, 20, fused, fused_rev, fused_adj)
     traffic, traffic_src = load_ncu_traffic(args.workload if not (args.store or args.k or args.tangential) else "-")
     tot = sum(v["us"] * counts[n] for n, v in kernels.items())
     for n, v in kernels.items():
@@ -417,7 +422,7 @@ def run_gpu(args, rank, world):
     # whole-pass effective bandwidth: algorithmic bytes of all stencil launches of one step / measured time
     fwd_names = ("fwd_e", "fwd_h", "fwd_fused", "fwd_fused_slabs")
     algo_fwd = sum(kernels[n]["algo_bytes"] * counts[n] for n in fwd_names if n in kernels) + kernels["record"]["algo_bytes"] * (nrec + 1)
-    rev_names = ("rev_fused", "grad", "inv_h", "grad_inv_e", "adj_h", "adj_e", "inject_h", "inject_e")
+    rev_names = ("rev_fused", "grad", "inv_h", "grad_inv_e", "adj_h", "adj_e", "adj_fused", "adj_fused_slabs", "inject_h", "inject_e")
     algo_rev = sum(kernels[n]["algo_bytes"] for n in rev_names if n in kernels) * w.nsteps
     fwd_gbs = algo_fwd / (f_ms / args.steps * 1e-3) / 1e9
     # the same forward time against the bytes of the two-kernel form (76 B per cell): comparable across paths
@@ -453,7 +458,7 @@ def run_gpu(args, rank, world):
         "store_bytes": store_bytes, "store_bytes_per_step": store_bytes / w.nsteps,
         "store_bytes_f32_k1": (w.nsteps + 1) * slot_vals * (3 if args.tangential else 1) * 4,   # all six components
         "effective_gbs": {"forward": fwd_gbs, "reverse": rev_gbs, "forward_frac_of_peak": fwd_gbs / peak,
-                          "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused), "reverse_fused": bool(fused_rev),
+                          "reverse_frac_of_peak": rev_gbs / peak, "forward_fused": bool(fused), "reverse_fused": bool(fused_rev), "adjoint_fused": bool(fused_adj),
                           "forward_two_kernel_equivalent": fwd2_gbs, "forward_two_kernel_equivalent_frac": fwd2_gbs / peak,
                           # also against the nominal HBM3e figure (8000 GB/s)
                           "forward_frac_of_nominal_8000": fwd_gbs / 8000.0, "reverse_frac_of_nominal_8000": rev_gbs / 8000.0,

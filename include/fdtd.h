@@ -154,7 +154,7 @@ fdtd_status fdtd_reset(fdtd_sim*);
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
 /* Fused marching kernels (two dependent half-steps per pass over the rows of the lean x-y range): mode -1
  * (default) = forward run fused where the marching kernel fills most of a wave of tiles (256x256x128 and larger), reverse primal
- * fused where it has several waves (512^3); 0 = never; 1 = forward AND reverse primal whenever the grid allows (nz % 4 == 0,
+ * and adjoint fused where it has several waves (512^3); 0 = never; 1 = forward, reverse primal and adjoint whenever the grid allows (nz % 4 == 0,
  * pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per block (0 = chosen by the library).  Results are bit-identical
  * in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being subtracted).
  * With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */
@@ -167,6 +167,8 @@ fdtd_status fdtd_set_rows(fdtd_sim*, int mode);
 int fdtd_uses_fused(const fdtd_sim*, int nsteps);
 /* 1 if fdtd_reverse would rebuild the primal with the fused marching kernel (inverse-H + inverse-E in one pass), else 0. */
 int fdtd_uses_fused_reverse(const fdtd_sim*);
+/* 1 if fdtd_reverse would also carry the adjoint fields with the adjoint marching kernel (adjoint of H + adjoint of E in one pass). */
+int fdtd_uses_fused_adjoint(const fdtd_sim*);
 
 /* Current fields: out_dev[6][nx][ny][nz].  fdtd_get_box: out_dev[ncomp][hi-lo] for the components in comp_mask. */
 fdtd_status fdtd_get_fields(fdtd_sim*, float* out_dev);

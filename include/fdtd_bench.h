@@ -17,7 +17,7 @@ extern "C" {
  * ids: 0 fwd_e, 1 fwd_h, 2 inv_h, 3 adj_h, 4 grad_inv_e, 5 adj_e, 6 record, 7 inject_h, 8 inject_e, 9 fused forward
  * marching kernel, 10 slab kernels of the fused forward path (FDTD_ERR_UNSUPPORTED where the grid cannot fuse); 11-14 the
  * lean / row kernel of split half-step id - 11 alone, 15-18 its general (slab-box) kernel alone; 19 the fused reverse marching
- * kernel (inverse-H + inverse-E), 20 the gradient kernel alone.  Ids 7 / 8 time inject as the active reverse path launches it.  Needs a reverse workspace for
+ * kernel (inverse-H + inverse-E), 20 the gradient kernel alone, 21 the adjoint marching kernel, 22 the slab kernels beside it.  Ids 7 / 8 time inject as the active reverse path launches it.  Needs a reverse workspace for
  * ids >= 2 and a completed forward run for ids 6-8 (its store stays readable through any sequence of these calls).  The field
  * contents are garbage afterwards: call fdtd_reset.
  * Synchronises.  algo_bytes (may be NULL) receives the algorithmic bytes one launch moves. */

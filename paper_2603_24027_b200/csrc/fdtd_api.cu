@@ -1045,7 +1045,9 @@ bool use_fused_reverse(const fdtd_sim* s) {
 bool use_fused_adjoint(const fdtd_sim* s) {
   if (s->fuse_adj_mode == 0 || !use_fused_reverse(s) || !s->fuse_za || !s->lb[1][0]) return false;
   if (s->fuse_adj_mode >= 1) return true;
-  return false;   // auto: off until measured
+  // auto: with the fused primal, where the marching kernels have several waves of tiles.  Measured on B200 (round 2): C4 reverse
+  // 2925 -> 2638 us per step (10.9 -> 7.6 GB of adjoint traffic per step); C3 (196 tiles) 223 vs 221: left on the row kernels.
+  return fused_tiles(s, 32) >= 4 * 2 * 148;
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
@@ -1475,6 +1477,7 @@ fdtd_status fdtd_set_rows(fdtd_sim* s, int mode) {
   return FDTD_OK;
 }
 
+int fdtd_uses_fused_adjoint(const fdtd_sim* s) { return (s && s->ws && use_fused_adjoint(s)) ? 1 : 0; }
 int fdtd_uses_fused_reverse(const fdtd_sim* s) { return (s && s->ws && use_fused_reverse(s)) ? 1 : 0; }
 int fdtd_uses_fused(const fdtd_sim* s, int nsteps) { return (s && s->ws && use_fused(s, nsteps)) ? 1 : 0; }
 
@@ -1709,10 +1712,11 @@ fdtd_status fdtd_codec_encode_slices_noalloc(fdtd_dtype dt, const float* x_dev, 
 }
 
 fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double* ms_out, double* bytes_out) {
-  if (!s || id < 0 || id > 20 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
+  if (!s || id < 0 || id > 22 || reps < 1 || warm < 0 || !ms_out) return FDTD_ERR_INVALID_ARG;
   if (!s->ws) return fail(s, FDTD_ERR_OOM, "no workspace");
   if (id >= 2 && !(s->flags & FDTD_WS_REVERSE)) return fail(s, FDTD_ERR_STATE, "needs a reverse workspace");
   if (((id >= 6 && id <= 8) || id == 2 || id == 4) && !s->forward_done) return fail(s, FDTD_ERR_STATE, "needs a completed forward run");
+  if ((id == 21 || id == 22) && !(s->fuse_za && s->lb[1][0])) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused adjoint path does not apply to this grid");
   if ((id == 9 || id == 10 || id == 19) && !s->can_fuse) return fail(s, FDTD_ERR_UNSUPPORTED, "the fused path needs nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4");
   s->cur = s->stream;
   const int mrev = std::min(s->nsteps, s->nsteps / 2 + 2);   // nstate = mrev-1 falls between two slots
@@ -1749,6 +1753,13 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
         else launch_inject(s, mrev, nullptr, id == 7 ? 1 : 0, 0);
         break;
       case 20: launch_grad(s); break;
+      case 21: launch_fused_adj(s, s->acb, s->acb ^ 1, 0); break;   // adjoint marching kernel, alone
+      case 22: {   // slab kernels of the fused adjoint path: adjoint of H, then adjoint of E on their boxes
+        const AdjIO ia = adj_io(s, s->acb, s->acb ^ 1, false), ib = adj_io(s, s->acb, s->acb ^ 1, true);
+        launch_gen(s, 2, 0, s->split[6], nullptr, &ia);
+        launch_gen(s, 3, 0, s->split[7], nullptr, &ib);
+        break;
+      }
       case 9: launch_fused(s, false, s->cb, s->cb ^ 1); break;
       case 19: launch_fused(s, true, s->cb, s->cb ^ 1); break;   // reverse marching kernel (inverse-H + inverse-E), alone
       case 11: case 12: case 13: case 14: launch_lean(s, id - 11); break;     // lean kernel of split half-step id - 11, alone
@@ -1808,6 +1819,21 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
       case 6: v = (double)s->st.slot_values * 4 + (double)slot_bytes_host(s, s->dtype); break;   // f32 gathered, slot written (block scales included)
       case 7: case 8: v = (s->store_mode == 1 ? 1.0 : 3.0) * shell * (2 * eb + 4); break;   // two slots read, one f32 written per component
       case 20: v = 40 * dcells; break;   // lE (12) + f64 accumulator rw (16) + H of the design cells (12)
+      case 21: {   // adjoint marching kernel: lambda_E, lambda_H read and written once, ce read; lambda_psi of the z axis rw
+        const double rows = (double)std::max(0, s->n[0] - 2 * s->P - 2) * std::max(0, s->n[1] - 2 * s->P - 2);
+        v = 52 * rows * s->n[2] + 32 * rows * 2 * s->P;
+        break;
+      }
+      case 22: {   // its slab kernels: 36 B on the adjoint-of-H boxes, 40 B on the adjoint-of-E boxes, lambda_psi of the boxes' cells
+        double in6 = 1, in7 = 1;
+        for (int a = 0; a < 3; ++a) {
+          in6 *= std::max(0, s->split[6].reg.hi[a] - s->split[6].reg.lo[a]);
+          in7 *= std::max(0, s->split[7].reg.hi[a] - s->split[7].reg.lo[a]);
+        }
+        const double rows = (double)std::max(0, s->n[0] - 2 * s->P - 2) * std::max(0, s->n[1] - 2 * s->P - 2);
+        v = 36 * (N - in6) + 40 * (N - in7) + 32 * (slab - rows * 2 * s->P);
+        break;
+      }
       case 19: {  // reverse marching kernel: 52 B per inner-interior cell
         v = 52 * Ninner;
         break;
@@ -1840,7 +1866,9 @@ fdtd_status fdtd_profile_kernel(fdtd_sim* s, int id, int warm, int reps, double*
           in5 *= std::max(0, s->split[5].reg.hi[a] - s->split[5].reg.lo[a]);
           in4 *= std::max(0, s->split[4].reg.hi[a] - s->split[4].reg.lo[a]);
         }
-        v = 36 * (N - in5) + 40 * (N - in4) + 32 * slab;
+        // psi of the boxes' cells only: the z-slab cells of the marching kernel's rows are counted with that kernel (id 9)
+        const double zrows = s->fuse_z ? (double)std::max(0, s->n[0] - 2 * s->P - 1) * std::max(0, s->n[1] - 2 * s->P - 1) : 0.0;
+        v = 36 * (N - in5) + 40 * (N - in4) + 32 * (slab - zrows * 2 * s->P);
       }
     }
     *bytes_out = v;

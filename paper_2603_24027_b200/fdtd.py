@@ -72,6 +72,7 @@ def lib():
     L.fdtd_set_fused.argtypes = [vp, C.c_int, C.c_int]
     L.fdtd_uses_fused.argtypes = [vp, C.c_int]
     L.fdtd_uses_fused_reverse.argtypes = [vp]
+    L.fdtd_uses_fused_adjoint.argtypes = [vp]
     L.fdtd_set_rows.argtypes = [vp, C.c_int]
     L.fdtd_set_store_mode.argtypes = [vp, C.c_int]
     L.fdtd_get_fields.argtypes = [vp, vp]
@@ -106,7 +107,7 @@ def lib():
 
 EXPORTED = ["fdtd_create", "fdtd_forward", "fdtd_reverse", "fdtd_store_bytes", "fdtd_set_cpml", "fdtd_set_design",
             "fdtd_set_monitor", "fdtd_workspace_bytes", "fdtd_set_workspace", "fdtd_set_eps", "fdtd_reset",
-            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_set_rows", "fdtd_uses_fused", "fdtd_uses_fused_reverse", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
+            "fdtd_set_graphs", "fdtd_set_fused", "fdtd_set_rows", "fdtd_uses_fused", "fdtd_uses_fused_reverse", "fdtd_uses_fused_adjoint", "fdtd_set_store_mode", "fdtd_get_fields", "fdtd_get_box", "fdtd_get_adjoint", "fdtd_num_slots",
             "fdtd_slot_values", "fdtd_slot_ptr", "fdtd_slot_bytes", "fdtd_set_eps_host", "fdtd_forward_host", "fdtd_reverse_host",
             "fdtd_codec_encode", "fdtd_codec_fetch", "fdtd_codec_encode_slices_noalloc", "fdtd_noalloc_last_error", "fdtd_profile_kernel", "fdtd_sync", "fdtd_last_error", "fdtd_destroy",
             "fdtd_launch_count", "fdtd_debug_guard_check"]
@@ -321,6 +322,9 @@ class Sim:
     def uses_fused_reverse(self):
         return bool(self._L.fdtd_uses_fused_reverse(self._h))
 
+    def uses_fused_adjoint(self):
+        return bool(self._L.fdtd_uses_fused_adjoint(self._h))
+
     def fields(self):
         self._same_stream()
         out = self._torch.empty((6,) + self.shape, dtype=self._torch.float32, device=self.eps.device)
@@ -368,7 +372,7 @@ class Sim:
     KERNELS = ["fwd_e", "fwd_h", "inv_h", "adj_h", "grad_inv_e", "adj_e", "record", "inject_h", "inject_e",
                "fwd_fused", "fwd_fused_slabs"]   # the last two: the fused forward path (fdtd_fused.cuh), large grids only
     # kernel groups of fdtd_profile_kernel by name; rev_fused / grad: the fused reverse primal (large grids) and the gradient kernel
-    KERNEL_IDS = {**{n: i for i, n in enumerate(KERNELS)}, "rev_fused": 19, "grad": 20}
+    KERNEL_IDS = {**{n: i for i, n in enumerate(KERNELS)}, "rev_fused": 19, "grad": 20, "adj_fused": 21, "adj_fused_slabs": 22}
 
     def profile_kernel(self, kernel_id, warm=5, reps=50):
         """(mean ms per launch, algorithmic bytes per launch) of one kernel timed alone, back to back (fdtd_profile_kernel)."""
