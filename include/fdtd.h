@@ -153,9 +153,10 @@ fdtd_status fdtd_reset(fdtd_sim*);
 /* Replay runs of k steps through CUDA graphs (default 1 = on). */
 fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
 /* Fused marching kernels (two dependent half-steps per pass over the rows of the lean x-y range): mode -1
- * (default) = forward run fused where the marching kernel fills most of a wave of tiles (256x256x128 and larger), reverse primal
- * and adjoint fused where it has several waves (512^3); 0 = never; 1 = forward, reverse primal and adjoint whenever the grid allows (nz % 4 == 0,
- * pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per block (0 = chosen by the library).  Results are bit-identical
+ * (default) = forward run, reverse primal and adjoint fused where the marching kernels have at least one block per multiprocessor
+ * (256x256x128 and larger; 128^3 lives in L2 and keeps the split kernels); 0 = never; 1 = forward, reverse primal and adjoint
+ * whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per block (0 = chosen by the
+ * library: 16 or 32 in the forward run; in the reverse run the count in [16, 64] with the fewest waves x (planes + 1)).  Results are bit-identical
  * in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being subtracted).
  * With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */
 fdtd_status fdtd_set_fused(fdtd_sim*, int mode, int xseg);

@@ -101,6 +101,8 @@ struct fdtd_sim {
   int fuse_mode = -1;      // -1 auto (by size), 0 never, 1 whenever possible
   int fuse_rev_mode = -1;  // the same for the reverse primal (inverse-H + inverse-E)
   int xseg = 0;            // planes per block of the fused marching kernels (0: chosen by fused_xseg)
+  int xseg_rev = 0;        // ... of the reverse-run marching kernels (primal and adjoint), if it is to differ
+  int sm_count = 148;      // multiprocessors of the device (fdtd_create)
   bool rows_auto = true;   // what fdtd_set_rows(-1) selects (by grid size, see fdtd_create)
   bool use_iz = true;      // fused reverse primal: k_fused_ip instead of k_fused_he<true>
   bool use_fz = true;      // fused forward path: whole-row marching kernel (k_fused_fp) instead of k_fused_he + class-Z slab boxes
@@ -695,8 +697,24 @@ long long fused_tiles(const fdtd_sim* s, int xseg) {
 // planes a block of the marching kernels walks.  Whole-row kernel (two blocks per SM): 32 where that leaves at least one tile per
 // SM, else 16.  Measured on B200 (round 2, k_fused_fp): C4 forward per 400 steps at 32 / 40 / 48 planes 548.4 / 548.5 / 551.0 ms;
 // C3 per 2000 steps at 16 / 20 / 24 / 28 / 32 planes 223.2 / 225.7 / 217.2 / 208.5 / 208.6 ms (196 tiles at 32).
-int fused_xseg(const fdtd_sim* s) {
+// planes per block of the reverse-run marching kernels (primal and adjoint; they run one after the other on one branch, two
+// blocks per SM): the count that minimises waves x (planes + 1) — whole waves of tiles, little priming overhead.  Measured on
+// B200 (round 2): C3 reverse per 2000 steps at 20 / 22 / 24 / 26 / 28 / 32 planes 495.8 / 408.0 / 407.8 / 414.9 / 420.3 / 443.4 ms
+// (24: 280 tiles for 296 slots); C4 per 400 steps at 24 / 32 / 40 planes 1047.9 / 1055.0 / 1046.4 ms.
+int fused_xseg_rev_auto(const fdtd_sim* s) {
+  const long long slots = 2LL * std::max(1, s->sm_count);
+  int best = 32;
+  long long best_cost = -1;
+  for (int x = 16; x <= 64; ++x) {
+    const long long t = fused_tiles(s, x), cost = (t + slots - 1) / slots * (x + 1);
+    if (best_cost < 0 || cost < best_cost || (cost == best_cost && x > best)) { best = x; best_cost = cost; }
+  }
+  return best;
+}
+int fused_xseg(const fdtd_sim* s, bool rev = false) {
+  if (rev && s->xseg_rev > 0) return s->xseg_rev;
   if (s->xseg > 0) return s->xseg;
+  if (rev && s->fuse_z) return fused_xseg_rev_auto(s);
   if (s->fuse_z) return fused_tiles(s, 32) >= 148 ? 32 : 16;
   return fused_tiles(s, 32) >= 4 * 3 * 148 ? 32 : 16;
 }
@@ -712,7 +730,7 @@ void launch_fused(fdtd_sim* s, bool inv, int from, int to) {
   // per plane beside its 6 vector stores
   if (!inv) a.lo[2] = (a.lo[2] + 3) / 4 * 4;
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1] || a.hi[2] <= a.lo[2]) return;
-  a.xseg = fused_xseg(s);
+  a.xseg = fused_xseg(s, inv);
   if (inv && s->use_iz && s->n[2] - 2 * s->P >= 8) {   // reverse twin in the structure of the whole-row kernel (k_fused_ip)
     FusedIArgs z;
     for (int c = 0; c < 3; ++c) { z.Ein[c] = a.Ein[c]; z.Hin[c] = a.Hin[c]; z.Eout[c] = a.Eout[c]; z.Hout[c] = a.Hout[c]; }
@@ -892,7 +910,7 @@ void launch_fused_adj(fdtd_sim* s, int from, int to, int pb) {
   a.pE_out[0] = s->d.lpsiE[nb][0][1]; a.pE_out[1] = s->d.lpsiE[nb][1][0];
   for (int ax = 0; ax < 2; ++ax) { a.lo[ax] = s->P + 1; a.hi[ax] = s->n[ax] - s->P - 1; }
   if (a.hi[0] <= a.lo[0] || a.hi[1] <= a.lo[1]) return;
-  a.xseg = fused_xseg(s);
+  a.xseg = fused_xseg(s, true);
   const dim3 g((unsigned)((s->n[2] / 4 + 31) / 32), (unsigned)((a.hi[1] - a.lo[1] + FUSED_TR - 1) / FUSED_TR),
                (unsigned)((a.hi[0] - a.lo[0] + a.xseg - 1) / a.xseg));
   k_fused_ap<<<g, dim3(32, FUSED_TR + 1), sizeof(FusedASmem), s->cur>>>(s->d, a);
@@ -1032,22 +1050,24 @@ bool use_fused(const fdtd_sim* s, int nsteps) {
   if (!s->fuse_z) return fused_tiles(s, fused_xseg(s)) >= 4 * 3 * 148;
   return fused_tiles(s, 16) >= 2 * 148;
 }
+bool fused_adjoint_possible(const fdtd_sim* s) { return s->fuse_adj_mode != 0 && s->fuse_za && s->lb[1][0] != nullptr; }
 bool use_fused_reverse(const fdtd_sim* s) {
   if (s->fuse_rev_mode == 0 || !s->can_fuse) return false;
   if (s->fuse_rev_mode >= 1) return true;
-  // mode -1 (auto): where the whole-row structure applies and the marching kernel has several waves of tiles (two blocks per SM).
-  // Bit-identical to the two-kernel reverse primal; 3.1 GB fewer bytes per step on C4.  Measured on B200: round 1 (k_fused_he<true>,
-  // 1.23 ms per launch) 3406 vs 3395 us per step on C4: off; round 2 with direct loads (1.20 ms) 3148 vs 3094: off; round 2 with
-  // the cp.async-pipelined kernel (k_fused_ip, 0.98 ms against 0.63 + 0.67 ms for the two inverse kernels): C4 2924 vs 3090 us per
-  // step: on; C3 (196 tiles) 234.8 vs 223.7: off.
-  return s->use_iz && s->n[2] - 2 * s->P >= 8 && fused_tiles(s, 32) >= 4 * 2 * 148;
+  if (!(s->use_iz && s->n[2] - 2 * s->P >= 8)) return false;
+  // mode -1 (auto).  Bit-identical to the two-kernel reverse primal; 3.1 GB fewer bytes per step on C4.  History of the primal
+  // alone on C4: round 1 (k_fused_he<true>, 1.23 ms per launch) 3406 vs 3395 us per step: off; round 2 with direct loads (1.20 ms)
+  // 3148 vs 3094: off; with the cp.async-pipelined kernel (k_fused_ip, 0.98 ms against 0.63 + 0.67 ms for the two inverse kernels)
+  // 2924 vs 3090: on; C3 (196 tiles) 234.8 vs 223.7: off.  TOGETHER with the adjoint marching kernel (fully fused reverse step) it
+  // pays from one block per SM upwards: C3 at 24 planes per block 203.9 vs 226.4 us per step, C4 2616 vs 3090; C2 (lives in L2,
+  // 65 tiles) stays on the split kernels.
+  if (fused_adjoint_possible(s)) return fused_tiles(s, fused_xseg(s, true)) >= std::max(1, s->sm_count);
+  return fused_tiles(s, 32) >= 4 * 2 * 148;
 }
 bool use_fused_adjoint(const fdtd_sim* s) {
-  if (s->fuse_adj_mode == 0 || !use_fused_reverse(s) || !s->fuse_za || !s->lb[1][0]) return false;
+  if (!fused_adjoint_possible(s) || !use_fused_reverse(s)) return false;
   if (s->fuse_adj_mode >= 1) return true;
-  // auto: with the fused primal, where the marching kernels have several waves of tiles.  Measured on B200 (round 2): C4 reverse
-  // 2925 -> 2638 us per step (10.9 -> 7.6 GB of adjoint traffic per step); C3 (196 tiles) 223 vs 221: left on the row kernels.
-  return fused_tiles(s, 32) >= 4 * 2 * 148;
+  return fused_tiles(s, fused_xseg(s, true)) >= std::max(1, s->sm_count);
 }
 fdtd_status forward_fused(fdtd_sim* s, int nsteps, int k) {
   // state 0 is recorded whole, then step 1's E half-step runs alone (in place)
@@ -1239,6 +1259,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
     int dev = 0, l2 = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    { int sms = 0; if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) s->sm_count = sms; }
     cudaGetLastError();
     const double fwd_bytes = 7.0 * 4.0 * (double)nx * ny * nz;
     s->zalign = (l2 > 0 && fwd_bytes > 1.5 * (double)l2) ? 32 : 16;
@@ -1262,6 +1283,7 @@ fdtd_status fdtd_create(fdtd_sim** out, int nx, int ny, int nz, double dx, doubl
   if (const char* e = std::getenv("FDTD_FUSE_ADJ")) { const int v = atoi(e); if (v >= -1 && v <= 1) s->fuse_adj_mode = v; }
   if (const char* e = std::getenv("FDTD_FA_DEBUG")) s->fa_debug = atoi(e) != 0;
   if (const char* e = std::getenv("FDTD_XSEG")) { const int v = atoi(e); if (v >= 1) s->xseg = v; }
+  if (const char* e = std::getenv("FDTD_XSEG_REV")) { const int v = atoi(e); if (v >= 1) s->xseg_rev = v; }
   bool ok = cudaEventCreateWithFlags(&s->ev_fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&s->ev_mid, cudaEventDisableTiming) == cudaSuccess;
   for (int b = 0; b < 4 && ok; ++b)

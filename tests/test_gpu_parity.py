@@ -511,6 +511,7 @@ def test_c2_shaped_short_run_sampled_parity():
     o = oracle_gradient(w, 32, w.store_dtype, w.k)
     g = gpu_gradient(w, w.store_dtype, w.k)
     f_err, g_err = _report("C2-shaped 120 steps", g, o)
+    assert not g["sim"].uses_fused(w.nsteps) and not g["sim"].uses_fused_reverse()      # lives in L2: split kernels
     assert np.abs(o["grad"]).max() > 0 and np.abs(g["grad"]).max() > 0
     for sl in (np.s_[:, 64], np.s_[:, :, 40], np.s_[:, :, :, 63]):
         assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
@@ -526,6 +527,7 @@ def test_c3_shaped_short_run_sampled_parity():
     o = oracle_gradient(w, 32, w.store_dtype, w.k)
     g = gpu_gradient(w, w.store_dtype, w.k)
     f_err, g_err = _report("C3-shaped 40 steps", g, o)
+    assert g["sim"].uses_fused(w.nsteps) and g["sim"].uses_fused_reverse() and g["sim"].uses_fused_adjoint()
     assert np.abs(o["grad"]).max() > 0
     for sl in (np.s_[:, 27], np.s_[:, :, 128], np.s_[:, :, :, 63]):
         assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
@@ -612,11 +614,13 @@ def test_c2_sized_cubic_interpolation_parity():
 
 def test_c3_500_steps_parity():
     """BASELINE.json configs[2] as bench.py --workload C3 runs it (256x256x128, P = 16, float16, k = 8, pulse-shape loss),
-    truncated to T = 500; row kernels are the launch configuration the library picks on this grid."""
+    truncated to T = 500; the marching kernels (forward, reverse primal, adjoint) beside the slab kernels are
+    the launch configuration the library picks on this grid."""
     w = W.c3(nsteps=500)
     o = oracle_gradient(w, 32, w.store_dtype, w.k)
     g = gpu_gradient(w, w.store_dtype, w.k)
     f_err, g_err = _report("C3, 500 steps", g, o)
+    assert g["sim"].uses_fused(w.nsteps) and g["sim"].uses_fused_reverse() and g["sim"].uses_fused_adjoint()
     assert np.abs(o["grad"]).max() > 0 and np.abs(g["grad"]).max() > 0
     assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
     for sl in (np.s_[:, 27], np.s_[:, :, 128], np.s_[:, :, :, 63], np.s_[:, :, :, 8]):
@@ -632,7 +636,8 @@ def test_c3_500_steps_parity():
 
 def test_c4_512_cubed_20_steps_parity():
     """BASELINE.json configs[3] on the full 512^3 grid in the launch configuration bench.py times (fused forward marching
-    kernel beside the slab kernels, row kernels in the reverse run; bf16, k = 4), T = 20.  Design box and
+    kernel beside the slab kernels, reverse primal and adjoint marching kernels in the reverse run; bf16, k = 4), T = 20
+    (SURVEY 8(d)).  Design box and
     monitor plane are moved next to the dipole plane (k = 48) so that 20 steps give a non-zero gradient.  Fields on the whole
     grid and on sampled planes, whole design-box gradient, every slot byte for byte."""
     w = W.c4(nsteps=20)
@@ -643,6 +648,7 @@ def test_c4_512_cubed_20_steps_parity():
     g = gpu_gradient(w, w.store_dtype, w.k, sim=s)
     o = oracle_gradient(w, 32, w.store_dtype, w.k)
     f_err, g_err = _report("C4 512^3, 20 steps", g, o)
+    assert s.uses_fused_reverse() and s.uses_fused_adjoint()
     assert np.abs(o["grad"]).max() > 0 and np.abs(g["grad"]).max() > 0
     for sl in (np.s_[:, 200], np.s_[:, :, 17], np.s_[:, :, :, 48], np.s_[:, :, :, 3], np.s_[:, :, :, 500]):
         assert rel_l2(g["final"][sl], o["final"][sl]) <= FIELD_TOL
