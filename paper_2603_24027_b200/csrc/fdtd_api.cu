@@ -694,13 +694,11 @@ long long fused_tiles(const fdtd_sim* s, int xseg) {
   tiles *= (s->n[0] - 2 * s->P + xseg - 1) / xseg;
   return tiles;
 }
-// planes a block of the marching kernels walks.  Whole-row kernel (two blocks per SM): 32 where that leaves at least one tile per
-// SM, else 16.  Measured on B200 (round 2, k_fused_fp): C4 forward per 400 steps at 32 / 40 / 48 planes 548.4 / 548.5 / 551.0 ms;
-// C3 per 2000 steps at 16 / 20 / 24 / 28 / 32 planes 223.2 / 225.7 / 217.2 / 208.5 / 208.6 ms (196 tiles at 32).
 // planes per block of the reverse-run marching kernels (primal and adjoint; they run one after the other on one branch, two
 // blocks per SM): the count that minimises waves x (planes + 1) — whole waves of tiles, little priming overhead.  Measured on
 // B200 (round 2): C3 reverse per 2000 steps at 20 / 22 / 24 / 26 / 28 / 32 planes 495.8 / 408.0 / 407.8 / 414.9 / 420.3 / 443.4 ms
-// (24: 280 tiles for 296 slots); C4 per 400 steps at 24 / 32 / 40 planes 1047.9 / 1055.0 / 1046.4 ms.
+// (10 segments x 28 = 280 tiles for 296 slots; the rule takes 23 there: the same 10 segments, one plane step fewer); C4 per 400
+// steps at 24 / 32 / 40 planes 1047.9 / 1055.0 / 1046.4 ms (the rule takes 30: 3840 tiles, 13 waves; 1053 ms).
 int fused_xseg_rev_auto(const fdtd_sim* s) {
   const long long slots = 2LL * std::max(1, s->sm_count);
   int best = 32;
@@ -711,6 +709,9 @@ int fused_xseg_rev_auto(const fdtd_sim* s) {
   }
   return best;
 }
+// planes a block of the marching kernels walks.  Whole-row kernel (two blocks per SM): 32 where that leaves at least one tile per
+// SM, else 16.  Measured on B200 (round 2, k_fused_fp): C4 forward per 400 steps at 32 / 40 / 48 planes 548.4 / 548.5 / 551.0 ms;
+// C3 per 2000 steps at 16 / 20 / 24 / 28 / 32 planes 223.2 / 225.7 / 217.2 / 208.5 / 208.6 ms (196 tiles at 32).
 int fused_xseg(const fdtd_sim* s, bool rev = false) {
   if (rev && s->xseg_rev > 0) return s->xseg_rev;
   if (s->xseg > 0) return s->xseg;
