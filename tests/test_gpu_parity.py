@@ -400,6 +400,40 @@ def test_fused_adjoint_marching_kernel_matches_two_kernel_path(which, xseg, grap
     assert np.array_equal(res[0]["state0"][interior], res[1]["state0"][interior])
 
 
+def test_default_launch_configuration_on_a_ragged_mid_size_grid():
+    """A non-cubic grid on which the library picks the three marching kernels BY ITSELF (mode -1) and nothing divides evenly:
+    176x200x144, P = 12: two z tiles (32 + 4 groups), 22 y tiles, 152 planes cut into 5 forward and 6 reverse segments (the
+    reverse kernels take their own planes-per-block count).  Against the split kernels bit for bit (fields, monitor record,
+    gradient, adjoint fields, reconstructed interior) and against the oracle; design box across the z tile boundary and onto the
+    shell, one source on the shell corner."""
+    rng = np.random.default_rng(77)
+    shape, P, T = (176, 200, 144), 12, 14
+    eps = rng.uniform(1.0, 12.25, shape).astype(np.float32)
+    wave = W.gauss_sine(T, 6, 2)
+    srcs = [W.Source(1, (80, 90, 118), (84, 93, 131), None, wave), W.Source(2, (P, P, P), (P + 1, P + 1, P + 2), None, wave),
+            W.Source(0, (150, 170, 60), (152, 171, 64), None, wave)]
+    design = ((70, 84, 112), (96, 100, shape[2] - P))
+    mon = ((88, 80, 110), (89, 104, shape[2] - P), 0b110110)
+    w = W.Workload("ragged-mid", shape, P, T, eps, design, srcs, mon, "flux_x", W.BF16, 4)
+    o = oracle_gradient(w, 32, w.store_dtype, w.k)
+    res = {}
+    for mode in (0, -1):
+        s = gpu_sim(w)
+        s.set_fused(mode, 0)
+        s.set_workspace(w.nsteps, w.store_dtype, w.k)
+        auto = mode == -1
+        assert s.uses_fused(w.nsteps) == auto and s.uses_fused_reverse() == auto and s.uses_fused_adjoint() == auto
+        res[mode] = gpu_gradient(w, w.store_dtype, w.k, sim=s)
+        res[mode]["adj"] = s.adjoint().cpu().numpy()
+    f_err, g_err = _report("ragged mid-size grid, default launch configuration", res[-1], o)
+    assert np.abs(o["grad"]).max() > 0
+    assert f_err <= FIELD_TOL and g_err <= GRAD_TOL
+    interior = (slice(None),) + tuple(slice(P, n - P) for n in shape)
+    for key in ("final", "mon", "grad", "adj"):
+        assert np.array_equal(res[0][key], res[-1][key]), key
+    assert np.array_equal(res[0]["state0"][interior], res[-1]["state0"][interior])
+
+
 def _inner_design(w):
     P = w.pml
     return dataclasses.replace(w, design=(tuple([P + 1] * 3), tuple(n - P - 1 for n in w.shape)))
