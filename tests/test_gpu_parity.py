@@ -434,6 +434,69 @@ def test_default_launch_configuration_on_a_ragged_mid_size_grid():
     assert np.array_equal(res[0]["state0"][interior], res[-1]["state0"][interior])
 
 
+def _random_workload(seed, big):
+    """Random grid for the differential test below: CPML width 4..16, nz on and next to the 128-cell tile boundaries or anywhere,
+    1-3 random sources plus one on the shell corner, design box around the first source, monitor plane behind it."""
+    rng = np.random.default_rng(seed)
+    P = int(rng.choice([4, 8, 12, 16]))
+    nz = max(int(rng.choice([4 * int(rng.integers((2 * P + 12) // 4, 110)), 128, 132, 256, 260, 384, 388])), 2 * P + 12)
+    nx = int(rng.integers(2 * P + 6, 200 if big else 80))
+    ny = int(rng.integers(2 * P + 6, 220 if big else 90))
+    while nx * ny * nz > 9_000_000:
+        nx, ny = max(2 * P + 6, nx * 3 // 4), max(2 * P + 6, ny * 3 // 4)
+    shape = (nx, ny, nz)
+    T = int(rng.integers(5, 22))
+    k = int(rng.choice([1, 2, 3, 4, 8]))
+    dtype = int(rng.choice([W.F32, W.F16, W.BF16, W.F8E4M3_SCALED, W.F8E4M3_MX32, W.F8E4M3B11FNUZ]))
+    eps = rng.uniform(1.0, 12.25, shape).astype(np.float32)
+    wave = W.gauss_sine(T, max(2, T // 3), 2)
+
+    def box(minw, maxw):
+        lo = []
+        hi = []
+        for a in range(3):
+            width = int(rng.integers(minw, min(maxw, shape[a] - 2 * P) + 1))
+            lo.append(int(rng.integers(P, shape[a] - P - width + 1)))
+            hi.append(lo[-1] + width)
+        return tuple(lo), tuple(hi)
+    srcs = [W.Source(int(rng.integers(0, 3)), *box(1, 6), None, wave) for _ in range(int(rng.integers(1, 4)))]
+    srcs.append(W.Source(2, (P, P, P), (P + 1, P + 1, P + 2), None, wave))
+    dlo, dhi = box(2, 40)
+    dlo = tuple(max(P, min(dlo[a], srcs[0].lo[a] - 1)) for a in range(3))
+    dhi = tuple(min(shape[a] - P, max(dhi[a], srcs[0].hi[a] + 2)) for a in range(3))
+    mx = min(shape[0] - P - 1, srcs[0].hi[0] + 2)
+    mon = ((mx, P, P), (mx + 1, shape[1] - P, shape[2] - P), 0b110110)
+    return W.Workload(f"random{seed}", shape, P, T, eps, (dlo, dhi), srcs, mon, "flux_x", dtype, k), rng
+
+
+@pytest.mark.parametrize("seed,big", [(s, False) for s in range(1000, 1012)] + [(s, True) for s in range(5000, 5012)])
+def test_marching_kernels_match_split_kernels_on_random_grids(seed, big):
+    """Differential test of the three marching kernels (forced on with a random planes-per-block count, and as the library picks
+    them) against the split kernels, which the other tests tie to the oracle: final fields, monitor record, gradient, adjoint
+    fields and the reconstructed interior bit for bit.  Grid shape, CPML width, run length, store dtype, k, interpolation, graphs
+    on / off are drawn from the seed (420 such cases were run once without a mismatch; these 24 stay)."""
+    w, rng = _random_workload(seed, big)
+    interp = int(rng.choice([W.LINEAR, W.CUBIC]))
+    graphs = bool(rng.integers(0, 2))
+    xseg = int(rng.choice([0, 0, 3, 5, 8, 13, 24]))
+    res = {}
+    for mode in (0, 1, -1):
+        s = gpu_sim(w)
+        s.set_fused(mode, xseg if mode == 1 else 0)
+        s.set_graphs(graphs)
+        res[mode] = gpu_gradient(w, w.store_dtype, w.k, interp=interp, sim=s)
+        res[mode]["adj"] = s.adjoint().cpu().numpy()
+        if mode == 1:
+            assert s.uses_fused(w.nsteps) and s.uses_fused_reverse()
+        del res[mode]["sim"], s
+    assert np.isfinite(res[0]["grad"]).all()
+    interior = (slice(None),) + tuple(slice(w.pml, n - w.pml) for n in w.shape)
+    for mode in (1, -1):
+        for key in ("final", "mon", "grad", "adj"):
+            assert np.array_equal(res[0][key], res[mode][key]), (mode, key, w.shape, w.pml)
+        assert np.array_equal(res[0]["state0"][interior], res[mode]["state0"][interior]), (mode, w.shape, w.pml)
+
+
 def _inner_design(w):
     P = w.pml
     return dataclasses.replace(w, design=(tuple([P + 1] * 3), tuple(n - P - 1 for n in w.shape)))
