@@ -58,7 +58,8 @@ typedef enum {
 /* Temporal interpolation between stored steps: linear is the paper's; cubic = 4-point Lagrange. */
 typedef enum { FDTD_LINEAR = 0, FDTD_CUBIC = 1 } fdtd_interp;
 
-/* Additive soft source: in step m (1-based) E_comp += amp * wave[m-1] on the box (R8). */
+/* Additive soft source: in step m (1-based) E_comp += amp * wave[m-1] on the box (R8).  Sources of one component whose
+ * boxes overlap are added in index order (one launch per source instead of one for all), so the sum is the same on every run. */
 typedef struct {
   int comp;          /* 0..2 = Ex,Ey,Ez */
   int lo[3], hi[3];  /* cell box inside the interior */
@@ -155,7 +156,7 @@ fdtd_status fdtd_set_graphs(fdtd_sim*, int enabled);
 /* Fused marching kernels (two dependent half-steps per pass over the rows of the lean x-y range): mode -1
  * (default) = forward run, reverse primal and adjoint fused where the marching kernels have at least one block per multiprocessor
  * (256x256x128 and larger; 128^3 lives in L2 and keeps the split kernels); 0 = never; 1 = forward, reverse primal and adjoint
- * whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4).  xseg = planes marched per block (0 = chosen by the
+ * whenever the grid allows (nz % 4 == 0, pml_width % 4 == 0, pml_width >= 4, nz - 2 * pml_width >= 8).  xseg = planes marched per block (0 = chosen by the
  * library: 16 or 32 in the forward run; in the reverse run the count in [16, 64] with the fewest waves x (planes + 1)).  Results are bit-identical
  * in every mode (sources that overlap on one cell excepted in the fused reverse run: they are summed before being subtracted).
  * With the fused reverse run the fields left after fdtd_reverse are state 0 on the interior only. */

@@ -85,6 +85,7 @@ struct fdtd_sim {
   StoreDev st{};
   std::vector<float> tables_host;
   std::vector<SrcDev> src_host;
+  bool src_overlap = false;         // two sources add to one cell of one component: applied one launch per source, in index order
   std::vector<float> waves_host;
   int nsrc = 0;
   // E/H buffer pair(s): fb[b][0..2] = E, fb[b][3..5] = H of buffer b; d.E / d.H always point at the current one (cb)
@@ -581,12 +582,21 @@ void launch_sources(fdtd_sim* s, int m_base, const int* step_dev, float sign, in
     maxc = std::max(maxc, (long long)(q.hi[0] - q.lo[0]) * (q.hi[1] - q.lo[1]) * (q.hi[2] - q.lo[2]));
   }
   const int threads = maxc >= 128 ? 128 : 32;
-  const dim3 g((unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024), (unsigned)s->nsrc);
+  const unsigned gx = (unsigned)std::min<long long>((maxc + threads - 1) / threads, 1024);
   Dev dd = s->d;
   if (buffer >= 0)
     for (int c = 0; c < 3; ++c) dd.E[c] = s->fb[buffer][c];
-  LAUNCH(s, k_sources, g, threads, dd, reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc),
-         reinterpret_cast<const float*>(s->ws + s->L.waves), m_base, step_dev, sign, x0, x1);
+  const SrcDev* desc = reinterpret_cast<const SrcDev*>(s->ws + s->L.srcdesc);
+  const float* waves = reinterpret_cast<const float*>(s->ws + s->L.waves);
+  if (!s->src_overlap) {
+    LAUNCH(s, k_sources, dim3(gx, (unsigned)s->nsrc), threads, dd, desc, waves, m_base, step_dev, sign, x0, x1);
+    return;
+  }
+  // overlapping sources: float addition does not commute with itself twice over ((E + a) + b != (E + b) + a), and the order of
+  // atomicAdd from concurrent blocks is not defined.  One launch per source, in index order — the order of the sum in R8.
+  for (int i = 0; i < s->nsrc; ++i)
+    if (s->src_host[i].lo[0] < x1 && s->src_host[i].hi[0] > x0)
+      LAUNCH(s, k_sources, dim3(gx, 1), threads, dd, desc + i, waves, m_base, step_dev, sign, x0, x1);
 }
 void launch_box(fdtd_sim* s, const BoxDev& b, float* rec, int m_base, const int* step_dev, int mode, int half = 2) {
   if ((half == 0 && !(b.mask & 7u)) || (half == 1 && !(b.mask & 56u))) return;
@@ -1028,6 +1038,14 @@ fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int 
     }
   }
   s->nsrc = nsrc;
+  s->src_overlap = false;
+  for (int i = 0; i < nsrc; ++i)
+    for (int j = i + 1; j < nsrc; ++j) {
+      const SrcDev &a = s->src_host[i], &b = s->src_host[j];
+      bool meet = a.comp == b.comp;
+      for (int c = 0; c < 3; ++c) meet = meet && std::max(a.lo[c], b.lo[c]) < std::min(a.hi[c], b.hi[c]);
+      s->src_overlap = s->src_overlap || meet;
+    }
   if (nsrc > 0) {
     CUDA_TRY(s, cudaMemcpyAsync(s->ws + s->L.srcdesc, s->src_host.data(), sizeof(SrcDev) * nsrc, cudaMemcpyHostToDevice,
                                 s->stream));
@@ -1041,8 +1059,11 @@ fdtd_status upload_sources(fdtd_sim* s, int nsteps, const fdtd_source* src, int 
 // Fused forward run (fdtd_fused.cuh).  Step 1's E half-step runs alone, then nsteps-1 fused steps (H half-step of step m +
 // E half-step of step m+1), then the H half-step of the last step.  States are recorded / monitored exactly as in
 // forward_step: state m = (E^m, H^{m+1/2}).
+// the marching kernels treat the first and the last interior group of a row differently (interface cells, z CPML hand-over): a row
+// needs both (found by random-grid testing: nz - 2P = 4 gave wrong fields in forced mode)
+bool fuse_grid_ok(const fdtd_sim* s) { return s->can_fuse && s->n[2] - 2 * s->P >= 8; }
 bool use_fused(const fdtd_sim* s, int nsteps) {
-  if (!s->can_fuse || nsteps < 2 || s->fuse_mode == 0) return false;
+  if (!fuse_grid_ok(s) || nsteps < 2 || s->fuse_mode == 0) return false;
   if (s->fuse_mode == 1) return true;
   // mode -1 (auto): where the marching kernel fills most of one wave of tiles (3 blocks per SM = 444 slots).  Round 1 (k_fused_he
   // beside class-Z slab boxes) paid only with several waves: C4 (7200 tiles) forward 1910 -> 1727 us per step, C3 (392 tiles)
@@ -1053,9 +1074,9 @@ bool use_fused(const fdtd_sim* s, int nsteps) {
 }
 bool fused_adjoint_possible(const fdtd_sim* s) { return s->fuse_adj_mode != 0 && s->fuse_za && s->lb[1][0] != nullptr; }
 bool use_fused_reverse(const fdtd_sim* s) {
-  if (s->fuse_rev_mode == 0 || !s->can_fuse) return false;
+  if (s->fuse_rev_mode == 0 || !fuse_grid_ok(s)) return false;
   if (s->fuse_rev_mode >= 1) return true;
-  if (!(s->use_iz && s->n[2] - 2 * s->P >= 8)) return false;
+  if (!s->use_iz) return false;
   // mode -1 (auto).  Bit-identical to the two-kernel reverse primal; 3.1 GB fewer bytes per step on C4.  History of the primal
   // alone on C4: round 1 (k_fused_he<true>, 1.23 ms per launch) 3406 vs 3395 us per step: off; round 2 with direct loads (1.20 ms)
   // 3148 vs 3094: off; with the cp.async-pipelined kernel (k_fused_ip, 0.98 ms against 0.63 + 0.67 ms for the two inverse kernels)
