@@ -145,7 +145,7 @@ class OracleSim:
         self.monitor = None
 
     def __del__(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:   # at interpreter exit the module globals may be gone already
             lib().orc_destroy(self._h)
             self._h = None
 
