@@ -4,7 +4,7 @@ The hand-built parity cases of test_gpu_parity.py pick their shapes; these draw 
 V = 1 / 2 kernels and the float4 ones, rows of a single group, one to three z tiles), run length, subsampling k, every store
 dtype, both interpolations, store mode, 1-3 random sources with or without amplitude arrays (overlapping ones included), random
 design / monitor / cotangent boxes and component masks, graphs on / off, marching kernels automatic / off / forced, row kernels
-automatic / off / on.  Checked per case: final fields, monitor record and every stored slot bit for bit; loss; gradient within
+automatic / off / on.  Every case runs in a guarded workspace (0xFF fill, guard bands: DESIGN.md section 3).  Checked per case: final fields, monitor record and every stored slot bit for bit; loss; gradient within
 north_star's 1e-4.  1 200 such cases were run once (two defects found and fixed: unordered sums of overlapping sources, marching
 kernels forced onto a single-group interior; both have tests of their own in test_gpu_parity.py); 50 seeded cases stay.
 """
@@ -13,6 +13,7 @@ import pytest
 
 from oracle import fdtd_oracle as orc
 from paper_2603_24027_b200 import workloads as W
+from paper_2603_24027_b200.fdtd import WS_GUARD, WS_REVERSE
 from tests.helpers import gpu_gradient, gpu_sim, make_oracle, oracle_gradient, rel_l2
 
 pytestmark = pytest.mark.gpu
@@ -75,12 +76,14 @@ def test_random_grid_flux_loss_against_oracle(seed):
     mon = ((mx, P, P), (mx + 1, shape[1] - P, shape[2] - P), 0b110110)
     w = W.Workload(f"random{seed}", shape, P, c["T"], c["eps"], (dlo, dhi), srcs, mon, "flux_x", c["dtype"], c["k"])
     graphs, fused, rows = _knobs(rng)
+    tag = f"{shape} P {P} T {w.nsteps} k {w.k} dtype {w.store_dtype} interp {c['interp']} mode {store_mode} graphs {graphs} fused {fused} rows {rows}"
     o = oracle_gradient(w, 32, w.store_dtype, w.k, c["interp"], store_mode=store_mode)
     s = gpu_sim(w, store_mode=store_mode, rows=rows)
     s.set_graphs(graphs)
     s.set_fused(fused, 0)
+    s.set_workspace(w.nsteps, w.store_dtype, w.k, WS_REVERSE | WS_GUARD)    # 0xFF-filled, a guard band behind every sub-array
     g = gpu_gradient(w, w.store_dtype, w.k, interp=c["interp"], sim=s)
-    tag = f"{shape} P {P} T {w.nsteps} k {w.k} dtype {w.store_dtype} interp {c['interp']} mode {store_mode} graphs {graphs} fused {fused} rows {rows}"
+    assert s.guard_check() == 0, tag
     assert np.array_equal(g["final"], o["final"]), tag
     assert np.array_equal(g["mon"], o["mon"]), tag
     assert abs(g["L"] - o["L"]) <= 1e-6 * abs(o["L"]), tag
@@ -136,11 +139,13 @@ def test_random_cotangents_against_oracle(seed):
     s = gpu_sim(w, rows=rows)
     s.set_graphs(graphs)
     s.set_fused(fused, 0)
+    s.set_workspace(T, w.store_dtype, w.k, WS_REVERSE | WS_GUARD)
     gmon = s.forward(T, srcs, w.store_dtype, w.k).cpu().numpy()
     tag = f"{shape} P {P} T {T} k {w.k} dtype {w.store_dtype} interp {c['interp']} mon {mlo}-{mhi} mask {mmask:06b} final {use_final} dmon {use_mon} graphs {graphs} fused {fused} rows {rows}"
     assert np.array_equal(s.fields().cpu().numpy().astype(np.float64), ofinal), tag
     assert np.array_equal(gmon.astype(np.float64), omon), tag
     gg = s.reverse(cot, None if dmon is None else torch.from_numpy(dmon).cuda(), c["interp"]).cpu().numpy().astype(np.float64)
+    assert s.guard_check() == 0, tag
     if np.linalg.norm(og) > 1e-30:
         assert rel_l2(gg, og) <= GRAD_TOL, tag
     else:
